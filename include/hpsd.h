@@ -1,0 +1,132 @@
+/*
+ * hpsd.h -- C ABI of the B200-native Hermitian PSD-cone projection library.
+ *
+ * The operation ("computing an eigendecomposition and setting
+ * all negative eigenvalues to zero"):
+ *
+ *     X = V diag(lambda) V^H   ->   P(X) = V diag(max(lambda, 0)) V^H
+ *
+ * for every Hermitian block of a cone list, on the real-vector encoding vec_R
+ * of Eq. (D10), which preserves the trace inner product
+ * (PAPER.md:1224-1226).  This is the step u = Pi_C(u~ - v) of each ADMM
+ * iteration, Eq. (D33).
+ *
+ * svec layout (the library's own):
+ *   - block b of size n_b starts at double offset sum_{c<b} n_c^2;
+ *   - inside a block the LOWER triangle is stored column by column; column j
+ *     starts at off(j) = j (2 n - j) and holds
+ *       [ X_jj, s Re X_{j+1,j}, s Im X_{j+1,j}, ..., s Re X_{n-1,j}, s Im X_{n-1,j} ],
+ *     s = sqrt(2); n^2 doubles per block.
+ *
+ * Conventions for every entry point
+ *   - "device pointer" = plain CUDA device address on the current device;
+ *     "host pointer"   = ordinary host memory.  No torch types cross this ABI.
+ *   - stream is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - Calls with device pointers only ENQUEUE work on `stream` and return; they
+ *     do not synchronise the host once the library workspace and the plan for
+ *     this size list exist (first call with a new size list allocates and may
+ *     synchronise; later calls are capturable in a CUDA graph).
+ *   - The caller owns every buffer it passes.  The library never frees caller
+ *     memory.  in_svec == out_svec (exact aliasing) is allowed; partial overlap
+ *     is not.
+ *   - Return value: HPSD_OK (0) or a negative HPSD_E* code; never throws.
+ *     Numerical trouble (an iteration that did not converge) cannot be
+ *     returned synchronously: it sets info_dev[b] != 0 on the device.
+ *   - NaN/Inf in the input propagate to the output; no check is made.
+ *   - n_b = 0 blocks are skipped; n_b = 1 gives out = max(in, 0).
+ *   - There is no CPU fallback: without a CUDA device every compute call
+ *     returns HPSD_ECUDA.
+ */
+#ifndef HPSD_H
+#define HPSD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HPSD_OK          0
+#define HPSD_EINVAL     -1   /* bad argument: negative count/size, NULL with non-empty work */
+#define HPSD_EWORKSPACE -2   /* caller workspace too small or misaligned (256 B) */
+#define HPSD_ECUDA      -3   /* a CUDA runtime call or kernel launch failed */
+#define HPSD_EALLOC     -4   /* device or host allocation failed */
+
+/* Library version: major*10000 + minor*100 + patch. */
+int hpsd_version(void);
+
+/* Static string for a return code. */
+const char *hpsd_strerror(int code);
+
+/* Projection of a cone list (Eq. D33).
+ *   n_blocks  number of Hermitian blocks (>= 0)
+ *   sizes     HOST array, sizes[b] = n_b >= 0
+ *   in_svec   DEVICE pointer, sum_b n_b^2 doubles, layout above (read only)
+ *   out_svec  DEVICE pointer, same length (may equal in_svec)
+ *   stream    cudaStream_t
+ * Uses a library-owned, per-device workspace that grows on demand. */
+int hpsd_project(int n_blocks, const int *sizes,
+                 const double *in_svec, double *out_svec, void *stream);
+
+/* Bytes of workspace hpsd_project_ws needs for this size list. */
+int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes);
+
+/* Same as hpsd_project with a caller-owned DEVICE workspace `ws` of at least
+ * hpsd_workspace_size() bytes, 256-byte aligned (e.g. a torch tensor), and an
+ * optional DEVICE array info_dev[n_blocks] (may be NULL) that receives 0 per
+ * block, or a positive code if an iteration in that block did not converge. */
+int hpsd_project_ws(int n_blocks, const int *sizes,
+                    const double *in_svec, double *out_svec,
+                    void *ws, size_t ws_bytes, int *info_dev, void *stream);
+
+/* The same projection through HOST buffers: copies in_host to the device,
+ * projects, copies the result back and synchronises `stream` before
+ * returning.  This is the end-to-end call bench.py's "e2e" times; the paper
+ * pays this host<->device round trip every iteration. */
+int hpsd_project_host(int n_blocks, const int *sizes,
+                      const double *in_host, double *out_host, void *stream);
+
+/* vec_R, Eq. (D10): lower triangle of a column-major complex
+ * FP64 matrix A (DEVICE, interleaved re/im, leading dimension lda >= n, in
+ * complex elements) -> svec (DEVICE, n^2 doubles).  Step S8 of SURVEY.md §8(a). */
+int hpsd_pack(int n, const void *A, int lda, double *svec, void *stream);
+
+/* mat_R, inverse of (D10): svec (DEVICE) -> full Hermitian column-major complex
+ * FP64 matrix A (DEVICE, lda >= n): both triangles written, Im(diag) = 0.
+ * Step S1 of SURVEY.md §8(a). */
+int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream);
+
+/* S2+S3 of SURVEY.md §8(a) alone: reduce one Hermitian block (svec, DEVICE) to a
+ * REAL symmetric tridiagonal matrix unitarily similar to it: diagonal d (DEVICE,
+ * n doubles) and sub-diagonal e (DEVICE, n-1 doubles).  First half of the
+ * "eigendecomposition" of PAPER.md:1536; lets tests check the reduction alone. */
+int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream);
+
+/* Eigenvalues of one Hermitian block given as svec (DEVICE), ascending, into
+ * lambda (DEVICE, n doubles).  Diagnostic/NEXT-2 entry:
+ * lambda_min for the post-processing mix. */
+int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
+
+/* Tuning/testing knob.  "jacobi_max_n" (1..84): blocks with 2 <= n <= value use
+ * the one-CTA Jacobi kernel, larger ones the Householder/D&C path.  Setting it
+ * to 1 forces every block through the large path (used by the edge-case tests). */
+int hpsd_set_option(const char *name, int value);
+
+/* Number of kernel launches the library issued in the last hpsd_project*
+ * call on this thread (bench.py reports it as gpu_launches). */
+int hpsd_last_launch_count(void);
+
+/* Release the library-owned workspace and cached plans of the current device. */
+int hpsd_release(void);
+
+/* Measurement aid for the FP64 roofline denominator, which
+ * MEASURED_PEAKS.json lacks: runs `iters` rounds of independent FP64 FMA
+ * chains (kind 0: DFMA; kind 1: DMMA m8n8k4) on every SM on `stream` and
+ * writes the flop count of one launch to *flops (HOST).  bench.py times the
+ * launch with CUDA events.  Not on the projection path. */
+int hpsd_fp64_peak_probe(int kind, int iters, double *flops, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HPSD_H */

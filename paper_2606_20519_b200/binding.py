@@ -1,0 +1,203 @@
+"""ctypes binding of libhpsd.so -- argument marshalling only (names follow include/hpsd.h)."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libhpsd.so")
+_lib = None
+
+# every symbol include/hpsd.h declares
+EXPORTS = [
+    "hpsd_version", "hpsd_strerror", "hpsd_project", "hpsd_workspace_size", "hpsd_project_ws",
+    "hpsd_project_host", "hpsd_pack", "hpsd_unpack", "hpsd_tridiagonalize", "hpsd_eigvalsh",
+    "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
+]
+
+
+class HpsdError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Load libhpsd.so.  Fails loudly when the extension has not been built
+    (python -m paper_2606_20519_b200.build, or __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise HpsdError(f"CUDA extension missing: {_LIB_PATH} (run __graft_entry__.build()); there is no CPU fallback")
+        lib = ctypes.CDLL(_LIB_PATH)
+        c_int, c_vp, c_sz = ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.hpsd_version.restype = c_int
+        lib.hpsd_strerror.restype = ctypes.c_char_p
+        lib.hpsd_strerror.argtypes = [c_int]
+        lib.hpsd_project.argtypes = [c_int, ip, c_vp, c_vp, c_vp]
+        lib.hpsd_workspace_size.argtypes = [c_int, ip, ctypes.POINTER(c_sz)]
+        lib.hpsd_project_ws.argtypes = [c_int, ip, c_vp, c_vp, c_vp, c_sz, c_vp, c_vp]
+        lib.hpsd_project_host.argtypes = [c_int, ip, c_vp, c_vp, c_vp]
+        lib.hpsd_pack.argtypes = [c_int, c_vp, c_int, c_vp, c_vp]
+        lib.hpsd_unpack.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
+        lib.hpsd_tridiagonalize.argtypes = [c_int, c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_eigvalsh.argtypes = [c_int, c_vp, c_vp, c_vp]
+        lib.hpsd_set_option.argtypes = [ctypes.c_char_p, c_int]
+        lib.hpsd_last_launch_count.restype = c_int
+        lib.hpsd_release.restype = c_int
+        lib.hpsd_fp64_peak_probe.argtypes = [c_int, c_int, ctypes.POINTER(ctypes.c_double), c_vp]
+        for name in EXPORTS:
+            if name not in ("hpsd_strerror",):
+                getattr(lib, name).restype = getattr(lib, name).restype or c_int
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        msg = load_library().hpsd_strerror(rc).decode()
+        raise HpsdError(f"{what} failed: {msg} (code {rc})")
+
+
+def _sizes(sizes: Sequence[int]):
+    arr = (ctypes.c_int * max(len(sizes), 1))(*[int(s) for s in sizes])
+    return arr, len(sizes)
+
+
+def _stream(stream: Optional[torch.cuda.Stream]) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _need_cuda_f64(t: torch.Tensor, name: str):
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise HpsdError(f"{name} must be a contiguous CUDA float64 tensor")
+
+
+def svec_len(sizes: Sequence[int]) -> int:
+    return int(sum(int(n) * int(n) for n in sizes))
+
+
+def version() -> int:
+    return int(load_library().hpsd_version())
+
+
+def set_option(name: str, value: int) -> None:
+    _check(load_library().hpsd_set_option(name.encode(), int(value)), "hpsd_set_option")
+
+
+def last_launch_count() -> int:
+    return int(load_library().hpsd_last_launch_count())
+
+
+def release() -> None:
+    _check(load_library().hpsd_release(), "hpsd_release")
+
+
+def project_(sizes: Sequence[int], in_svec: torch.Tensor, out_svec: torch.Tensor,
+             stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_project: enqueue the projection of a cone list on `stream`; out may alias in."""
+    lib = load_library()
+    _need_cuda_f64(in_svec, "in_svec")
+    _need_cuda_f64(out_svec, "out_svec")
+    total = svec_len(sizes)
+    if in_svec.numel() != total or out_svec.numel() != total:
+        raise HpsdError(f"svec length {in_svec.numel()}/{out_svec.numel()} != sum n^2 = {total}")
+    arr, nb = _sizes(sizes)
+    with torch.cuda.device(in_svec.device):
+        _check(lib.hpsd_project(nb, arr, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)), "hpsd_project")
+    return out_svec
+
+
+def project(sizes: Sequence[int], in_svec: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    return project_(sizes, in_svec, torch.empty_like(in_svec), stream)
+
+
+def workspace_size(sizes: Sequence[int]) -> int:
+    arr, nb = _sizes(sizes)
+    out = ctypes.c_size_t(0)
+    _check(load_library().hpsd_workspace_size(nb, arr, ctypes.byref(out)), "hpsd_workspace_size")
+    return int(out.value)
+
+
+def project_ws(sizes: Sequence[int], in_svec: torch.Tensor, out_svec: torch.Tensor, ws: torch.Tensor,
+               info: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_project_ws: caller-owned workspace (uint8 CUDA tensor) and optional int32 info[n_blocks]."""
+    lib = load_library()
+    _need_cuda_f64(in_svec, "in_svec")
+    _need_cuda_f64(out_svec, "out_svec")
+    if not (ws.is_cuda and ws.dtype == torch.uint8 and ws.is_contiguous()):
+        raise HpsdError("ws must be a contiguous CUDA uint8 tensor")
+    if info is not None and not (info.is_cuda and info.dtype == torch.int32 and info.numel() >= len(sizes)):
+        raise HpsdError("info must be a CUDA int32 tensor with n_blocks entries")
+    arr, nb = _sizes(sizes)
+    with torch.cuda.device(in_svec.device):
+        _check(lib.hpsd_project_ws(nb, arr, in_svec.data_ptr(), out_svec.data_ptr(), ws.data_ptr(), ws.numel(),
+                                   info.data_ptr() if info is not None else None, _stream(stream)), "hpsd_project_ws")
+    return out_svec
+
+
+def project_host(sizes: Sequence[int], in_host: torch.Tensor, out_host: Optional[torch.Tensor] = None,
+                 stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_project_host: HOST float64 tensors in and out (pinned for async copies); synchronises."""
+    lib = load_library()
+    if in_host.is_cuda or in_host.dtype != torch.float64 or not in_host.is_contiguous():
+        raise HpsdError("in_host must be a contiguous CPU float64 tensor")
+    if out_host is None:
+        out_host = torch.empty_like(in_host, pin_memory=in_host.is_pinned())
+    arr, nb = _sizes(sizes)
+    _check(lib.hpsd_project_host(nb, arr, in_host.data_ptr(), out_host.data_ptr(), _stream(stream)), "hpsd_project_host")
+    return out_host
+
+
+def pack(A: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_pack: A is an (n, n) CUDA complex128 tensor holding the matrix in COLUMN-major order,
+    i.e. A[j, i] in torch's row-major indexing is X_ij (pass X.T.contiguous())."""
+    if not (A.is_cuda and A.dtype == torch.complex128 and A.is_contiguous() and A.dim() == 2 and A.shape[0] == A.shape[1]):
+        raise HpsdError("A must be a contiguous square CUDA complex128 tensor (column-major content)")
+    n = A.shape[0]
+    out = torch.empty(n * n, dtype=torch.float64, device=A.device)
+    with torch.cuda.device(A.device):
+        _check(load_library().hpsd_pack(n, A.data_ptr(), n, out.data_ptr(), _stream(stream)), "hpsd_pack")
+    return out
+
+
+def unpack(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_unpack: returns an (n, n) complex128 tensor with column-major content (out[j, i] = X_ij)."""
+    _need_cuda_f64(svec, "svec")
+    if svec.numel() != n * n:
+        raise HpsdError("svec length != n^2")
+    out = torch.empty((n, n), dtype=torch.complex128, device=svec.device)
+    with torch.cuda.device(svec.device):
+        _check(load_library().hpsd_unpack(n, svec.data_ptr(), out.data_ptr(), n, _stream(stream)), "hpsd_unpack")
+    return out
+
+
+def tridiagonalize(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = None):
+    _need_cuda_f64(svec, "svec")
+    d = torch.empty(n, dtype=torch.float64, device=svec.device)
+    e = torch.empty(max(n - 1, 0), dtype=torch.float64, device=svec.device)
+    with torch.cuda.device(svec.device):
+        _check(load_library().hpsd_tridiagonalize(n, svec.data_ptr(), d.data_ptr(), e.data_ptr(), _stream(stream)), "hpsd_tridiagonalize")
+    return d, e
+
+
+def eigvalsh(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    _need_cuda_f64(svec, "svec")
+    lam = torch.empty(n, dtype=torch.float64, device=svec.device)
+    with torch.cuda.device(svec.device):
+        _check(load_library().hpsd_eigvalsh(n, svec.data_ptr(), lam.data_ptr(), _stream(stream)), "hpsd_eigvalsh")
+    return lam
+
+
+def fp64_peak_probe(kind: int, iters: int, stream: Optional[torch.cuda.Stream] = None) -> float:
+    """Enqueue the FP64 probe kernel; returns the flop count of the launch (time it with CUDA events)."""
+    flops = ctypes.c_double(0.0)
+    _check(load_library().hpsd_fp64_peak_probe(kind, iters, ctypes.byref(flops), _stream(stream)), "hpsd_fp64_peak_probe")
+    return float(flops.value)

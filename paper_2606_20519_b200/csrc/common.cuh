@@ -1,0 +1,68 @@
+// common.cuh -- shared device/host helpers for the hpsd CUDA library (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+namespace hpsd {
+
+// complex FP64, interleaved (re, im); 16-byte aligned so one element is one LDG.128/LDS.128
+struct __align__(16) cplx {
+    double x, y;
+};
+
+__host__ __device__ __forceinline__ cplx mk(double x, double y) { cplx r; r.x = x; r.y = y; return r; }
+__host__ __device__ __forceinline__ cplx conj_(cplx a) { return mk(a.x, -a.y); }
+__host__ __device__ __forceinline__ cplx operator+(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
+__host__ __device__ __forceinline__ cplx operator-(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
+__host__ __device__ __forceinline__ cplx operator*(cplx a, cplx b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__host__ __device__ __forceinline__ cplx operator*(double s, cplx a) { return mk(s * a.x, s * a.y); }
+__host__ __device__ __forceinline__ double abs2(cplx a) { return a.x * a.x + a.y * a.y; }
+// acc += a*b
+__device__ __forceinline__ void cfma(cplx &acc, cplx a, cplx b) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a)*b
+__device__ __forceinline__ void cfma_conj(cplx &acc, cplx a, cplx b) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+}
+
+// L2-coherent loads (bypass L1) for data produced by other CTAs of the same kernel
+__device__ __forceinline__ double ldcg_(const double *p) { return __ldcg(p); }
+__device__ __forceinline__ cplx ldcg_(const cplx *p) { const double2 v = __ldcg(reinterpret_cast<const double2 *>(p)); return mk(v.x, v.y); }
+
+constexpr double kSqrt2 = 1.4142135623730951;      // nearest double to sqrt(2)
+constexpr double kEps = 2.220446049250313e-16;     // 2^-52
+
+// svec layout (include/hpsd.h): start of column j of the lower triangle
+__host__ __device__ __forceinline__ size_t svec_col_off(int n, int j) { return (size_t)j * (size_t)(2 * n - j); }
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ cplx warp_sum(cplx v) { return mk(warp_sum(v.x), warp_sum(v.y)); }
+
+// Per-thread launch counter (hpsd_last_launch_count)
+extern thread_local int g_launches;
+
+#define HPSD_CUDA_OK(expr)                                        \
+    do {                                                          \
+        cudaError_t e__ = (expr);                                 \
+        if (e__ != cudaSuccess) return HPSD_ECUDA_;               \
+    } while (0)
+constexpr int HPSD_ECUDA_ = -3;
+
+#define HPSD_LAUNCH_CHECK()                                       \
+    do {                                                          \
+        ::hpsd::g_launches++;                                     \
+        if (cudaPeekAtLastError() != cudaSuccess) return ::hpsd::HPSD_ECUDA_; \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace hpsd

@@ -1,0 +1,383 @@
+// hpsd_api.cu -- C ABI (include/hpsd.h), S0 plan/dispatch of SURVEY.md §8(a):
+// size class per block, svec offsets sum n_k^2, workspace carve-up, launches on the caller's stream.
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <mutex>
+#include <vector>
+
+#include "../../include/hpsd.h"
+#include "kernels.h"
+#include "large.h"
+#include "largepath.h"
+
+namespace hpsd {
+
+thread_local int g_launches = 0;
+
+namespace {
+
+struct Options {
+    int jacobi_max_n = kJacobiMaxN;   // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
+} g_opt;
+
+struct JacobiGroup {
+    int n, count;
+    size_t off_index;   // index (in long long units) of this group's offsets in the descriptor buffer
+    size_t idx_index;   // index (in int units) of this group's info indices
+};
+
+struct LargeBlock { int n; long long off; int idx; };
+
+struct Plan {
+    std::vector<int> sizes;
+    int jacobi_max_n;
+    std::vector<JacobiGroup> groups;
+    std::vector<LargeBlock> large;
+    int n_scalar = 0;
+    size_t scalar_off_index = 0;
+    // device descriptor buffer: [long long offsets ...][int info idx ...]
+    void *desc_dev = nullptr;
+    size_t n_ll = 0, n_int = 0;
+    std::map<int, int2 *> tiles_dev;   // tridiagonalisation tile tables per distinct large n
+    size_t ws_bytes = 0;               // scratch needed by the large path (max over large blocks) + info
+    ~Plan() {
+        if (desc_dev) cudaFree(desc_dev);
+        for (auto &kv : tiles_dev) cudaFree(kv.second);
+    }
+    const long long *ll(size_t i) const { return reinterpret_cast<const long long *>(desc_dev) + i; }
+    const int *ii(size_t i) const { return reinterpret_cast<const int *>(reinterpret_cast<const long long *>(desc_dev) + n_ll) + i; }
+};
+
+struct DeviceState {
+    std::vector<std::unique_ptr<Plan>> plans;
+    void *ws = nullptr; size_t ws_bytes = 0;
+    double *stage_in = nullptr, *stage_out = nullptr; size_t stage_elems = 0;
+    bool inited = false;
+};
+
+std::mutex g_mu;
+std::map<int, DeviceState> g_dev;
+
+int init_device(DeviceState &ds) {
+    if (ds.inited) return 0;
+    int rc = jacobi_init();
+    if (rc) return rc;
+    rc = tridiag_init();
+    if (rc) return rc;
+    rc = largepath_init();
+    if (rc) return rc;
+    ds.inited = true;
+    return 0;
+}
+
+int build_plan(int n_blocks, const int *sizes, Plan &pl) {
+    pl.sizes.assign(sizes, sizes + n_blocks);
+    pl.jacobi_max_n = g_opt.jacobi_max_n;
+    std::vector<long long> ll;
+    std::vector<int> ints;
+    std::map<int, std::vector<std::pair<long long, int>>> by_n;
+    std::vector<long long> scalars;
+    long long off = 0;
+    for (int b = 0; b < n_blocks; ++b) {
+        const int n = sizes[b];
+        if (n == 1) scalars.push_back(off);
+        else if (n >= 2 && n <= pl.jacobi_max_n) by_n[n].push_back({off, b});
+        else if (n > pl.jacobi_max_n) pl.large.push_back({n, off, b});
+        off += (long long)n * n;
+    }
+    pl.n_scalar = (int)scalars.size();
+    pl.scalar_off_index = ll.size();
+    for (long long o : scalars) ll.push_back(o);
+    for (auto &kv : by_n) {
+        JacobiGroup g;
+        g.n = kv.first; g.count = (int)kv.second.size();
+        g.off_index = ll.size(); g.idx_index = ints.size();
+        for (auto &pr : kv.second) { ll.push_back(pr.first); ints.push_back(pr.second); }
+        pl.groups.push_back(g);
+    }
+    pl.n_ll = ll.size(); pl.n_int = ints.size();
+    const size_t bytes = ll.size() * sizeof(long long) + ints.size() * sizeof(int);
+    if (bytes) {
+        if (cudaMalloc(&pl.desc_dev, bytes) != cudaSuccess) return HPSD_EALLOC;
+        std::vector<unsigned char> host(bytes);
+        std::memcpy(host.data(), ll.data(), ll.size() * sizeof(long long));
+        std::memcpy(host.data() + ll.size() * sizeof(long long), ints.data(), ints.size() * sizeof(int));
+        if (cudaMemcpy(pl.desc_dev, host.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) return HPSD_ECUDA;
+    }
+    size_t ws = 0;
+    for (auto &lb : pl.large) {
+        if (!pl.tiles_dev.count(lb.n)) {
+            const size_t nt = tridiag_tile_count(lb.n);
+            std::vector<int2> t(nt);
+            tridiag_fill_tiles(lb.n, t.data());
+            int2 *dptr = nullptr;
+            if (cudaMalloc(&dptr, nt * sizeof(int2)) != cudaSuccess) return HPSD_EALLOC;
+            if (cudaMemcpy(dptr, t.data(), nt * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(dptr); return HPSD_ECUDA; }
+            pl.tiles_dev[lb.n] = dptr;
+        }
+        const size_t w = largepath_ws_bytes(lb.n);
+        if (w > ws) ws = w;
+    }
+    pl.ws_bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
+    return 0;
+}
+
+// Find or create the plan for this size list on the current device.  Creation allocates and
+// synchronises (cudaMalloc/cudaMemcpy); later calls with the same list are launch-only.
+int get_plan(DeviceState &ds, int n_blocks, const int *sizes, Plan **out) {
+    for (auto &p : ds.plans) {
+        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n &&
+            (n_blocks == 0 || std::memcmp(p->sizes.data(), sizes, sizeof(int) * n_blocks) == 0)) {
+            *out = p.get();
+            return 0;
+        }
+    }
+    std::unique_ptr<Plan> pl(new Plan());
+    int rc = build_plan(n_blocks, sizes, *pl);
+    if (rc) return rc;
+    if (ds.plans.size() >= 32) ds.plans.erase(ds.plans.begin());
+    ds.plans.push_back(std::move(pl));
+    *out = ds.plans.back().get();
+    return 0;
+}
+
+int check_args(int n_blocks, const int *sizes, const void *in, const void *out, size_t *total) {
+    if (n_blocks < 0) return HPSD_EINVAL;
+    if (n_blocks > 0 && sizes == nullptr) return HPSD_EINVAL;
+    size_t t = 0;
+    for (int b = 0; b < n_blocks; ++b) {
+        if (sizes[b] < 0 || sizes[b] > 32768) return HPSD_EINVAL;
+        t += (size_t)sizes[b] * sizes[b];
+    }
+    if (t > 0 && (in == nullptr || out == nullptr)) return HPSD_EINVAL;
+    *total = t;
+    return 0;
+}
+
+int run_plan(const Plan &pl, const double *in, double *out, void *ws, int *info_dev, cudaStream_t st) {
+    // info lives at the start of the workspace when the caller gave none
+    int *info = info_dev ? info_dev : reinterpret_cast<int *>(ws);
+    unsigned char *scratch = reinterpret_cast<unsigned char *>(ws) + align_up(pl.sizes.size() * sizeof(int) + 4, 256);
+    if (!pl.sizes.empty()) {
+        if (cudaMemsetAsync(info, 0, pl.sizes.size() * sizeof(int), st) != cudaSuccess) return HPSD_ECUDA;
+    }
+    int rc = 0;
+    if (pl.n_scalar) {
+        rc = launch_clamp_scalars(pl.n_scalar, pl.ll(pl.scalar_off_index), in, out, st);
+        if (rc) return rc;
+    }
+    for (const JacobiGroup &g : pl.groups) {
+        rc = launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st);
+        if (rc) return rc;
+    }
+    for (const LargeBlock &lb : pl.large) {
+        rc = largepath_project(lb.n, in + lb.off, out + lb.off, scratch, pl.tiles_dev.at(lb.n), info + lb.idx, st);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+}  // namespace
+}  // namespace hpsd
+
+using namespace hpsd;
+
+extern "C" {
+
+int hpsd_version(void) { return 100; }
+
+const char *hpsd_strerror(int code) {
+    switch (code) {
+        case HPSD_OK: return "success";
+        case HPSD_EINVAL: return "invalid argument";
+        case HPSD_EWORKSPACE: return "workspace too small or misaligned";
+        case HPSD_ECUDA: return "CUDA runtime or launch failure";
+        case HPSD_EALLOC: return "allocation failed";
+        default: return "unknown error";
+    }
+}
+
+int hpsd_set_option(const char *name, int value) {
+    if (!name) return HPSD_EINVAL;
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (std::strcmp(name, "jacobi_max_n") == 0) {
+        if (value < 1 || value > kJacobiMaxN) return HPSD_EINVAL;
+        g_opt.jacobi_max_n = value;
+        return HPSD_OK;
+    }
+    return HPSD_EINVAL;
+}
+
+int hpsd_last_launch_count(void) { return g_launches; }
+
+int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
+    if (!bytes) return HPSD_EINVAL;
+    size_t total;
+    int rc = check_args(n_blocks, sizes, (void *)1, (void *)1, &total);
+    if (rc) return rc;
+    size_t ws = 0;
+    for (int b = 0; b < n_blocks; ++b)
+        if (sizes[b] > g_opt.jacobi_max_n) {
+            const size_t w = largepath_ws_bytes(sizes[b]);
+            if (w > ws) ws = w;
+        }
+    *bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int) + 4, 256) + 256;
+    return HPSD_OK;
+}
+
+int hpsd_project_ws(int n_blocks, const int *sizes, const double *in_svec, double *out_svec,
+                    void *ws, size_t ws_bytes, int *info_dev, void *stream) {
+    g_launches = 0;
+    size_t total;
+    int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
+    if (rc) return rc;
+    if (n_blocks == 0) return HPSD_OK;
+    size_t need;
+    rc = hpsd_workspace_size(n_blocks, sizes, &need);
+    if (rc) return rc;
+    if (ws == nullptr || ws_bytes < need || (reinterpret_cast<uintptr_t>(ws) & 255u)) return HPSD_EWORKSPACE;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    rc = init_device(ds);
+    if (rc) return rc;
+    Plan *pl;
+    rc = get_plan(ds, n_blocks, sizes, &pl);
+    if (rc) return rc;
+    return run_plan(*pl, in_svec, out_svec, ws, info_dev, (cudaStream_t)stream);
+}
+
+int hpsd_project(int n_blocks, const int *sizes, const double *in_svec, double *out_svec, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
+    if (rc) return rc;
+    if (n_blocks == 0) { g_launches = 0; return HPSD_OK; }
+    size_t need;
+    rc = hpsd_workspace_size(n_blocks, sizes, &need);
+    if (rc) return rc;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    void *ws;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        DeviceState &ds = g_dev[dev];
+        if (ds.ws_bytes < need) {
+            if (ds.ws) cudaFree(ds.ws);   // synchronises; only when the workspace grows
+            ds.ws = nullptr; ds.ws_bytes = 0;
+            if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
+            ds.ws_bytes = need;
+        }
+        ws = ds.ws;
+        need = ds.ws_bytes;
+    }
+    return hpsd_project_ws(n_blocks, sizes, in_svec, out_svec, ws, need, nullptr, stream);
+}
+
+int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, double *out_host, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, in_host, out_host, &total);
+    if (rc) return rc;
+    if (total == 0) { g_launches = 0; return HPSD_OK; }
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    double *din, *dout;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        DeviceState &ds = g_dev[dev];
+        if (ds.stage_elems < total) {
+            if (ds.stage_in) cudaFree(ds.stage_in);
+            if (ds.stage_out) cudaFree(ds.stage_out);
+            ds.stage_in = ds.stage_out = nullptr; ds.stage_elems = 0;
+            if (cudaMalloc(&ds.stage_in, total * sizeof(double)) != cudaSuccess) return HPSD_EALLOC;
+            if (cudaMalloc(&ds.stage_out, total * sizeof(double)) != cudaSuccess) return HPSD_EALLOC;
+            ds.stage_elems = total;
+        }
+        din = ds.stage_in; dout = ds.stage_out;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(din, in_host, total * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return HPSD_ECUDA;
+    rc = hpsd_project(n_blocks, sizes, din, dout, stream);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(out_host, dout, total * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess) return HPSD_ECUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return HPSD_ECUDA;
+    return HPSD_OK;
+}
+
+int hpsd_pack(int n, const void *A, int lda, double *svec, void *stream) {
+    if (n < 0 || (n > 0 && (!A || !svec || lda < n))) return HPSD_EINVAL;
+    g_launches = 0;
+    return launch_pack(n, reinterpret_cast<const cplx *>(A), lda, svec, (cudaStream_t)stream);
+}
+
+int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream) {
+    if (n < 0 || (n > 0 && (!A || !svec || lda < n))) return HPSD_EINVAL;
+    g_launches = 0;
+    return launch_unpack(n, svec, reinterpret_cast<cplx *>(A), lda, 1, (cudaStream_t)stream);
+}
+
+// S2+S3 alone: real symmetric tridiagonal (d[n], e[n-1]) unitarily similar to the block.
+int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream) {
+    if (n < 0 || (n > 0 && (!in_svec || !d)) || (n > 1 && !e)) return HPSD_EINVAL;
+    if (n == 0) return HPSD_OK;
+    g_launches = 0;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    const int sizes[1] = {n};
+    void *ws; Plan *pl;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        DeviceState &ds = g_dev[dev];
+        int rc = init_device(ds);
+        if (rc) return rc;
+        const int saved = g_opt.jacobi_max_n;
+        g_opt.jacobi_max_n = 1;                 // force the large-path plan for any n >= 2
+        rc = get_plan(ds, 1, sizes, &pl);
+        g_opt.jacobi_max_n = saved;
+        if (rc) return rc;
+        const size_t need = largepath_ws_bytes(n) + 1024;
+        if (ds.ws_bytes < need) {
+            if (ds.ws) cudaFree(ds.ws);
+            ds.ws = nullptr; ds.ws_bytes = 0;
+            if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
+            ds.ws_bytes = need;
+        }
+        ws = ds.ws;
+    }
+    if (n == 1) {
+        return cudaMemcpyAsync(d, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    }
+    return largepath_tridiag_only(n, in_svec, d, e, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+}
+
+int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream) {
+    (void)n; (void)in_svec; (void)lambda; (void)stream;
+    return HPSD_EINVAL;   // filled in once S4 lands
+}
+
+int hpsd_release(void) {
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_dev.find(dev);
+    if (it != g_dev.end()) {
+        cudaDeviceSynchronize();
+        DeviceState &ds = it->second;
+        ds.plans.clear();
+        if (ds.ws) cudaFree(ds.ws);
+        if (ds.stage_in) cudaFree(ds.stage_in);
+        if (ds.stage_out) cudaFree(ds.stage_out);
+        ds.ws = nullptr; ds.ws_bytes = 0; ds.stage_in = ds.stage_out = nullptr; ds.stage_elems = 0;
+    }
+    return HPSD_OK;
+}
+
+int hpsd_fp64_peak_probe(int kind, int iters, double *flops, void *stream) {
+    if (iters <= 0 || (kind != 0 && kind != 1)) return HPSD_EINVAL;
+    g_launches = 0;
+    return launch_fp64_probe(kind, iters, flops, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// pack.cu -- S1 (mat_R) and S8 (vec_R) of SURVEY.md §8(a); Eq. (D10).
+// HBM-bound streaming kernels: every svec double is read/written exactly once,
+// consecutive threads walk consecutive rows of one column (coalesced on both sides).
+#include "kernels.h"
+
+namespace hpsd {
+
+// One CTA handles a chunk of one column j: rows i = j .. n-1.
+// svec column j: [X_jj, s Re X_{j+1,j}, s Im X_{j+1,j}, ...]
+template <int FULL>
+__global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__restrict__ sv, cplx *__restrict__ A, int lda) {
+    const int j = blockIdx.y;
+    const double *c = sv + svec_col_off(n, j);
+    for (int i = j + blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        cplx v;
+        if (i == j) {
+            v = mk(c[0], 0.0);
+        } else {
+            const int k = i - j - 1;
+            // division, not multiplication by 1/sqrt2: bit-identical to vec_R^-1 as defined
+            v = mk(c[1 + 2 * k] / kSqrt2, c[2 + 2 * k] / kSqrt2);
+        }
+        A[(size_t)j * lda + i] = v;
+        if (FULL && i != j) A[(size_t)i * lda + j] = conj_(v);
+    }
+}
+
+__global__ void __launch_bounds__(256) pack_kernel(int n, const cplx *__restrict__ A, int lda, double *__restrict__ sv) {
+    const int j = blockIdx.y;
+    double *c = sv + svec_col_off(n, j);
+    for (int i = j + blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const cplx v = A[(size_t)j * lda + i];
+        if (i == j) {
+            c[0] = v.x;
+        } else {
+            const int k = i - j - 1;
+            c[1 + 2 * k] = kSqrt2 * v.x;
+            c[2 + 2 * k] = kSqrt2 * v.y;
+        }
+    }
+}
+
+__global__ void clamp_scalars_kernel(int count, const long long *__restrict__ offs, const double *__restrict__ in, double *__restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) {
+        double v = in[offs[i]];
+        out[offs[i]] = v > 0.0 ? v : (v != v ? v : 0.0);   // NaN propagates
+    }
+}
+
+static dim3 col_grid(int n) {
+    int gx = (n + 1023) / 1024;  // up to 4 rows per thread before the grid-stride loop wraps
+    if (gx < 1) gx = 1;
+    return dim3(gx, n, 1);
+}
+
+int launch_unpack(int n, const double *svec, cplx *A, int lda, int full, cudaStream_t st) {
+    if (n <= 0) return 0;
+    if (n > 65535) return -1;
+    if (full) unpack_kernel<1><<<col_grid(n), 256, 0, st>>>(n, svec, A, lda);
+    else unpack_kernel<0><<<col_grid(n), 256, 0, st>>>(n, svec, A, lda);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_pack(int n, const cplx *A, int lda, double *svec, cudaStream_t st) {
+    if (n <= 0) return 0;
+    if (n > 65535) return -1;
+    pack_kernel<<<col_grid(n), 256, 0, st>>>(n, A, lda, svec);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_clamp_scalars(int count, const long long *offs_dev, const double *in, double *out, cudaStream_t st) {
+    if (count <= 0) return 0;
+    clamp_scalars_kernel<<<(count + 127) / 128, 128, 0, st>>>(count, offs_dev, in, out);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
+}  // namespace hpsd
