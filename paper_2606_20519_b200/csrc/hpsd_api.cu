@@ -148,7 +148,7 @@ int check_args(int n_blocks, const int *sizes, const void *in, const void *out, 
     if (n_blocks > 0 && sizes == nullptr) return HPSD_EINVAL;
     size_t t = 0;
     for (int b = 0; b < n_blocks; ++b) {
-        if (sizes[b] < 0 || sizes[b] > 32768) return HPSD_EINVAL;
+        if (sizes[b] < 0 || sizes[b] > kMaxLargeN) return HPSD_EINVAL;
         t += (size_t)sizes[b] * sizes[b];
     }
     if (t > 0 && (in == nullptr || out == nullptr)) return HPSD_EINVAL;
@@ -319,42 +319,55 @@ int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream) {
 }
 
 // S2+S3 alone: real symmetric tridiagonal (d[n], e[n-1]) unitarily similar to the block.
-int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream) {
-    if (n < 0 || (n > 0 && (!in_svec || !d)) || (n > 1 && !e)) return HPSD_EINVAL;
-    if (n == 0) return HPSD_OK;
-    g_launches = 0;
+int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream);
+
+// shared by hpsd_tridiagonalize / hpsd_eigvalsh: plan + workspace for a single block forced onto the large path
+static int single_large_setup(int n, void **ws_out, Plan **pl_out) {
     int dev;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
     const int sizes[1] = {n};
-    void *ws; Plan *pl;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        DeviceState &ds = g_dev[dev];
-        int rc = init_device(ds);
-        if (rc) return rc;
-        const int saved = g_opt.jacobi_max_n;
-        g_opt.jacobi_max_n = 1;                 // force the large-path plan for any n >= 2
-        rc = get_plan(ds, 1, sizes, &pl);
-        g_opt.jacobi_max_n = saved;
-        if (rc) return rc;
-        const size_t need = largepath_ws_bytes(n) + 1024;
-        if (ds.ws_bytes < need) {
-            if (ds.ws) cudaFree(ds.ws);
-            ds.ws = nullptr; ds.ws_bytes = 0;
-            if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
-            ds.ws_bytes = need;
-        }
-        ws = ds.ws;
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    int rc = init_device(ds);
+    if (rc) return rc;
+    const int saved = g_opt.jacobi_max_n;
+    g_opt.jacobi_max_n = 1;                 // force the large-path plan for any n >= 2
+    rc = get_plan(ds, 1, sizes, pl_out);
+    g_opt.jacobi_max_n = saved;
+    if (rc) return rc;
+    const size_t need = largepath_ws_bytes(n) + 1024;
+    if (ds.ws_bytes < need) {
+        if (ds.ws) cudaFree(ds.ws);
+        ds.ws = nullptr; ds.ws_bytes = 0;
+        if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
+        ds.ws_bytes = need;
     }
-    if (n == 1) {
-        return cudaMemcpyAsync(d, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
-    }
-    return largepath_tridiag_only(n, in_svec, d, e, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+    *ws_out = ds.ws;
+    return 0;
 }
 
 int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream) {
-    (void)n; (void)in_svec; (void)lambda; (void)stream;
-    return HPSD_EINVAL;   // filled in once S4 lands
+    if (n < 0 || n > kMaxLargeN || (n > 0 && (!in_svec || !lambda))) return HPSD_EINVAL;
+    if (n == 0) return HPSD_OK;
+    g_launches = 0;
+    if (n == 1)
+        return cudaMemcpyAsync(lambda, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    void *ws; Plan *pl;
+    int rc = single_large_setup(n, &ws, &pl);
+    if (rc) return rc;
+    return largepath_eigvals(n, in_svec, lambda, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+}
+
+int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream) {
+    if (n < 0 || n > kMaxLargeN || (n > 0 && (!in_svec || !d)) || (n > 1 && !e)) return HPSD_EINVAL;
+    if (n == 0) return HPSD_OK;
+    g_launches = 0;
+    if (n == 1)
+        return cudaMemcpyAsync(d, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    void *ws; Plan *pl;
+    int rc = single_large_setup(n, &ws, &pl);
+    if (rc) return rc;
+    return largepath_tridiag_only(n, in_svec, d, e, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
 }
 
 int hpsd_release(void) {

@@ -26,4 +26,50 @@ size_t tridiag_tile_count(int n);
 void tridiag_fill_tiles(int n, int2 *tiles_host);
 int launch_tridiag(const TridiagWs &w, cudaStream_t st);
 
+
+// ---- stedc.cu (S4) ------------------------------------------------------------
+constexpr int kLeaf = 32;         // D&C leaves are solved by one warp each
+constexpr int kMaxLargeN = 8192;  // shared-memory bound of the deflation scan (24 N bytes)
+
+struct StedcWs {
+    int n, ldz, depth;
+    double *Za, *Zb, *Qw, *U;          // ldz x n each (eigenvector ping-pong, gathered copy, secular vectors)
+    double *lamA, *lamB;               // n: eigenvalue ping-pong
+    double *dmod;                      // n: diagonal with the rank-one tears removed
+    double *dt, *zt;                   // n: sorted non-deflated poles / weights per node segment
+    double *mu, *lamroot, *zhat;       // n
+    double *dval;                      // n: deflated eigenvalues (ascending) per node segment
+    double *rc, *rs;                   // n: deflation rotations
+    int *org, *grow, *gsrc, *dcol, *dest_root, *dest_defl, *rp, *rq;   // n each
+    int *nodeinfo;                     // 8 ints per node: K, k1, k2, k3, nrot, ndefl
+    double *rho;                       // per node
+    int *info;                         // device flag (may be null)
+};
+int stedc_depth(int n);
+size_t stedc_ws_doubles(int n, int ldz);   // helper for carving (doubles incl. int arrays)
+int stedc_init();
+// Eigen-decomposition of the real symmetric tridiagonal (d, e): on return *lam_out / *Z_out point
+// at the ping-pong buffers that hold the ascending eigenvalues and the eigenvectors (ldz x n).
+int launch_stedc(const StedcWs &w, const double *d, const double *e, double **lam_out, double **Z_out, cudaStream_t st);
+
+
+// ---- backherk.cu (S5 back-transform, S6 clamp/scale, S7 HERK, S8 pack) --------------------------
+constexpr int kNBT = 64;          // reflectors per compact-WY block in the back-transformation
+constexpr int kSplitK = 8;        // split of the long K dimension of X = V^H Z
+
+struct BackWs {
+    int n, lda, ldz;
+    const cplx *A;     // reflectors V (lower part, cleaned), lda x n
+    const cplx *tau;   // n (tau[n-1] = 0)
+    cplx *VT;          // lda x n : V_b T_b per block
+    cplx *Tm;          // nblocks x kNBT x kNBT : Gram, then T
+    cplx *Zc;          // ldz x n : complex scaled eigenvectors of the positive part
+    cplx *Xp;          // kSplitK x kNBT x n partial products
+    cplx *X;           // kNBT x n
+    int *cnt;          // [0] = p0 (#lambda <= 0), [1] = kpos
+};
+int backherk_init();
+// lam ascending (n), Zt real eigenvectors of T (ldzt x n); writes the projection's svec to out.
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, double *out, cudaStream_t st);
+
 }  // namespace hpsd

@@ -1,5 +1,5 @@
 // largepath.cu -- large-block pipeline: S1 unpack -> S2/S3 tridiagonalise -> S4 D&C ->
-// S5 back-transform -> S6 clamp/scale -> S7 HERK -> S8 pack.
+// S6 clamp/scale -> S5 back-transform -> S7 HERK -> S8 pack.
 #include "kernels.h"
 #include "large.h"
 #include "largepath.h"
@@ -12,6 +12,8 @@ int g_sms = 0;
 
 struct LargeWs {
     TridiagWs t;
+    StedcWs s;
+    BackWs b;
     size_t bytes;
 };
 
@@ -24,24 +26,57 @@ LargeWs carve(int n, unsigned char *base) {
         off += align_up(bytes, 256);
         return p;
     };
+    auto dbl = [&](size_t cnt) { return reinterpret_cast<double *>(take(sizeof(double) * cnt)); };
+    auto cpx = [&](size_t cnt) { return reinterpret_cast<cplx *>(take(sizeof(cplx) * cnt)); };
+    auto itg = [&](size_t cnt) { return reinterpret_cast<int *>(take(sizeof(int) * cnt)); };
     const int N = (int)align_up((size_t)n, 8);
     const int ts = tridiag_tile_size(n);
     const int nblk = (n + ts - 1) / ts;
     const int G = g_sms > 0 ? g_sms : 148;
+    // ---- S2/S3
     w.t.n = n; w.t.lda = N; w.t.ldw = N; w.t.ldp = nblk * ts;
-    w.t.A = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)N * n));
-    w.t.W = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)N * kNB));
-    w.t.d = reinterpret_cast<double *>(take(sizeof(double) * (size_t)N));
-    w.t.e = reinterpret_cast<double *>(take(sizeof(double) * (size_t)N));
-    w.t.tau = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)N));
-    w.t.PR = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)nblk * w.t.ldp));
-    w.t.PC = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)nblk * w.t.ldp));
-    w.t.part = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)G * (2 * kNB + 1)));
-    w.t.tot = reinterpret_cast<cplx *>(take(sizeof(cplx) * 2 * kNB));
-    w.t.qpart = reinterpret_cast<double *>(take(sizeof(double) * (size_t)G));
+    w.t.A = cpx((size_t)N * n);
+    w.t.W = cpx((size_t)N * kNB);
+    w.t.d = dbl(N);
+    w.t.e = dbl(N);
+    w.t.tau = cpx(N);
+    w.t.PR = cpx((size_t)nblk * w.t.ldp);
+    w.t.PC = cpx((size_t)nblk * w.t.ldp);
+    w.t.part = cpx((size_t)G * (2 * kNB + 1));
+    w.t.tot = cpx(2 * kNB);
+    w.t.qpart = dbl(G);
     w.t.tiles = nullptr;
+    // ---- S4
+    w.s.n = n; w.s.ldz = N; w.s.depth = stedc_depth(n);
+    w.s.Za = dbl((size_t)N * n); w.s.Zb = dbl((size_t)N * n); w.s.Qw = dbl((size_t)N * n); w.s.U = dbl((size_t)N * n);
+    w.s.lamA = dbl(N); w.s.lamB = dbl(N); w.s.dmod = dbl(N); w.s.dt = dbl(N); w.s.zt = dbl(N);
+    w.s.mu = dbl(N); w.s.lamroot = dbl(N); w.s.zhat = dbl(N); w.s.dval = dbl(N); w.s.rc = dbl(N); w.s.rs = dbl(N);
+    w.s.org = itg(N); w.s.grow = itg(N); w.s.gsrc = itg(N); w.s.dcol = itg(N);
+    w.s.dest_root = itg(N); w.s.dest_defl = itg(N); w.s.rp = itg(N); w.s.rq = itg(N);
+    const int maxnodes = 1 << (w.s.depth > 0 ? w.s.depth - 1 : 0);
+    w.s.nodeinfo = itg((size_t)8 * maxnodes);
+    w.s.rho = dbl(maxnodes);
+    w.s.info = nullptr;
+    // ---- S5..S8
+    const int nblocks = (n + kNBT - 1) / kNBT;
+    w.b.n = n; w.b.lda = N; w.b.ldz = N;
+    w.b.A = w.t.A; w.b.tau = w.t.tau;
+    w.b.VT = cpx((size_t)N * n);
+    w.b.Tm = cpx((size_t)nblocks * kNBT * kNBT);
+    w.b.Zc = cpx((size_t)N * n);
+    w.b.Xp = cpx((size_t)kSplitK * kNBT * n);
+    w.b.X = cpx((size_t)kNBT * n);
+    w.b.cnt = itg(8);
     w.bytes = off;
     return w;
+}
+
+int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, cudaStream_t st) {
+    if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
+    int rc = launch_unpack(n, in, w.t.A, w.t.lda, 0, st);
+    if (rc) return rc;
+    return launch_tridiag(w.t, st);
 }
 
 }  // namespace
@@ -50,7 +85,9 @@ int largepath_init() {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HPSD_ECUDA_;
-    return 0;
+    int rc = stedc_init();
+    if (rc) return rc;
+    return backherk_init();
 }
 
 size_t largepath_ws_bytes(int n) { return carve(n, nullptr).bytes; }
@@ -58,18 +95,35 @@ size_t largepath_ws_bytes(int n) { return carve(n, nullptr).bytes; }
 int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsigned char *scratch, const int2 *tiles, cudaStream_t st) {
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
-    int rc = launch_unpack(n, in, w.t.A, w.t.lda, 0, st);
-    if (rc) return rc;
-    rc = launch_tridiag(w.t, st);
+    int rc = reduce_to_tridiagonal(w, n, in, st);
     if (rc) return rc;
     if (cudaMemcpyAsync(d, w.t.d, sizeof(double) * n, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return HPSD_ECUDA_;
     if (n > 1 && cudaMemcpyAsync(e, w.t.e, sizeof(double) * (n - 1), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return HPSD_ECUDA_;
     return 0;
 }
 
+int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *scratch, const int2 *tiles, cudaStream_t st) {
+    LargeWs w = carve(n, scratch);
+    w.t.tiles = tiles;
+    int rc = reduce_to_tridiagonal(w, n, in, st);
+    if (rc) return rc;
+    double *lam, *Z;
+    rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(lambda, lam, sizeof(double) * n, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return HPSD_ECUDA_;
+    return 0;
+}
+
 int largepath_project(int n, const double *in, double *out, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st) {
-    (void)n; (void)in; (void)out; (void)scratch; (void)tiles; (void)info; (void)st;
-    return -1;   // S4..S8 land next
+    LargeWs w = carve(n, scratch);
+    w.t.tiles = tiles;
+    w.s.info = info;
+    int rc = reduce_to_tridiagonal(w, n, in, st);
+    if (rc) return rc;
+    double *lam, *Z;
+    rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
+    if (rc) return rc;
+    return launch_back_herk(w.b, lam, Z, w.s.ldz, out, st);
 }
 
 }  // namespace hpsd

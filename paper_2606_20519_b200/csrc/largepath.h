@@ -9,4 +9,6 @@ size_t largepath_ws_bytes(int n);
 int largepath_project(int n, const double *in, double *out, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st);
 // S1+S2+S3 only (diagnostic / eigenvalue-only entry points).
 int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsigned char *scratch, const int2 *tiles, cudaStream_t st);
+// S1..S4: ascending eigenvalues only.
+int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *scratch, const int2 *tiles, cudaStream_t st);
 }  // namespace hpsd
