@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Hermitian PSD-cone projection (the hot path of arxiv/paper_2606_20519).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (S0..S10) over one cone list of
+BASELINE.json's configs (default: config 3, the single n=625 block the metric is quoted on).
+Prints ONE JSON line (see the task contract): `value` = projections/s with inputs resident in HBM,
+`e2e` = the same through hpsd_project_host with host buffers, `roofline` for the dominant kernel
+(live CUDA-event stage timers inside the library), `cpu_baseline` = the oracle on the host cores.
+`--impl reference` times the CPU oracle alone.  Multi-GPU: a single block does not shard
+(DESIGN.md §Multi-GPU): N ranks run N independent replicas ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402  (seeded input generators only; none of the method's arithmetic)
+
+METRIC = "hermitian_psd_projections_per_sec"
+UNIT = "projections/s"
+L2_FLUSH_BYTES = 512 << 20
+
+
+def f_alg(n: int, kpos: int) -> float:
+    """Algorithmic real flops of one projection: reduction + tridiagonal D&C +
+    one back-transform of the kpos kept columns + HERK.  Extra work of a variant is not counted."""
+    if n <= 1:
+        return 0.0
+    return (16.0 / 3.0) * n ** 3 + (4.0 / 3.0) * n ** 3 + 8.0 * n * n * kpos + 4.0 * n * n * kpos
+
+
+# stage -> the part of f_alg that stage carries (flops), used for the dominant-kernel roofline
+def stage_flops(stage: str, sizes, kpos, jmax: int) -> float:
+    tot = 0.0
+    for n, k in zip(sizes, kpos):
+        large = n > jmax
+        if stage == "S2S3_tridiag_panel" and large:
+            tot += (8.0 / 3.0) * n ** 3          # the mat-vec half of the reduction
+        elif stage == "S2_her2k_trailing" and large:
+            tot += (8.0 / 3.0) * n ** 3          # the rank-2k half
+        elif stage == "S4_stedc" and large:
+            tot += (4.0 / 3.0) * n ** 3
+        elif stage == "S5S6_backtransform" and large:
+            tot += 8.0 * n * n * k
+        elif stage == "S7S8_herk_pack" and large:
+            tot += 4.0 * n * n * k
+        elif stage == "S9S10_jacobi" and 2 <= n <= jmax:
+            tot += f_alg(n, k)
+    return tot
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            if len(r) < 8:
+                continue
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg: int):
+    """A bounded sample of the workload for the CPU oracle (about 10-30 s): (sizes, matrices, scale,
+    description); time(full workload) ~ scale * time(sample) by the n^3 cost law."""
+    w = workloads.make(cfg) if cfg in (1, 2, 3) else None
+    if cfg == 1:
+        return w.sizes, [b.X for b in w.blocks], 1.0, "the whole workload (one n=16 block), repeated"
+    if cfg == 2:
+        return w.sizes[:64], [b.X for b in w.blocks[:64]], 4.0, "64 of the 256 n=81 blocks; time x4"
+    if cfg == 3:
+        return w.sizes, [b.X for b in w.blocks], 1.0, "the whole workload (one n=625 block)"
+    if cfg == 4:
+        rng = np.random.default_rng(workloads.BASE_SEED + 4)
+        b = workloads.gue_like(rng, 1296, 1.0 / 36.0)
+        scale = (1296.0 ** 3 + 2401.0 ** 3 + 64 * 36.0 ** 3) / 1296.0 ** 3
+        return [1296], [b.X], scale, f"the n=1296 block only; time x{scale:.3f} (sum n^3 / 1296^3)"
+    rng = np.random.default_rng(workloads.BASE_SEED + 5)
+    b = workloads.from_spectrum(rng, workloads.spectrum_clustered(rng, 1024, n_big=16, n_clusters=8, mult=32))
+    return [1024], [b.X], 64.0, "a config-5-type block (clusters of 32 repeats) at n=1024; time x64 ((4096/1024)^3)"
+
+
+def run_oracle(cfg: int, steps: int, warmup: int, min_seconds: float = 0.0):
+    """Times the oracle as it stands on the host cores.  Returns (projections/s, s per step, cores, sample)."""
+    import oracle
+    oracle.build()
+    sizes, mats, scale, desc = oracle_sample(cfg)
+    sv = np.concatenate([oracle.pack(m) for m in mats])
+    threads = oracle.max_threads()
+    for _ in range(warmup):
+        oracle.project(sizes, sv, nthreads=threads)
+    times = []
+    t_all = time.perf_counter()
+    while len(times) < steps or (time.perf_counter() - t_all) < min_seconds:
+        t0 = time.perf_counter()
+        oracle.project(sizes, sv, nthreads=threads)
+        times.append(time.perf_counter() - t0)
+        if len(times) >= max(steps, 1) and min_seconds <= 0.0:
+            break
+    per_step = scale * sum(times) / len(times)
+    return 1.0 / per_step, per_step, threads, f"{desc}; {len(times)} timed run(s), {threads} OpenMP thread(s)"
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the n=4096 ms/projection figure")
+    ap.add_argument("--all-configs", action="store_true", help="also time every other BASELINE.json config (table)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = args.config
+    wname = {1: "cfg1: 1 x n=16 Haar/Gaussian spectrum", 2: "cfg2: 256 x n=81 GUE-like",
+             3: "cfg3: 1 x n=625 ADMM-like low-rank spectrum", 4: "cfg4: n=1296 + n=2401 + 64 x n=36 GUE-like",
+             5: "cfg5: 1 x n=4096 clustered spectrum"}[cfg]
+
+    # ------------------------------------------------------------------ reference arm = the oracle
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        value, per_step, threads, sample = run_oracle(cfg, max(args.steps, 1), min(args.warmup, 1))
+        print(json.dumps({
+            "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wname, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+        }))
+        return
+
+    # ------------------------------------------------------------------ our arm
+    import torch
+    import paper_2606_20519_b200 as hp
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    hp.load_library()
+    jmax = 84
+
+    def device_inputs(c):
+        w = workloads.make(c)
+        parts = [hp.pack(torch.from_numpy(np.ascontiguousarray(b.X.T)).to(dev)) for b in w.blocks]
+        return w.sizes, torch.cat(parts)
+
+    def count_pos(sizes, sv):
+        out, off = [], 0
+        for n in sizes:
+            if n >= 2:
+                lam = hp.eigvalsh(sv[off:off + n * n].clone(), n)
+                out.append(int((lam > 0).sum().item()))
+            else:
+                out.append(int(n == 1 and sv[off].item() > 0))
+            off += n * n
+        return out
+
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def time_device(sizes, sv, out, steps, warmup):
+        for _ in range(warmup):
+            hp.project_(sizes, sv, out)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        for a, b in ev:
+            flush.zero_()                       # evict L2 between timed iterations
+            a.record()
+            hp.project_(sizes, sv, out)
+            b.record()
+        barrier()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        return sum(ms), ms
+
+    def time_e2e(sizes, h_in, h_out, steps, warmup):
+        for _ in range(warmup):
+            hp.project_host(sizes, h_in, h_out)
+        barrier()
+        tot = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            hp.project_host(sizes, h_in, h_out)   # H2D + projection + D2H + stream sync inside
+            tot += time.perf_counter() - t0
+        barrier()
+        return tot * 1e3
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    sizes, sv = device_inputs(cfg)
+    out = torch.empty_like(sv)
+    kpos = count_pos(sizes, sv)
+    K, W = max(args.steps, 1), args.warmup
+
+    # FP64 peak of this GPU, measured here (MEASURED_PEAKS.json has no FP64 figure): DFMA and DMMA chains
+    def probe(kind):
+        best = 0.0
+        for it in range(4):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fl = hp.fp64_peak_probe(kind, 4096)
+            b.record()
+            torch.cuda.synchronize()
+            if it:
+                best = max(best, fl / (a.elapsed_time(b) * 1e-3) / 1e12)
+        return best
+    peak_dfma, peak_dmma = probe(0), probe(1)
+    fp64_peak = max(peak_dfma, peak_dmma)
+
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")
+    phys = int(vis[local_rank]) if local_rank < len(vis) and vis[local_rank].isdigit() else local_rank
+    sampler = ClockSampler(phys)
+    sampler.start()
+    total_ms, per = time_device(sizes, sv, out, K, W)
+    clocks = sampler.stop()
+    launches_per_step = hp.last_launch_count()
+    total_ms = max_over_ranks(total_ms)
+    ms_per_step = total_ms / K
+    value = world * 1.0 / (ms_per_step * 1e-3)      # cone-list projections per second, all replicas
+
+    # stage timers: same K steps again with the library's CUDA-event spans on the launching stream
+    hp.set_option("profile", 1)
+    stage_ms = {}
+    for _ in range(K):
+        flush.zero_()
+        hp.project_(sizes, sv, out)
+        for name, (ms, spans) in hp.profile_read().items():
+            acc = stage_ms.setdefault(name, [0.0, 0])
+            acc[0] += ms; acc[1] += spans
+    hp.set_option("profile", 0)
+    stages = {k: {"ms_per_step": v[0] / K, "launch_spans_per_step": v[1] / K} for k, v in stage_ms.items() if v[1]}
+    dom = max(stages, key=lambda k: stages[k]["ms_per_step"])
+    dom_ms = stages[dom]["ms_per_step"]
+    dom_spans = max(stages[dom]["launch_spans_per_step"], 1)
+    dom_flops = stage_flops(dom, sizes, kpos, jmax)
+    achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    F = sum(f_alg(n, k) for n, k in zip(sizes, kpos))
+    roofline = {
+        "kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+        "frac": achieved / fp64_peak if fp64_peak else None, "traffic": None,
+        "avg_launch_ms": dom_ms / dom_spans, "launches_per_step": dom_spans,
+        "share_of_step": dom_ms / sum(s["ms_per_step"] for s in stages.values()),
+        "peak_source": f"measured in this run by hpsd_fp64_peak_probe: DFMA {peak_dfma:.1f}, DMMA {peak_dmma:.1f} TFLOP/s "
+                       "(MEASURED_PEAKS.json has no FP64 figure)",
+        "algorithmic_flops_per_step": dom_flops,
+        "whole_path": {"f_alg_flops": F, "achieved_tflops": F / (ms_per_step * 1e-3) / 1e12,
+                       "frac_of_fp64_peak": F / (ms_per_step * 1e-3) / 1e12 / fp64_peak if fp64_peak else None,
+                       "hbm_floor_ms": 16.0 * sum(n * n for n in sizes) / 6553.9e9 * 1e3},
+        "stages": stages,
+    }
+
+    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    h_in = sv.cpu().pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    e2e_ms = max_over_ranks(time_e2e(sizes, h_in, h_out, K, W)) / K
+    e2e = {"value": world / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+           "h2d_bytes_per_step": int(sv.numel() * 8), "d2h_bytes_per_step": int(sv.numel() * 8)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "sizes": sizes if len(sizes) <= 4 else f"{len(sizes)} blocks",
+                   "positive_eigenvalues": kpos if len(kpos) <= 4 else None,
+                   "l2": f"L2 flushed between timed iterations by writing a {L2_FLUSH_BYTES >> 20} MiB buffer",
+                   "parallelism": "replicas only (a single block does not shard)" if world > 1 else "single GPU"},
+        "ms_min": min(per), "ms_median": statistics.median(per),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * K, "launches_per_step": launches_per_step,
+        "roofline": roofline,
+    }
+
+    if rank == 0 and world == 1:
+        extra = {}
+        others = []
+        if args.all_configs:
+            others = [c for c in (1, 2, 3, 4, 5) if c != cfg]
+        elif not args.no_secondary and cfg != 5:
+            others = [5]                         # the metric's second clause: ms/projection at n=4096
+        for c in others:
+            s2, v2 = device_inputs(c)
+            o2 = torch.empty_like(v2)
+            k2 = count_pos(s2, v2)
+            steps2 = 3 if c in (4, 5) else 10
+            t2, per2 = time_device(s2, v2, o2, steps2, 2)
+            F2 = sum(f_alg(n, k) for n, k in zip(s2, k2))
+            extra[f"cfg{c}"] = {"ms_per_projection": t2 / steps2, "ms_min": min(per2), "f_alg_gflop": F2 / 1e9,
+                                "frac_of_fp64_peak": F2 / (t2 / steps2 * 1e-3) / 1e12 / fp64_peak,
+                                "launches": hp.last_launch_count()}
+            del v2, o2
+        line["other_configs"] = extra
+        if "cfg5" in extra:
+            line["ms_per_projection_n4096"] = extra["cfg5"]["ms_per_projection"]
+        if not args.no_cpu_baseline:
+            v, per_step, threads, sample = run_oracle(cfg, 1, 0, min_seconds=10.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                                    "ms_per_projection": per_step * 1e3}
+        line["paper_context"] = ("paper (Tesla T4, JAX eigh only, complex128): 0.06 s at n=625, 6.33 s at n=4096 "
+                                 "(PAPER.md:1515-1518); whole SDP six-fold vs CPU SCS (PAPER.md:1554); other hardware, context only")
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

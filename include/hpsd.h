@@ -107,10 +107,22 @@ int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void
  * lambda_min for the post-processing mix. */
 int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
 
-/* Tuning/testing knob.  "jacobi_max_n" (1..84): blocks with 2 <= n <= value use
- * the one-CTA Jacobi kernel, larger ones the Householder/D&C path.  Setting it
- * to 1 forces every block through the large path (used by the edge-case tests). */
+/* Tuning/testing knobs.
+ *   "jacobi_max_n" (1..84): blocks with 2 <= n <= value use the one-CTA Jacobi
+ *       kernel, larger ones the Householder/D&C path.  Setting it to 1 forces
+ *       every block through the large path (used by the edge-case tests).
+ *   "profile" (0/1): record CUDA events on the caller's stream around every stage
+ *       of the path (S1..S10) for hpsd_profile_read.  Off by default. */
 int hpsd_set_option(const char *name, int value);
+
+/* Stage timers (measurement): number of stages, their names, and the
+ * device time in milliseconds each stage took in the LAST hpsd_project* call made with
+ * "profile" = 1 (summed over its launches; spans[i] = number of timed spans, may be
+ * NULL).  ms and spans are HOST arrays of at least hpsd_profile_stage_count() entries.
+ * hpsd_profile_read synchronises on the recorded events. */
+int hpsd_profile_stage_count(void);
+const char *hpsd_profile_stage_name(int stage);
+int hpsd_profile_read(double *ms, int *spans, int n);
 
 /* Number of kernel launches the library issued in the last hpsd_project*
  * call on this thread (bench.py reports it as gpu_launches). */

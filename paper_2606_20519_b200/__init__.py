@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     project_,
     project_host,
     project_ws,
+    profile_read,
     release,
     set_option,
     svec_len,

@@ -16,6 +16,7 @@ EXPORTS = [
     "hpsd_version", "hpsd_strerror", "hpsd_project", "hpsd_workspace_size", "hpsd_project_ws",
     "hpsd_project_host", "hpsd_pack", "hpsd_unpack", "hpsd_tridiagonalize", "hpsd_eigvalsh",
     "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
+    "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read",
 ]
 
 
@@ -52,8 +53,11 @@ def load_library():
         lib.hpsd_last_launch_count.restype = c_int
         lib.hpsd_release.restype = c_int
         lib.hpsd_fp64_peak_probe.argtypes = [c_int, c_int, ctypes.POINTER(ctypes.c_double), c_vp]
+        lib.hpsd_profile_stage_name.restype = ctypes.c_char_p
+        lib.hpsd_profile_stage_name.argtypes = [c_int]
+        lib.hpsd_profile_read.argtypes = [ctypes.POINTER(ctypes.c_double), ip, c_int]
         for name in EXPORTS:
-            if name not in ("hpsd_strerror",):
+            if name not in ("hpsd_strerror", "hpsd_profile_stage_name"):
                 getattr(lib, name).restype = getattr(lib, name).restype or c_int
         _lib = lib
     return _lib
@@ -194,6 +198,16 @@ def eigvalsh(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = N
     with torch.cuda.device(svec.device):
         _check(load_library().hpsd_eigvalsh(n, svec.data_ptr(), lam.data_ptr(), _stream(stream)), "hpsd_eigvalsh")
     return lam
+
+
+def profile_read() -> dict:
+    """hpsd_profile_read: {stage name: (milliseconds, spans)} of the last call made with option profile=1."""
+    lib = load_library()
+    n = int(lib.hpsd_profile_stage_count())
+    ms = (ctypes.c_double * n)()
+    spans = (ctypes.c_int * n)()
+    _check(lib.hpsd_profile_read(ms, spans, n), "hpsd_profile_read")
+    return {lib.hpsd_profile_stage_name(i).decode(): (float(ms[i]), int(spans[i])) for i in range(n)}
 
 
 def fp64_peak_probe(kind: int, iters: int, stream: Optional[torch.cuda.Stream] = None) -> float:

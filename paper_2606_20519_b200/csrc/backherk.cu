@@ -10,6 +10,7 @@
 #include "kernels.h"
 #include "gemm.cuh"
 #include "large.h"
+#include "prof.h"
 
 namespace hpsd {
 
@@ -186,6 +187,7 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     if (rc) return rc;
     const int nblocks = (n + kNBT - 1) / kNBT;
     const int nt = (n + 63) / 64;
+    prof_begin(ST_BACK, st);
     count_pos_kernel<<<1, 32, 0, st>>>(n, lam, w.cnt);
     HPSD_LAUNCH_CHECK();
     scale_convert_kernel<<<dim3((n + 1023) / 1024, n), 256, 0, st>>>(n, lam, Zt, ldzt, w.Zc, w.ldz, w.cnt);
@@ -207,7 +209,10 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
         bt_update_kernel<<<dim3((m + 63) / 64, nt), BG_THREADS, kSmemMK, st>>>(w, b);
         HPSD_LAUNCH_CHECK();
     }
+    prof_end(ST_BACK, st);
+    prof_begin(ST_HERK_PACK, st);
     herk_pack_kernel<<<dim3(nt, nt), BG_THREADS, kSmemMM, st>>>(w, out);
+    prof_end(ST_HERK_PACK, st);
     HPSD_LAUNCH_CHECK();
     return 0;
 }

@@ -11,10 +11,39 @@
 #include "kernels.h"
 #include "large.h"
 #include "largepath.h"
+#include "prof.h"
 
 namespace hpsd {
 
 thread_local int g_launches = 0;
+bool g_profile = false;
+
+// ---- stage timers (prof.h) -----------------------------------------------------------------
+namespace {
+struct ProfSpan { int stage; cudaEvent_t a, b; };
+std::vector<ProfSpan> g_spans;          // spans of the last hpsd_project* call
+std::vector<cudaEvent_t> g_event_pool;
+size_t g_event_next = 0;
+cudaEvent_t prof_event() {
+    if (g_event_next == g_event_pool.size()) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        g_event_pool.push_back(e);
+    }
+    return g_event_pool[g_event_next++];
+}
+void prof_reset() { g_spans.clear(); g_event_next = 0; }
+}  // namespace
+
+void prof_begin_(int stage, cudaStream_t st) {
+    ProfSpan sp{stage, prof_event(), prof_event()};
+    cudaEventRecord(sp.a, st);
+    g_spans.push_back(sp);
+}
+void prof_end_(int stage, cudaStream_t st) {
+    for (size_t i = g_spans.size(); i-- > 0;)
+        if (g_spans[i].stage == stage) { cudaEventRecord(g_spans[i].b, st); return; }
+}
 
 namespace {
 
@@ -164,12 +193,17 @@ int run_plan(const Plan &pl, const double *in, double *out, void *ws, int *info_
         if (cudaMemsetAsync(info, 0, pl.sizes.size() * sizeof(int), st) != cudaSuccess) return HPSD_ECUDA;
     }
     int rc = 0;
+    if (g_profile) prof_reset();
     if (pl.n_scalar) {
+        prof_begin(ST_SCALAR, st);
         rc = launch_clamp_scalars(pl.n_scalar, pl.ll(pl.scalar_off_index), in, out, st);
+        prof_end(ST_SCALAR, st);
         if (rc) return rc;
     }
     for (const JacobiGroup &g : pl.groups) {
+        prof_begin(ST_JACOBI, st);
         rc = launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st);
+        prof_end(ST_JACOBI, st);
         if (rc) return rc;
     }
     for (const LargeBlock &lb : pl.large) {
@@ -202,6 +236,10 @@ const char *hpsd_strerror(int code) {
 int hpsd_set_option(const char *name, int value) {
     if (!name) return HPSD_EINVAL;
     std::lock_guard<std::mutex> lk(g_mu);
+    if (std::strcmp(name, "profile") == 0) {
+        g_profile = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "jacobi_max_n") == 0) {
         if (value < 1 || value > kJacobiMaxN) return HPSD_EINVAL;
         g_opt.jacobi_max_n = value;
@@ -211,6 +249,28 @@ int hpsd_set_option(const char *name, int value) {
 }
 
 int hpsd_last_launch_count(void) { return g_launches; }
+
+int hpsd_profile_stage_count(void) { return ST_COUNT; }
+
+const char *hpsd_profile_stage_name(int stage) {
+    static const char *names[ST_COUNT] = {"S1_unpack", "S2S3_tridiag_panel", "S2_her2k_trailing", "S4_stedc",
+                                          "S5S6_backtransform", "S7S8_herk_pack", "S9S10_jacobi", "n1_clamp"};
+    return (stage >= 0 && stage < ST_COUNT) ? names[stage] : "";
+}
+
+int hpsd_profile_read(double *ms, int *spans, int n) {
+    if (n < ST_COUNT || !ms) return HPSD_EINVAL;
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (int i = 0; i < ST_COUNT; ++i) { ms[i] = 0.0; if (spans) spans[i] = 0; }
+    for (const ProfSpan &sp : g_spans) {
+        if (cudaEventSynchronize(sp.b) != cudaSuccess) return HPSD_ECUDA;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, sp.a, sp.b) != cudaSuccess) return HPSD_ECUDA;
+        ms[sp.stage] += t;
+        if (spans) spans[sp.stage]++;
+    }
+    return HPSD_OK;
+}
 
 int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     if (!bytes) return HPSD_EINVAL;

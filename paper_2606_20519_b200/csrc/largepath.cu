@@ -3,6 +3,7 @@
 #include "kernels.h"
 #include "large.h"
 #include "largepath.h"
+#include "prof.h"
 
 namespace hpsd {
 
@@ -74,7 +75,9 @@ LargeWs carve(int n, unsigned char *base) {
 int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, cudaStream_t st) {
     if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
+    prof_begin(ST_UNPACK, st);
     int rc = launch_unpack(n, in, w.t.A, w.t.lda, 0, st);
+    prof_end(ST_UNPACK, st);
     if (rc) return rc;
     return launch_tridiag(w.t, st);
 }
@@ -121,7 +124,9 @@ int largepath_project(int n, const double *in, double *out, unsigned char *scrat
     int rc = reduce_to_tridiagonal(w, n, in, st);
     if (rc) return rc;
     double *lam, *Z;
+    prof_begin(ST_STEDC, st);
     rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
+    prof_end(ST_STEDC, st);
     if (rc) return rc;
     return launch_back_herk(w.b, lam, Z, w.s.ldz, out, st);
 }

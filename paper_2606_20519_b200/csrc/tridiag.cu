@@ -16,6 +16,7 @@
 #include "kernels.h"
 #include "gemm.cuh"
 #include "large.h"
+#include "prof.h"
 
 namespace cg = cooperative_groups;
 
@@ -470,8 +471,10 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
         void *args[] = {&p};
         const size_t smem = panel_smem_bytes(ts);
         cudaError_t e;
+        prof_begin(ST_PANEL, st);
         if (ts == 64) e = cudaLaunchCooperativeKernel((void *)tridiag_panel_kernel<64>, dim3(p.G), dim3(kPanelThreads), args, smem, st);
         else e = cudaLaunchCooperativeKernel((void *)tridiag_panel_kernel<32>, dim3(p.G), dim3(kPanelThreads), args, smem, st);
+        prof_end(ST_PANEL, st);
         g_launches++;
         if (e != cudaSuccess) return HPSD_ECUDA_;
         const int m2 = n - (j0 + kNB);
@@ -485,7 +488,9 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
             Her2kEpi epi{w.A + (size_t)(j0 + kNB) * w.lda + (j0 + kNB), w.lda};
             const int nt = (m2 + 63) / 64;
             constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
+            prof_begin(ST_HER2K, st);
             her2k_kernel<<<dim3(nt, nt), H2_WM * H2_WN * 32, h2, st>>>(gp, epi);
+            prof_end(ST_HER2K, st);
             HPSD_LAUNCH_CHECK();
         }
     }

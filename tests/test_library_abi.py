@@ -1,0 +1,86 @@
+"""CPU-side checks of the boundary: the C-ABI library builds for sm_100a, loads, and exports every
+symbol include/hpsd.h declares; argument errors are reported without a GPU; the product has no CPU
+fallback and never touches oracle/."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_20519_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "hpsd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(hpsd_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_all_exported(lib):
+    from paper_2606_20519_b200 import binding
+    names = declared_symbols()
+    assert len(names) >= 14
+    assert sorted(binding.EXPORTS) == names
+    for name in names:
+        assert getattr(lib, name) is not None, name
+
+
+def test_version_and_strerror(lib):
+    assert lib.hpsd_version() >= 100
+    assert lib.hpsd_strerror(0) == b"success"
+    assert b"argument" in lib.hpsd_strerror(-1)
+    assert b"workspace" in lib.hpsd_strerror(-2)
+    assert b"CUDA" in lib.hpsd_strerror(-3)
+    assert lib.hpsd_strerror(-99) == b"unknown error"
+
+
+def test_argument_errors_without_gpu(lib):
+    bad = (ctypes.c_int * 2)(4, -1)
+    sz = ctypes.c_size_t(0)
+    assert lib.hpsd_workspace_size(2, bad, ctypes.byref(sz)) == -1
+    assert lib.hpsd_workspace_size(-1, bad, ctypes.byref(sz)) == -1
+    ok = (ctypes.c_int * 3)(16, 625, 36)
+    assert lib.hpsd_workspace_size(3, ok, ctypes.byref(sz)) == 0
+    assert sz.value > 16 * 625 * 625          # at least one complex copy of the large block
+    small = (ctypes.c_int * 2)(16, 36)
+    sz2 = ctypes.c_size_t(0)
+    assert lib.hpsd_workspace_size(2, small, ctypes.byref(sz2)) == 0
+    assert sz2.value < 4096                   # Jacobi blocks need no scratch, only the info words
+    assert lib.hpsd_set_option(b"no_such_option", 1) == -1
+    assert lib.hpsd_set_option(b"jacobi_max_n", 0) == -1
+    assert lib.hpsd_set_option(b"jacobi_max_n", 84) == 0
+    assert lib.hpsd_project(0, None, None, None, None) == 0       # empty list: nothing to do
+
+
+def test_no_cpu_fallback_without_device(lib):
+    """Without a CUDA device every compute call fails loudly (include/hpsd.h)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    n = (ctypes.c_int * 1)(4)
+    buf = (ctypes.c_double * 16)()
+    assert lib.hpsd_project_host(1, n, buf, buf, None) < 0
+    import paper_2606_20519_b200 as hp
+    with pytest.raises(hp.HpsdError):
+        hp.project([4], torch.zeros(16, dtype=torch.float64))
+
+
+def test_product_never_imports_oracle():
+    """oracle/ is test infrastructure: nothing under the package may import, link or run it."""
+    pkg = os.path.join(ROOT, "paper_2606_20519_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "hpsd_oracle" not in txt and "libhpsd_oracle" not in txt, f
+    otxt = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "hpsd_oracle.c")).read()
+    assert not re.search(r"^\s*(import|from)\s+paper_2606_20519_b200\b", otxt, flags=re.M)
+    assert '#include "' not in otxt
