@@ -35,7 +35,9 @@ struct StedcWs {
     int n, ldz, depth;
     double *Za, *Zb, *Qw, *U;          // ldz x n each (eigenvector ping-pong, gathered copy, secular vectors)
     double *lamA, *lamB;               // n: eigenvalue ping-pong
-    double *dmod;                      // n: diagonal with the rank-one tears removed
+    double *dmod;                      // n: scaled diagonal with the rank-one tears removed
+    double *es;                        // n: scaled sub-diagonal
+    double *scal;                      // [sigma, 1/sigma]: power-of-two scaling of T
     double *dt, *zt;                   // n: sorted non-deflated poles / weights per node segment
     double *mu, *lamroot, *zhat;       // n
     double *dval;                      // n: deflated eigenvalues (ascending) per node segment

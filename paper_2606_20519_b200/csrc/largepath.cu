@@ -50,7 +50,7 @@ LargeWs carve(int n, unsigned char *base) {
     // ---- S4
     w.s.n = n; w.s.ldz = N; w.s.depth = stedc_depth(n);
     w.s.Za = dbl((size_t)N * n); w.s.Zb = dbl((size_t)N * n); w.s.Qw = dbl((size_t)N * n); w.s.U = dbl((size_t)N * n);
-    w.s.lamA = dbl(N); w.s.lamB = dbl(N); w.s.dmod = dbl(N); w.s.dt = dbl(N); w.s.zt = dbl(N);
+    w.s.lamA = dbl(N); w.s.lamB = dbl(N); w.s.dmod = dbl(N); w.s.es = dbl(N); w.s.scal = dbl(2); w.s.dt = dbl(N); w.s.zt = dbl(N);
     w.s.mu = dbl(N); w.s.lamroot = dbl(N); w.s.zhat = dbl(N); w.s.dval = dbl(N); w.s.rc = dbl(N); w.s.rs = dbl(N);
     w.s.org = itg(N); w.s.grow = itg(N); w.s.gsrc = itg(N); w.s.dcol = itg(N);
     w.s.dest_root = itg(N); w.s.dest_defl = itg(N); w.s.rp = itg(N); w.s.rq = itg(N);

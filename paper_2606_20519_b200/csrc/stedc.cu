@@ -27,23 +27,57 @@ int stedc_depth(int n) {
     return D;
 }
 
-// ---- K0: remove the rank-one tears from the diagonal ---------------------------------------
-__global__ void stedc_prepare_kernel(int n, int depth, const double *__restrict__ d, const double *__restrict__ e, double *__restrict__ dmod) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    double v = d[i];
-    if (depth > 0) {
-        // is x a leaf boundary?  x == bound(depth, ceil(x 2^depth / n))
-        auto is_bound = [&](int x) -> bool {
-            if (x <= 0 || x >= n) return false;
-            const long long num = ((long long)x << depth);
-            const int j = (int)((num + n - 1) / n);
-            return node_bound(n, depth, j) == x;
-        };
-        if (is_bound(i + 1)) v -= fabs(e[i]);       // i is the last index of a leaf
-        if (is_bound(i)) v -= fabs(e[i - 1]);       // i is the first index of a leaf
+// ---- K0: scale T to unit max-norm by an exact power of two (the deflation tolerances below
+// assume ||T|| ~ 1, as LAPACK's dstedc does) and remove the rank-one tears from the diagonal -----
+__global__ void __launch_bounds__(1024) stedc_prepare_kernel(int n, int depth, const double *__restrict__ d, const double *__restrict__ e,
+                                                             double *__restrict__ dmod, double *__restrict__ es, double *__restrict__ scal) {
+    __shared__ double s_max[32];
+    __shared__ double s_sigma;
+    const int tid = threadIdx.x;
+    double m = 0.0;
+    for (int i = tid; i < n; i += 1024) {
+        m = fmax(m, fabs(d[i]));
+        if (i < n - 1) m = fmax(m, fabs(e[i]));
     }
-    dmod[i] = v;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((tid & 31) == 0) s_max[tid >> 5] = m;
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < 32; ++w) m = fmax(m, s_max[w]);
+        double sigma = 1.0;
+        if (m > 0.0 && m < 1.7e308) {
+            int ex;
+            frexp(m, &ex);                 // m = f 2^ex, f in [0.5, 1)
+            sigma = ldexp(1.0, -ex);       // sigma m in [0.5, 1)
+        }
+        s_sigma = sigma;
+        scal[0] = sigma; scal[1] = 1.0 / sigma;
+    }
+    __syncthreads();
+    const double sigma = s_sigma;
+    // is x a leaf boundary?  x == bound(depth, ceil(x 2^depth / n))
+    auto is_bound = [&](int x) -> bool {
+        if (x <= 0 || x >= n) return false;
+        const long long num = ((long long)x << depth);
+        const int j = (int)((num + n - 1) / n);
+        return node_bound(n, depth, j) == x;
+    };
+    for (int i = tid; i < n; i += 1024) {
+        double v = d[i] * sigma;
+        const double ei = (i < n - 1) ? e[i] * sigma : 0.0;
+        es[i] = ei;
+        if (depth > 0) {
+            if (is_bound(i + 1)) v -= fabs(ei);                       // i is the last index of a leaf
+            if (is_bound(i)) v -= fabs(e[i - 1] * sigma);             // i is the first index of a leaf
+        }
+        dmod[i] = v;
+    }
+}
+
+__global__ void stedc_unscale_kernel(int n, double *__restrict__ lam, const double *__restrict__ scal) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) lam[i] *= scal[1];
 }
 
 // ---- K1: leaves -- implicit QL with Wilkinson shift in one warp -----------------------------
@@ -487,8 +521,9 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
     // zero both eigenvector buffers: the off-diagonal quadrants of every node block are structural zeros
     if (cudaMemsetAsync(w.Za, 0, sizeof(double) * (size_t)w.ldz * n, st) != cudaSuccess) return HPSD_ECUDA_;
     if (D > 0 && cudaMemsetAsync(w.Zb, 0, sizeof(double) * (size_t)w.ldz * n, st) != cudaSuccess) return HPSD_ECUDA_;
-    stedc_prepare_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, D, d, e, w.dmod);
+    stedc_prepare_kernel<<<1, 1024, 0, st>>>(n, D, d, e, w.dmod, w.es, w.scal);
     HPSD_LAUNCH_CHECK();
+    e = w.es;    // everything below works on the scaled tridiagonal
     stedc_leaf_kernel<<<1 << D, 32, 0, st>>>(n, D, w.dmod, e, w.Za, w.ldz, w.lamA, w.info);
     HPSD_LAUNCH_CHECK();
     double *Zin = w.Za, *Zout = w.Zb, *lin = w.lamA, *lout = w.lamB;
@@ -518,6 +553,8 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
         double *t = Zin; Zin = Zout; Zout = t;
         t = lin; lin = lout; lout = t;
     }
+    stedc_unscale_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, lin, w.scal);
+    HPSD_LAUNCH_CHECK();
     *lam_out = lin; *Z_out = Zin;
     return 0;
 }
