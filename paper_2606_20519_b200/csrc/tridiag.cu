@@ -3,10 +3,17 @@
 // so T's sub-diagonal is real without a separate phase pass).  "Eigendecomposition" of
 // PAPER.md:1536 starts here; the paper names no kernel (library call), the design is ours.
 //
-// One-stage blocked reduction (see DESIGN.md for why not dense->band->tridiagonal on B200):
-//   * panel of NB columns in ONE persistent cooperative kernel, two grid barriers per column.
-//     Per column: Hermitian mat-vec y = A22 v over the stored lower triangle (the HBM/L2-bound
-//     half of the flops), rank-2NB corrections from the panel (V, W), next-column update.
+// One-stage blocked reduction (DESIGN.md §7 for why not dense->band->tridiagonal on B200):
+//   * panel of NB = 32 columns in ONE persistent cooperative kernel, two grid barriers per column.
+//     The trailing matrix is NOT modified inside a panel, so its 32 x 32 tiles are distributed over
+//     the shared memory of all SMs ONCE per panel (12 slots of 16.5 KB per CTA: 28 MB over 148 SMs,
+//     i.e. trailing sizes up to ~1880 stay resident; larger ones stream through the same slots
+//     with per-warp cp.async rings that prefetch across the grid barrier).
+//     Phase A (per column): every warp multiplies its own tiles by the Householder vector
+//       (y = A22 v, row parts and column parts of the stored lower triangle), no block-level sync.
+//     Phase B: rows are spread over the CTAs; y is assembled from the tile partials, w is formed,
+//       the next column is updated and its norm / V^H a, W^H a partials are left for phase A.
+//     Each phase has ONE dependent L2 round trip.
 //   * trailing update A22 -= V W^H + W V^H after each panel as a DMMA HER2K (gemm.cuh).
 //
 // Storage: lower triangle of A (column-major, lda).  After the reduction column c holds the
@@ -23,9 +30,16 @@ namespace cg = cooperative_groups;
 namespace hpsd {
 
 constexpr int kPanelThreads = 256;
+constexpr int kTS = 32;                  // tile edge of the distributed trailing matrix
+constexpr int kTP = kTS + 1;             // shared-memory pitch (elements): row- and column-wise reads conflict free
+constexpr int kSlots = 12;               // tile slots per CTA
+constexpr int kSlotElems = kTS * kTP;
+static_assert(kNB == kTS, "panel width and tile edge must agree (tile set is fixed per panel)");
 
 struct PanelArgs {
-    int n, lda, ldw, ldp, j0, nbp, ts, nblk, G;
+    int n, lda, ldw, ldp, j0, nbp, nblk, G;
+    int T;                  // tiles of this panel's trailing matrix (prefix of `tiles`)
+    int q;                  // tiles per CTA = ceil(T / G)
     cplx *A, *W;            // W: ldw x NB panel workspace
     double *d, *e;
     cplx *tau;
@@ -35,6 +49,19 @@ struct PanelArgs {
     double *qpart;          // G
     const int2 *tiles;      // lower-triangle tile list, tile column descending
 };
+
+#ifdef HPSD_PANEL_TRACE
+// dev-only: per-column phase timestamps of CTA 0 and CTA G/2 (clock64), first traced launch only
+__device__ long long g_trace[2 * 32 * 8];
+__device__ int g_trace_armed = 0;
+#define TRACE(slot)                                                                                   \
+    do {                                                                                              \
+        if (trace_on)                                                                                 \
+            g_trace[((g == 0 ? 0 : 1) * 32 + i) * 8 + (slot)] = clock64();                             \
+    } while (0)
+#else
+#define TRACE(slot) do {} while (0)
+#endif
 
 __device__ __forceinline__ cplx group8_sum(cplx v) {
 #pragma unroll
@@ -59,59 +86,94 @@ __device__ __forceinline__ void householder_scalars(cplx alpha, double xnorm2, d
     }
 }
 
-// Column preparation: apply the panel's first `cnt` reflector pairs (V, W) to column cn (rows >= cn),
-// store it, set d[cn], and leave per-CTA partials  S = sum_{r>=cn+2}|a_r|^2,
-// gV[t] = sum_{r>=cn+2} conj(V[r,t]) a_r, gW[t] likewise.  `have_new`: reflector cnt-1 lives in
-// registers of the caller (v_r, w_r) -- not used here; this variant reads everything from memory and
-// is only used at panel start (cnt = 0).
-template <int TS>
-__device__ void panel_body(const PanelArgs &p) {
+// Phase-B row distribution: 31 rows per CTA (one per 8-lane group; group 31 is the helper), more
+// only when the rows outnumber 31 G.  Few producers keep the cross-CTA reductions small.
+__device__ __forceinline__ int rows_per_cta(int rows, int G) { const int l = (rows + G - 1) / G; return l > 31 ? l : 31; }
+__device__ __forceinline__ int producers(int rows, int G) { const int l = rows_per_cta(rows, G); return (rows + l - 1) / l; }
+
+// One warp copies tile (I, J) of A into a shared-memory slot (zero fill outside the matrix).
+__device__ __forceinline__ void warp_load_tile(cplx *slot, const cplx *__restrict__ A, int lda, int n, int2 ij, int lane) {
+    const int r = ij.x * kTS + lane, c0 = ij.y * kTS;
+    const bool rok = r < n;
+#pragma unroll 8
+    for (int cc = 0; cc < kTS; ++cc) {
+        const bool ok = rok && (c0 + cc < n);
+        cp_async_16(slot + cc * kTP + lane, ok ? A + (size_t)(c0 + cc) * lda + r : A, ok);
+    }
+}
+
+__device__ __forceinline__ void cp_async_wait_dyn(int pending) {
+    if (pending <= 0) cp_async_wait<0>(); else cp_async_wait<1>();
+}
+
+__global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelArgs p) {
     cg::grid_group grid = cg::this_grid();
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // shared layout
-    cplx *s_vI = reinterpret_cast<cplx *>(smem_raw);          // TS
-    cplx *s_vJ = s_vI + TS;                                    // TS
-    cplx *s_row = s_vJ + TS;                                   // 8 x TS
-    cplx *s_col = s_row + 8 * TS;                              // TS
-    cplx *s_cV = s_col + TS;                                   // kNB
+    cplx *s_slots = reinterpret_cast<cplx *>(smem_raw);        // kSlots x kSlotElems
+    cplx *s_v = s_slots + kSlots * kSlotElems;                 // 8 warps x 2 x kTS : v pieces of the tile in flight
+    cplx *s_cV = s_v + 8 * 2 * kTS;                            // kNB
     cplx *s_cW = s_cV + kNB;                                   // kNB
     cplx *s_Vc1 = s_cW + kNB;                                  // kNB : V[c+1, t]
     cplx *s_Wc1 = s_Vc1 + kNB;                                 // kNB : W[c+1, t]
-    cplx *s_gV = s_Wc1 + kNB;                                  // 32 x kNB
-    cplx *s_gW = s_gV + 32 * kNB;                              // 32 x kNB
-    double *s_S = reinterpret_cast<double *>(s_gW + 32 * kNB); // 32
-    double *s_q = s_S + 32;                                    // 8
-    cplx *s_sc = reinterpret_cast<cplx *>(s_q + 8);            // scalars: [0]=tau [1]=scale [2]=(beta, alpha') [3]=w_{c+1}
+    cplx *s_gV = s_Wc1 + kNB;                                  // 8 x kNB
+    cplx *s_gW = s_gV + 8 * kNB;                               // 8 x kNB
+    cplx *s_sc = s_gW + 8 * kNB;                               // [0]=tau [1]=scale [2]=w_{c+1}
+    double *s_S = reinterpret_cast<double *>(s_sc + 4);        // 8
+    double *s_q = s_S + 8;                                     // 8 (+1: total)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = blockIdx.x, G = p.G;
     const int n = p.n, lda = p.lda, ldw = p.ldw, ldp = p.ldp;
     cplx *A = p.A, *W = p.W;
-    const int grp = tid >> 3, gl = tid & 7;          // 32 row groups of 8 lanes
-    const int PSTRIDE = 2 * kNB + 1;
+#ifdef HPSD_PANEL_TRACE
+    const bool trace_on = (tid == 0 && g_trace_armed == 1 && p.j0 == 0 && (g == 0 || g == G / 2));
+#endif
+    constexpr int PSTRIDE = 2 * kNB + 1;
+    const int T = p.T, q = p.q;
+    const bool streaming = q > kSlots;
 
-    // ---------------- panel start: partial norm of column j0 (already fully updated) -----
+    // ---------------- tile slots: this warp owns slots `warp` and (for warps 0..3) `warp + 8` ---------
+    // tile k of this CTA is tiles[g + k G]; it lives in slot k % kSlots, served by warp (k % kSlots) % 8.
+    const int nsl = (warp + 8 < kSlots) ? 2 : 1;
+    int issued = 0;
+    int ready_seq[2] = {0, 0};
+    for (int h = 0; h < nsl; ++h) {
+        const int k = warp + 8 * h;
+        const int idx = g + k * G;
+        if (k < q && idx < T) {
+            warp_load_tile(s_slots + (size_t)k * kSlotElems, A, lda, n, p.tiles[idx], lane);
+            cp_async_commit();
+            ready_seq[h] = ++issued;
+        }
+    }
+
+    // this warp's tiles in sequence order j = 0..cnt-1: k(j) = (j / nsl) kSlots + warp + 8 (j % nsl), ascending in j
+    int cnt = 0;
+    for (int j = 0;; ++j) {
+        const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
+        if (k >= q || g + k * G >= T) break;
+        cnt = j + 1;
+    }
+
+    // ---------------- panel start: d[j0] and the partial norm of column j0 (already fully updated) -----
     {
         const int cn = p.j0;
-        const int rows = n - cn;                     // rows cn .. n-1
-        const int L = (rows + G - 1) / G;
+        const int rows = n - cn;
+        const int L = rows_per_cta(rows, G);
         double S = 0.0;
-        for (int rr = grp; rr < L; rr += 32) {
+        for (int rr = tid; rr < L; rr += kPanelThreads) {
             const int r = cn + g * L + rr;
-            if (r < n && gl == 0) {
-                if (r == cn) {
-                    cplx a = A[(size_t)cn * lda + r];
-                    p.d[cn] = a.x;
-                } else if (r >= cn + 2) {
-                    S += abs2(A[(size_t)cn * lda + r]);
-                }
+            if (r < n) {
+                if (r == cn) p.d[cn] = A[(size_t)cn * lda + r].x;
+                else if (r >= cn + 2) S += abs2(A[(size_t)cn * lda + r]);
             }
         }
-        if (gl == 0) s_S[grp] = S;
+        S = warp_sum(S);
+        if (lane == 0) s_S[warp] = S;
         __syncthreads();
         if (tid == 0) {
             double t = 0.0;
-            for (int k = 0; k < 32; ++k) t += s_S[k];
+            for (int k = 0; k < 8; ++k) t += s_S[k];
             p.part[(size_t)g * PSTRIDE] = mk(t, 0.0);
         }
     }
@@ -120,275 +182,268 @@ __device__ void panel_body(const PanelArgs &p) {
     for (int i = 0; i < p.nbp; ++i) {
         const int c = p.j0 + i;
         if (c >= n - 1) break;
-        // ================= phase A =================
-        // (a) Householder scalars, redundantly and identically in every CTA
+        // ================= phase A: y = A22 v over this CTA's tiles (no block-level sync) =================
+        TRACE(0);
+        // raw pieces of column c for this warp's first tiles: issued before anything that waits
+        // Tiles are walked forwards on even columns and backwards on odd ones: when they stream, the tail
+        // of one pass is the head of the next, so it is still in the slots / in L2.
+        const bool fwd = (i & 1) == 0;
+        cplx rawI[2], rawJ[2];
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+            rawI[jj] = mk(0.0, 0.0); rawJ[jj] = mk(0.0, 0.0);
+            if (jj < cnt) {
+                const int j = fwd ? jj : cnt - 1 - jj;
+                const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
+                const int2 ij = p.tiles[g + k * G];
+                const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
+                if (rI < n && rI > c + 1) rawI[jj] = ldcg_(&A[(size_t)c * lda + rI]);
+                if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[jj] = ldcg_(&A[(size_t)c * lda + rJ]);
+            }
+        }
+        const int nprod = producers(n - c, G);          // CTAs that left partials for this column
+        // warp 0: Householder scalars from the partial norms
         if (warp == 0) {
             double S = 0.0;
-            for (int k = lane; k < G; k += 32) S += ldcg_(&p.part[(size_t)k * PSTRIDE].x);
+            for (int k = lane; k < nprod; k += 32) S += ldcg_(&p.part[(size_t)k * PSTRIDE].x);
+            const cplx alpha = ldcg_(&A[(size_t)c * lda + c + 1]);
             S = warp_sum(S);
+            double beta; cplx tau0, scale0;
+            householder_scalars(alpha, S, beta, tau0, scale0);
             if (lane == 0) {
-                const cplx alpha = ldcg_(&A[(size_t)c * lda + c + 1]);
-                double beta; cplx tau, scale;
-                householder_scalars(alpha, S, beta, tau, scale);
-                s_sc[0] = tau; s_sc[1] = scale; s_sc[2] = mk(beta, 0.0);
-                if (g == 0) { p.e[c] = beta; p.tau[c] = tau; }
+                s_sc[0] = tau0; s_sc[1] = scale0;
+                if (g == 0) { p.e[c] = beta; p.tau[c] = tau0; }
             }
+        }
+        // warp 7 of CTA idx < 64: reducers cV[t] = (V22^H v)_t, cW[t] = (W22^H v)_t (rows >= c+1)
+        cplx red_s = mk(0.0, 0.0), red_top = mk(0.0, 0.0);
+        const bool reducer = (warp == 7 && i > 0 && g < 2 * kNB && (g % kNB) < i);
+        if (reducer) {
+            const int t = g % kNB, which = g / kNB;
+            for (int k = lane; k < nprod; k += 32) red_s = red_s + ldcg_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
+            red_top = which == 0 ? ldcg_(&A[(size_t)(p.j0 + t) * lda + c + 1]) : ldcg_(&W[(size_t)t * ldw + c + 1]);
+            red_s = warp_sum(red_s);
         }
         __syncthreads();
         const cplx tau = s_sc[0], scale = s_sc[1];
-
-        // (b) reducer CTA: cV = V22^H v, cW = W22^H v  (rows >= c+1) from the per-CTA partials
-        if (g == G - 1 && i > 0) {
-            // thread -> (slice = tid/64, which = (tid/32)&1, t = tid%32)
-            const int t = tid & 31, which = (tid >> 5) & 1, slice = tid >> 6;
-            cplx acc = mk(0.0, 0.0);
-            if (t < i) {
-                for (int k = slice; k < G; k += 4) {
-                    const cplx v = ldcg_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
-                    acc = acc + v;
-                }
-            }
-            s_gV[(slice * 2 + which) * kNB + t] = acc;
-            __syncthreads();
-            if (tid < 64 && t < i) {
-                cplx s = (s_gV[(0 * 2 + which) * kNB + t] + s_gV[(1 * 2 + which) * kNB + t]) +
-                         (s_gV[(2 * 2 + which) * kNB + t] + s_gV[(3 * 2 + which) * kNB + t]);
-                // row c+1 term (v = 1 there) plus scale * sum over rows >= c+2
-                const cplx top = which == 0 ? ldcg_(&A[(size_t)(p.j0 + t) * lda + c + 1]) : ldcg_(&W[(size_t)t * ldw + c + 1]);
-                s = conj_(top) + scale * s;
-                p.tot[which * kNB + t] = s;
-            }
-            __syncthreads();
-        }
-
-        // (c) Hermitian mat-vec partials over the lower-triangle tiles of A[c+1:, c+1:]
+        TRACE(1);
+        if (reducer && lane == 0)     // row c+1 term (v = 1 there) plus scale * sum over rows >= c+2
+            p.tot[(g / kNB) * kNB + (g % kNB)] = conj_(red_top) + scale * red_s;
+        double qacc = 0.0;
         {
-            const int J0 = (c + 1) / TS;
-            const int nbk = p.nblk - J0;
-            const int T = nbk * (nbk + 1) / 2;
-            double qacc = 0.0;          // thread 0 only
-            constexpr int RH = TS / 32, CPW = TS / 8;
-            for (int idx = g; idx < T; idx += G) {
-                const int2 ij = p.tiles[idx];
-                const int I = ij.x, J = ij.y;
-                const int r0 = I * TS, c0 = J * TS;
-                __syncthreads();
-                // vector pieces (v formed on the fly; zero outside the trailing matrix)
-                for (int k = tid; k < 2 * TS; k += kPanelThreads) {
-                    const int r = (k < TS) ? r0 + k : c0 + (k - TS);
-                    cplx v = mk(0.0, 0.0);
-                    if (r < n) {
-                        if (r == c + 1) v = mk(1.0, 0.0);
-                        else if (r > c + 1) v = scale * ldcg_(&A[(size_t)c * lda + r]);
+            cplx *vI = s_v + warp * 2 * kTS, *vJ = vI + kTS;
+            {
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const int j = fwd ? jj : cnt - 1 - jj;
+                    const int h = j % nsl;
+                    const int k = (j / nsl) * kSlots + warp + 8 * h;
+                    const int2 ij = p.tiles[g + k * G];
+                    const int r0 = ij.x * kTS, c0 = ij.y * kTS;
+                    const bool diag = (ij.x == ij.y);
+                    // v pieces (formed on the fly; zero outside the trailing matrix)
+                    {
+                        const int rI = r0 + lane, rJ = c0 + lane;
+                        cplx a, b;
+                        if (jj == 0) { a = rawI[0]; b = rawJ[0]; }
+                        else if (jj == 1) { a = rawI[1]; b = rawJ[1]; }
+                        else {
+                            a = mk(0.0, 0.0); b = mk(0.0, 0.0);
+                            if (rI < n && rI > c + 1) a = ldcg_(&A[(size_t)c * lda + rI]);
+                            if (!diag && rJ < n && rJ > c + 1) b = ldcg_(&A[(size_t)c * lda + rJ]);
+                        }
+                        a = (rI == c + 1) ? mk(1.0, 0.0) : scale * a;
+                        b = diag ? a : ((rJ == c + 1) ? mk(1.0, 0.0) : scale * b);
+                        __syncwarp();
+                        vI[lane] = a; vJ[lane] = b;
                     }
-                    if (k < TS) s_vI[k] = v; else s_vJ[k - TS] = v;
-                }
-                __syncthreads();
-                cplx accR[RH];
-#pragma unroll
-                for (int h = 0; h < RH; ++h) accR[h] = mk(0.0, 0.0);
-                const bool diag = (I == J);
-                // issue all loads first (ILP), then consume
-                cplx a[CPW][RH];
-#pragma unroll
-                for (int cc = 0; cc < CPW; ++cc) {
-                    const int col = c0 + warp + 8 * cc;
-#pragma unroll
-                    for (int h = 0; h < RH; ++h) {
-                        const int r = r0 + lane + 32 * h;
-                        const bool ok = (r < n) && (col < n) && (!diag || r >= col);
-                        a[cc][h] = ok ? A[(size_t)col * lda + r] : mk(0.0, 0.0);
-                        if (diag && r == col) a[cc][h].y = 0.0;
+                    cp_async_wait_dyn(issued - ready_seq[h]);
+                    __syncwarp();
+                    const cplx *sl = s_slots + (size_t)(k % kSlots) * kSlotElems;
+                    cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0);
+                    if (!diag) {
+#pragma unroll 8
+                        for (int cc = 0; cc < kTS; ++cc) {
+                            cfma(accR, sl[cc * kTP + lane], vJ[cc]);          // lane = row
+                            cfma_conj(accC, sl[lane * kTP + cc], vI[cc]);     // lane = column, cc = row
+                        }
+                    } else {
+#pragma unroll 8
+                        for (int cc = 0; cc < kTS; ++cc) {
+                            cplx a = sl[cc * kTP + lane];                      // row = lane, col = cc
+                            a.x = (lane >= cc) ? a.x : 0.0;
+                            a.y = (lane > cc) ? a.y : 0.0;                     // real diagonal, nothing above it
+                            cfma(accR, a, vJ[cc]);
+                            cplx b = sl[lane * kTP + cc];                      // col = lane, row = cc
+                            b.x = (cc > lane) ? b.x : 0.0;
+                            b.y = (cc > lane) ? b.y : 0.0;
+                            cfma_conj(accC, b, vI[cc]);
+                        }
                     }
-                }
-#pragma unroll
-                for (int cc = 0; cc < CPW; ++cc) {
-                    const int cl = warp + 8 * cc;
-                    const cplx vj = s_vJ[cl];
-                    cplx colacc = mk(0.0, 0.0);
-#pragma unroll
-                    for (int h = 0; h < RH; ++h) {
-                        const int rl = lane + 32 * h;
-                        cfma(accR[h], a[cc][h], vj);
-                        // column part: conj(a) * v_I[r]; on the diagonal tile skip r == col (counted in the row part)
-                        if (!(diag && rl == cl)) cfma_conj(colacc, a[cc][h], s_vI[rl]);
-                    }
-                    colacc = warp_sum(colacc);
-                    if (lane == 0) s_col[cl] = colacc;
-                }
-#pragma unroll
-                for (int h = 0; h < RH; ++h) s_row[warp * TS + lane + 32 * h] = accR[h];
-                __syncthreads();
-                if (tid < TS) {
-                    cplx s = mk(0.0, 0.0);
-#pragma unroll
-                    for (int w = 0; w < 8; ++w) s = s + s_row[w * TS + tid];
                     double qterm;
                     if (diag) {
-                        s = s + s_col[tid];
-                        p.PR[(size_t)J * ldp + r0 + tid] = s;
-                        qterm = s_vI[tid].x * s.x + s_vI[tid].y * s.y;
+                        const cplx s = accR + accC;
+                        p.PR[(size_t)ij.y * ldp + r0 + lane] = s;
+                        qterm = vI[lane].x * s.x + vI[lane].y * s.y;
                     } else {
-                        p.PR[(size_t)J * ldp + r0 + tid] = s;
-                        p.PC[(size_t)I * ldp + c0 + tid] = s_col[tid];
-                        qterm = 2.0 * (s_vI[tid].x * s.x + s_vI[tid].y * s.y);
+                        p.PR[(size_t)ij.y * ldp + r0 + lane] = accR;
+                        p.PC[(size_t)ij.x * ldp + c0 + lane] = accC;
+                        qterm = 2.0 * (vI[lane].x * accR.x + vI[lane].y * accR.y);
                     }
-                    qterm = warp_sum(qterm);
-                    if (lane == 0) s_q[warp] = qterm;
-                }
-                __syncthreads();
-                if (tid == 0) {
-                    for (int w = 0; w < TS / 32; ++w) qacc += s_q[w];
+                    qacc += warp_sum(qterm);
+                    if (streaming) {
+                        // refill this slot with the tile that uses it next in this pass; at the end of a pass
+                        // the slot keeps its tile, which is the first one the reversed next pass needs
+                        const int jn = fwd ? j + nsl : j - nsl;
+                        if (jn >= 0 && jn < cnt) {
+                            const int kn = (jn / nsl) * kSlots + warp + 8 * h;
+                            __syncwarp();
+                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, A, lda, n, p.tiles[g + kn * G], lane);
+                            cp_async_commit();
+                            ready_seq[h] = ++issued;
+                        }
+                    }
                 }
             }
-            if (tid == 0) p.qpart[g] = qacc;
+        }
+        if (lane == 0) s_q[warp] = qacc;
+        TRACE(2);
+        __syncthreads();
+        if (tid == 0 && g < T) {
+            double t = 0.0;
+            for (int k = 0; k < 8; ++k) t += s_q[k];
+            p.qpart[g] = t;
         }
         grid.sync();
 
-        // ================= phase B =================
+        TRACE(3);
+        // ================= phase B: rows spread over the CTAs; one dependent L2 round trip =================
+        // lane = row (31 consecutive rows per CTA; lane 31 is the helper row c+1, whose w every CTA needs
+        // for the next-column update); warp w serves tile columns b = J0 + w (mod 8) of the partials and
+        // panel columns t = w (mod 8) of V and W: every global load is a coalesced 512-byte row segment.
         {
             const bool do_next = (i + 1 < p.nbp);
-            if (tid < kNB) {
-                cplx cv = mk(0.0, 0.0), cw = mk(0.0, 0.0), v1 = mk(0.0, 0.0), w1 = mk(0.0, 0.0);
-                if (tid < i) {
-                    cv = ldcg_(&p.tot[tid]);
-                    cw = ldcg_(&p.tot[kNB + tid]);
-                    // row c+1 of V and W (needed for the next-column update)
-                    v1 = ldcg_(&A[(size_t)(p.j0 + tid) * lda + c + 1]);
-                    w1 = ldcg_(&W[(size_t)tid * ldw + c + 1]);
-                }
-                s_cV[tid] = cv; s_cW[tid] = cw; s_Vc1[tid] = v1; s_Wc1[tid] = w1;
-            }
-            if (warp == 1) {
-                double q = 0.0;
-                for (int k = lane; k < G; k += 32) q += ldcg_(&p.qpart[k]);
-                q = warp_sum(q);
-                if (lane == 0) s_q[0] = q;
-            }
-            __syncthreads();
-            if (tid == 0) {
-                double re = 0.0;   // Re(cV^H cW)
-                for (int t = 0; t < i; ++t) re += s_cV[t].x * s_cW[t].x + s_cV[t].y * s_cW[t].y;
-                const double vHy = s_q[0] - 2.0 * re;
-                s_sc[2].y = -0.5 * abs2(tau) * vHy;   // alpha'
-            }
-            __syncthreads();
-            const double alphap = s_sc[2].y;
-
-            const int J0 = (c + 1) / TS;
-            // y of one row from the tile partials + panel corrections; all 8 lanes get the result
-            // (every lane of the warp must call this: it shuffles with a full mask; `ok` predicates loads)
-            auto row_yw = [&](bool ok, int r, cplx vr, cplx (&Vr)[kNB / 8], cplx (&Wr)[kNB / 8]) -> cplx {
-                const int R = r / TS;
-                cplx ys = mk(0.0, 0.0);
-                if (ok) {
-                    for (int b = J0 + gl; b < p.nblk; b += 8) {
-                        const cplx v = (b <= R) ? ldcg_(&p.PR[(size_t)b * ldp + r]) : ldcg_(&p.PC[(size_t)b * ldp + r]);
-                        ys = ys + v;
-                    }
-                }
-                cplx corr = mk(0.0, 0.0);
-#pragma unroll
-                for (int k = 0; k < kNB / 8; ++k) {
-                    const int t = gl + 8 * k;
-                    if (ok && t < i) {
-                        Vr[k] = ldcg_(&A[(size_t)(p.j0 + t) * lda + r]);
-                        Wr[k] = ldcg_(&W[(size_t)t * ldw + r]);
-                        cfma(corr, Vr[k], s_cW[t]);
-                        cfma(corr, Wr[k], s_cV[t]);
-                    } else { Vr[k] = mk(0.0, 0.0); Wr[k] = mk(0.0, 0.0); }
-                }
-                ys = group8_sum(ys - corr);
-                return tau * ys + alphap * vr;
-            };
-
-            // w_{c+1} (row c+1 of the new W column), needed by every CTA for the next-column update
-            if (do_next) {
-                if (warp == 0) {   // all four 8-lane groups of warp 0 compute the same value
-                    cplx Vr[kNB / 8], Wr[kNB / 8];
-                    const cplx w = row_yw(true, c + 1, mk(1.0, 0.0), Vr, Wr);
-                    if (lane == 0) s_sc[3] = w;
-                }
-                __syncthreads();
-            }
-            const cplx wc1 = s_sc[3];
-
+            const int J0 = (c + 1) / kTS;
             const int rows = n - (c + 1);
-            const int L = (rows + G - 1) / G;
+            const int L = rows_per_cta(rows, G);
+            const bool active = g * L < rows;                    // block-uniform: this CTA owns rows
+            cplx *s_p1 = s_gV, *s_p2 = s_gW;                     // 8 x 32 each
+            double *s_re = s_S;                                  // 8
             cplx accV[kNB / 8], accW[kNB / 8];
 #pragma unroll
             for (int k = 0; k < kNB / 8; ++k) { accV[k] = mk(0.0, 0.0); accW[k] = mk(0.0, 0.0); }
             double S = 0.0;
-            for (int base = 0; base < L; base += 32) {      // warp-uniform trip count
-                const int rr = base + grp;
-                const int r = c + 1 + g * L + rr;
-                const bool ok = (rr < L) && (r < n);
-                const cplx ar = ok ? ldcg_(&A[(size_t)c * lda + r]) : mk(0.0, 0.0);
-                const cplx vr = (r == c + 1) ? mk(1.0, 0.0) : scale * ar;
-                cplx Vr[kNB / 8], Wr[kNB / 8];
-                const cplx wr = row_yw(ok, r, vr, Vr, Wr);
-                if (ok && gl == 0) {
-                    W[(size_t)i * ldw + r] = wr;
-                    A[(size_t)c * lda + r] = vr;
-                }
-                if (do_next) {
-                    // a'_r = A[r,c+1] - sum_{t<=i} V[r,t] conj(W[c+1,t]) + W[r,t] conj(V[c+1,t])
-                    cplx upd = mk(0.0, 0.0);
-#pragma unroll
-                    for (int k = 0; k < kNB / 8; ++k) {
-                        const int t = gl + 8 * k;
-                        if (t < i) {
-                            cfma(upd, Vr[k], conj_(s_Wc1[t]));
-                            cfma(upd, Wr[k], conj_(s_Vc1[t]));
-                        }
-                    }
-                    upd = group8_sum(upd);
-                    cfma(upd, vr, conj_(wc1));
-                    upd = upd + wr;                   // V[c+1, i] = 1
-                    cplx an = (ok ? ldcg_(&A[(size_t)(c + 1) * lda + r]) : mk(0.0, 0.0)) - upd;
-                    if (ok && r == c + 1) { an.y = 0.0; if (gl == 0) p.d[c + 1] = an.x; }
-                    if (ok && gl == 0) A[(size_t)(c + 1) * lda + r] = an;
-                    if (ok && r >= c + 3) {
-                        if (gl == 0) S += abs2(an);
-#pragma unroll
-                        for (int k = 0; k < kNB / 8; ++k) {
-                            const int t = gl + 8 * k;
-                            if (t < i) { cfma_conj(accV[k], Vr[k], an); cfma_conj(accW[k], Wr[k], an); }
-                            else if (t == i) { cfma_conj(accV[k], vr, an); cfma_conj(accW[k], wr, an); }
-                        }
-                    }
-                }
-            }
-            if (do_next) {
+            for (int base = 0; active && base < L; base += 31) {          // block-uniform trip count
+                const bool helper = (lane == 31);
+                const int rr = base + lane;
+                const int r = helper ? c + 1 : c + 1 + g * L + rr;
+                const bool ok = helper ? do_next : (rr < L && r < n);
+                const bool okr = ok && !helper;
+                // ---- every global load of the pass is issued before the first shared-memory write
+                const cplx ar = okr ? ldcg_(&A[(size_t)c * lda + r]) : mk(0.0, 0.0);
+                const cplx anx = (okr && do_next) ? ldcg_(&A[(size_t)(c + 1) * lda + r]) : mk(0.0, 0.0);
+                cplx Vr[kNB / 8], Wr[kNB / 8], cv[kNB / 8], cw[kNB / 8];
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
-                    s_gV[grp * kNB + gl + 8 * k] = accV[k];
-                    s_gW[grp * kNB + gl + 8 * k] = accW[k];
+                    const int t = warp + 8 * k;
+                    Vr[k] = mk(0.0, 0.0); Wr[k] = mk(0.0, 0.0); cv[k] = mk(0.0, 0.0); cw[k] = mk(0.0, 0.0);
+                    if (t < i) {
+                        if (ok) {
+                            Vr[k] = ldcg_(&A[(size_t)(p.j0 + t) * lda + r]);
+                            Wr[k] = ldcg_(&W[(size_t)t * ldw + r]);
+                        }
+                        cv[k] = ldcg_(&p.tot[t]);
+                        cw[k] = ldcg_(&p.tot[kNB + t]);
+                    }
                 }
-                if (gl == 0) s_S[grp] = S;
+                cplx p1 = mk(0.0, 0.0);
+                if (ok) {
+                    const int R = r / kTS;
+#pragma unroll 4
+                    for (int bb = J0 + warp; bb < p.nblk; bb += 8)
+                        p1 = p1 + ((bb <= R) ? ldcg_(&p.PR[(size_t)bb * ldp + r]) : ldcg_(&p.PC[(size_t)bb * ldp + r]));
+                }
+                double qv = 0.0;
+                if (warp == 1) {
+                    for (int k = lane; k < (T < G ? T : G); k += 32) qv += ldcg_(&p.qpart[k]);
+                    qv = warp_sum(qv);
+                }
+                // ---- partial sums of this warp: y - V cW - W cV,  V conj(W[c+1,:]) + W conj(V[c+1,:]),  Re(cV^H cW)
+                cplx p2 = mk(0.0, 0.0);
+                double re = 0.0;
+#pragma unroll
+                for (int k = 0; k < kNB / 8; ++k) {
+                    // rows c+1 of V and W sit in the helper lane
+                    const cplx v1 = mk(__shfl_sync(0xffffffffu, Vr[k].x, 31), __shfl_sync(0xffffffffu, Vr[k].y, 31));
+                    const cplx w1 = mk(__shfl_sync(0xffffffffu, Wr[k].x, 31), __shfl_sync(0xffffffffu, Wr[k].y, 31));
+                    cplx corr = mk(0.0, 0.0);
+                    cfma(corr, Vr[k], cw[k]); cfma(corr, Wr[k], cv[k]);
+                    p1 = p1 - corr;
+                    cfma(p2, Vr[k], conj_(w1)); cfma(p2, Wr[k], conj_(v1));
+                    re += cv[k].x * cw[k].x + cv[k].y * cw[k].y;
+                }
+                __syncthreads();                                  // previous pass / previous column readers done
+                s_p1[warp * 32 + lane] = p1;
+                s_p2[warp * 32 + lane] = p2;
+                if (lane == 0) s_re[warp] = re;
+                if (warp == 1 && lane == 0) s_q[8] = qv;
                 __syncthreads();
-                if (tid < 2 * kNB) {
-                    const int t = tid % kNB;
-                    const cplx *src = (tid < kNB) ? s_gV : s_gW;
-                    cplx s = mk(0.0, 0.0);
-                    for (int k = 0; k < 32; ++k) s = s + src[k * kNB + t];
-                    p.part[(size_t)g * PSTRIDE + 1 + tid] = s;
-                } else if (tid == 2 * kNB) {
-                    double t = 0.0;
-                    for (int k = 0; k < 32; ++k) t += s_S[k];
-                    p.part[(size_t)g * PSTRIDE] = mk(t, 0.0);
+                TRACE(4);
+                cplx ys = mk(0.0, 0.0), upd = mk(0.0, 0.0);
+                double ret = 0.0;
+#pragma unroll
+                for (int w8 = 0; w8 < 8; ++w8) { ys = ys + s_p1[w8 * 32 + lane]; upd = upd + s_p2[w8 * 32 + lane]; ret += s_re[w8]; }
+                // alpha' = -1/2 |tau|^2 (v^H y), v^H y = q - 2 Re(cV^H cW);  w_r = tau (y_r - V_r cW - W_r cV) + alpha' v_r
+                const double alphap = -0.5 * abs2(tau) * (s_q[8] - 2.0 * ret);
+                const cplx vr = (r == c + 1) ? mk(1.0, 0.0) : scale * ar;
+                const cplx wr = tau * ys + alphap * vr;
+                if (okr && warp == 0) W[(size_t)i * ldw + r] = wr;
+                if (okr && warp == 1) A[(size_t)c * lda + r] = vr;
+                if (!do_next) continue;                           // block-uniform
+                const cplx wc1 = mk(__shfl_sync(0xffffffffu, wr.x, 31), __shfl_sync(0xffffffffu, wr.y, 31));
+                // a'_r = A[r,c+1] - sum_{t<=i} V[r,t] conj(W[c+1,t]) + W[r,t] conj(V[c+1,t])
+                cfma(upd, vr, conj_(wc1));
+                upd = upd + wr;                                   // V[c+1, i] = 1
+                cplx an = anx - upd;
+                if (okr && r == c + 1) { an.y = 0.0; if (warp == 2) p.d[c + 1] = an.x; }
+                if (okr && warp == 2) A[(size_t)(c + 1) * lda + r] = an;
+                if (!(okr && r >= c + 3)) an = mk(0.0, 0.0);       // rows that enter the next column's partials
+                if (warp == 3) S += abs2(an);
+#pragma unroll
+                for (int k = 0; k < kNB / 8; ++k) {
+                    const int t = warp + 8 * k;
+                    if (t < i) { cfma_conj(accV[k], Vr[k], an); cfma_conj(accW[k], Wr[k], an); }
+                    else if (t == i) { cfma_conj(accV[k], vr, an); cfma_conj(accW[k], wr, an); }
+                }
+            }
+            TRACE(5);
+            if (do_next && active) {
+                // partials of the next column: sums over this CTA's rows (lanes), written straight to global
+#pragma unroll
+                for (int k = 0; k < kNB / 8; ++k) {
+                    const int t = warp + 8 * k;
+                    if (t <= i) {                                  // warp-uniform
+                        const cplx sv = warp_sum(accV[k]), sw = warp_sum(accW[k]);
+                        if (lane == 0) {
+                            p.part[(size_t)g * PSTRIDE + 1 + t] = sv;
+                            p.part[(size_t)g * PSTRIDE + 1 + kNB + t] = sw;
+                        }
+                    }
+                }
+                if (warp == 3) {
+                    S = warp_sum(S);
+                    if (lane == 0) p.part[(size_t)g * PSTRIDE] = mk(S, 0.0);
                 }
             }
         }
+        TRACE(6);
         if (i + 1 < p.nbp) grid.sync();
+        TRACE(7);
     }
+    cp_async_wait<0>();
 }
 
-template <int TS>
-__global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelArgs p) { panel_body<TS>(p); }
-
-static size_t panel_smem_bytes(int ts) {
-    return sizeof(cplx) * (size_t)(2 * ts + 8 * ts + ts + 4 * kNB + 64 * kNB + 4) + sizeof(double) * 40;
+static size_t panel_smem_bytes() {
+    return sizeof(cplx) * (size_t)(kSlots * kSlotElems + 8 * 2 * kTS + 4 * kNB + 16 * kNB + 4) + sizeof(double) * 20;
 }
 
 // ---------------------------------------------------------------- HER2K (DMMA)
@@ -425,15 +480,22 @@ int tridiag_init() {
     int dev = 0;
     cudaGetDevice(&dev);
     if (g_panel_init_dev == dev) return 0;
-    if (cudaFuncSetAttribute(tridiag_panel_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)panel_smem_bytes(32)) != cudaSuccess) return HPSD_ECUDA_;
-    if (cudaFuncSetAttribute(tridiag_panel_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)panel_smem_bytes(64)) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(tridiag_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)panel_smem_bytes()) != cudaSuccess) return HPSD_ECUDA_;
     constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
     if (cudaFuncSetAttribute(her2k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h2) != cudaSuccess) return HPSD_ECUDA_;
     g_panel_init_dev = dev;
     return 0;
 }
 
-int tridiag_tile_size(int n) { return n >= 1536 ? 64 : 32; }
+#ifdef HPSD_PANEL_TRACE
+extern "C" int hpsd_debug_trace(int arm, long long *out) {
+    if (arm >= 0) cudaMemcpyToSymbol(g_trace_armed, &arm, sizeof(int));
+    if (out) cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 2 * 32 * 8);
+    return 0;
+}
+#endif
+
+int tridiag_tile_size(int) { return kTS; }
 
 size_t tridiag_tile_count(int n) {
     const int ts = tridiag_tile_size(n);
@@ -459,7 +521,8 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int ts = tridiag_tile_size(n);
     PanelArgs p;
-    p.n = n; p.lda = w.lda; p.ldw = w.ldw; p.ts = ts; p.nblk = (n + ts - 1) / ts; p.G = sms;
+    p.n = n; p.lda = w.lda; p.ldw = w.ldw; p.nblk = (n + ts - 1) / ts; p.G = sms;
+    if (p.G < 2 * kNB) return HPSD_ECUDA_;   // the reducers of phase A need 64 CTAs
     p.A = w.A; p.W = w.W; p.d = w.d; p.e = w.e; p.tau = w.tau;
     p.ldp = w.ldp; p.PR = w.PR; p.PC = w.PC; p.part = w.part; p.tot = w.tot; p.qpart = w.qpart; p.tiles = w.tiles;
     if (n == 1) {
@@ -468,12 +531,14 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
     for (int j0 = 0; j0 < n; j0 += kNB) {
         p.j0 = j0;
         p.nbp = (n - j0 < kNB) ? (n - j0) : kNB;
+        const int nbk = p.nblk - j0 / kTS;              // tile rows/columns of this panel's trailing matrix
+        p.T = nbk * (nbk + 1) / 2;
+        p.q = (p.T + p.G - 1) / p.G;
         void *args[] = {&p};
-        const size_t smem = panel_smem_bytes(ts);
+        const size_t smem = panel_smem_bytes();
         cudaError_t e;
         prof_begin(ST_PANEL, st);
-        if (ts == 64) e = cudaLaunchCooperativeKernel((void *)tridiag_panel_kernel<64>, dim3(p.G), dim3(kPanelThreads), args, smem, st);
-        else e = cudaLaunchCooperativeKernel((void *)tridiag_panel_kernel<32>, dim3(p.G), dim3(kPanelThreads), args, smem, st);
+        e = cudaLaunchCooperativeKernel((void *)tridiag_panel_kernel, dim3(p.G), dim3(kPanelThreads), args, smem, st);
         prof_end(ST_PANEL, st);
         g_launches++;
         if (e != cudaSuccess) return HPSD_ECUDA_;
