@@ -116,10 +116,11 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
                     bool under = false;
                     for (i = mm - 1; i >= l; --i) {
                         const double f = s * ee[i], b = c * ee[i];
-                        r = hypot(f, g);
+                        r = sqrt(f * f + g * g);
+                        if (r < 1e-140) r = hypot(f, g);        // squares underflowed: take the safe route
                         ee[i + 1] = r;
                         if (r == 0.0) { dd[i + 1] -= p; ee[mm] = 0.0; under = true; break; }
-                        s = f / r; c = g / r;
+                        { const double ir = 1.0 / r; s = f * ir; c = g * ir; }
                         g = dd[i + 1] - p;
                         r = (dd[i] - g) * s + 2.0 * c * b;
                         p = s * r;
@@ -240,10 +241,11 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
             if (rho * fabs(zs[r]) <= tol) { push_defl(r); continue; }
             if (pj < 0) { pj = r; continue; }
             double s = zs[pj], c = zs[r];
-            const double tau = hypot(c, s);
             const double t = ds[r] - ds[pj];
-            c /= tau; s = -s / tau;
-            if (fabs(t * c * s) <= tol) {
+            // |t c s| <= tol with c = z_r/tau, s = -z_pj/tau, tau^2 = z_r^2 + z_pj^2, tested without sqrt or division
+            if (fabs(t) * fabs(c * s) <= tol * (c * c + s * s)) {
+                const double tau = sqrt(c * c + s * s);      // weights are <= 1 in magnitude and > tol/rho: no over/underflow
+                c /= tau; s = -s / tau;
                 // close poles: rotate the weight of pj into r and deflate pj
                 zs[r] = tau; zs[pj] = 0.0;
                 a.rp[lo + nrot] = src[pj] & 0x0fffffff; a.rq[lo + nrot] = src[r] & 0x0fffffff;
@@ -284,14 +286,13 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
 }
 
 // ---- M2: apply the deflation rotations to the children's eigenvectors, gather kept columns ----
-__global__ void __launch_bounds__(256) stedc_rotate_gather_kernel(MergeArgs a) {
+__global__ void __launch_bounds__(256) stedc_rotate_kernel(MergeArgs a) {
     const int node = blockIdx.y;
     const int lo = node_bound(a.n, a.depth, node), hi = node_bound(a.n, a.depth, node + 1);
     const int N = hi - lo;
     const int r = blockIdx.x * 256 + threadIdx.x;
-    if (r >= N) return;
-    const int *ni = a.nodeinfo + 8 * node;
-    const int K = ni[0], nrot = ni[4];
+    const int nrot = a.nodeinfo[8 * node + 4];
+    if (r >= N || nrot == 0) return;
     double *Z = const_cast<double *>(a.Zin) + (size_t)lo * a.ldz + lo + r;    // row r of the node block
     for (int t = 0; t < nrot; ++t) {
         const int p = a.rp[lo + t], q = a.rq[lo + t];
@@ -300,8 +301,31 @@ __global__ void __launch_bounds__(256) stedc_rotate_gather_kernel(MergeArgs a) {
         Z[(size_t)p * a.ldz] = c * x + s * y;
         Z[(size_t)q * a.ldz] = c * y - s * x;
     }
-    double *Q = a.Qw + (size_t)lo * a.ldz + lo + r;
-    for (int g = 0; g < K; ++g) Q[(size_t)g * a.ldz] = Z[(size_t)a.gsrc[lo + g] * a.ldz];
+}
+
+// Qw[:, g] = Z[:, gsrc[g]] for the K kept columns (grouped order); one CTA copies 256 rows of 8 columns
+constexpr int kGatherCols = 8;
+__global__ void __launch_bounds__(256) stedc_gather_kernel(MergeArgs a) {
+    const int node = blockIdx.z;
+    const int lo = node_bound(a.n, a.depth, node), hi = node_bound(a.n, a.depth, node + 1);
+    const int N = hi - lo;
+    const int K = a.nodeinfo[8 * node];
+    const int g0 = blockIdx.y * kGatherCols;
+    const int r = blockIdx.x * 256 + threadIdx.x;
+    if (g0 >= K || r >= N) return;
+    const double *__restrict__ Z = a.Zin + (size_t)lo * a.ldz + lo + r;
+    double *__restrict__ Q = a.Qw + (size_t)lo * a.ldz + lo + r;
+    double v[kGatherCols];
+#pragma unroll
+    for (int cc = 0; cc < kGatherCols; ++cc) {
+        const int g = g0 + cc;
+        v[cc] = (g < K) ? Z[(size_t)a.gsrc[lo + g] * a.ldz] : 0.0;
+    }
+#pragma unroll
+    for (int cc = 0; cc < kGatherCols; ++cc) {
+        const int g = g0 + cc;
+        if (g < K) Q[(size_t)g * a.ldz] = v[cc];
+    }
 }
 
 // ---- M3: secular equation, one warp per root ------------------------------------------------
@@ -539,7 +563,9 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
         a.rp = w.rp; a.rq = w.rq; a.nodeinfo = w.nodeinfo; a.info = w.info;
         stedc_merge_setup_kernel<<<nodes, 256, (size_t)24 * maxN, st>>>(a);
         HPSD_LAUNCH_CHECK();
-        stedc_rotate_gather_kernel<<<dim3((maxN + 255) / 256, nodes), 256, 0, st>>>(a);
+        stedc_rotate_kernel<<<dim3((maxN + 255) / 256, nodes), 256, 0, st>>>(a);
+        HPSD_LAUNCH_CHECK();
+        stedc_gather_kernel<<<dim3((maxN + 255) / 256, (maxN + kGatherCols - 1) / kGatherCols, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
         stedc_secular_kernel<<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();

@@ -381,13 +381,14 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     cfma(p2, Vr[k], conj_(w1)); cfma(p2, Wr[k], conj_(v1));
                     re += cv[k].x * cw[k].x + cv[k].y * cw[k].y;
                 }
+                TRACE(4);
                 __syncthreads();                                  // previous pass / previous column readers done
                 s_p1[warp * 32 + lane] = p1;
                 s_p2[warp * 32 + lane] = p2;
                 if (lane == 0) s_re[warp] = re;
                 if (warp == 1 && lane == 0) s_q[8] = qv;
                 __syncthreads();
-                TRACE(4);
+                TRACE(5);
                 cplx ys = mk(0.0, 0.0), upd = mk(0.0, 0.0);
                 double ret = 0.0;
 #pragma unroll
@@ -415,7 +416,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     else if (t == i) { cfma_conj(accV[k], vr, an); cfma_conj(accW[k], wr, an); }
                 }
             }
-            TRACE(5);
             if (do_next && active) {
                 // partials of the next column: sums over this CTA's rows (lanes), written straight to global
 #pragma unroll
