@@ -46,42 +46,57 @@ struct SubEpi {        // C[i + j*ld] -= acc
     }
 };
 
-// Gram matrices G_b = V_b^H V_b for every block (blockIdx.z = b)
+// Gram matrices G_b = V_b^H V_b for every block (blockIdx.z = b), K split over kSplitK CTAs (blockIdx.x);
+// the partial Grams go to Xp (free at this point), bt_tfactor_kernel sums them.
 __global__ void __launch_bounds__(BG_THREADS) bt_gram_kernel(BackWs w) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int b = blockIdx.z, cb = b * kNBT;
     const int nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
     if (m <= 0) return;
+    const int chunk = (((m + kSplitK - 1) / kSplitK) + 15) & ~15;
+    const int k0 = blockIdx.x * chunk;
+    const int klen = min(chunk, m - k0);
     GemmProblem<cplx, cplx> p;
-    p.A = w.A + (size_t)cb * w.lda + cb + 1; p.lda = w.lda; p.B = p.A; p.ldb = w.lda;
-    p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = nbw; p.K = m; p.K2 = 0;
-    StoreEpi epi{w.Tm + (size_t)b * kNBT * kNBT, kNBT};
+    p.A = w.A + (size_t)cb * w.lda + cb + 1 + k0; p.lda = w.lda; p.B = p.A; p.ldb = w.lda;
+    p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = nbw; p.K = klen > 0 ? klen : 0; p.K2 = 0;
+    StoreEpi epi{w.Xp + ((size_t)b * kSplitK + blockIdx.x) * kNBT * kNBT, kNBT};
     gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, 0, 0, smem_raw, epi);
 }
 
-// T_b from the Gram matrix by the forward recurrence  T(0:j, j) = -tau_j T(0:j,0:j) G(0:j, j), T(j,j) = tau_j
+// T_b from the Gram matrix by the forward recurrence  T(0:j, j) = -tau_j T(0:j,0:j) G(0:j, j), T(j,j) = tau_j,
+// in shared memory (64 KB): thread t owns row t of T and only re-reads its own earlier writes.
 __global__ void __launch_bounds__(kNBT) bt_tfactor_kernel(BackWs w) {
-    // In place over the Gram matrix (global, column-major 64 x 64): thread t owns row t of T and only
-    // re-reads its own earlier writes; column j of G is staged through shared memory first.
-    __shared__ cplx g[kNBT];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *T = reinterpret_cast<cplx *>(smem_raw);       // kNBT x kNBT, column-major; holds G first
     const int b = blockIdx.x, cb = b * kNBT, t = threadIdx.x;
     const int nbw = min(kNBT, w.n - cb);
-    cplx *T = w.Tm + (size_t)b * kNBT * kNBT;
+    const cplx *part = w.Xp + (size_t)b * kSplitK * kNBT * kNBT;
+    for (int e = t; e < kNBT * kNBT; e += kNBT) {
+        const int r = e % kNBT, c = e / kNBT;
+        cplx s = mk(0.0, 0.0);
+        if (r < nbw && c < nbw) {
+#pragma unroll
+            for (int k = 0; k < kSplitK; ++k) s = s + part[(size_t)k * kNBT * kNBT + e];
+        }
+        T[e] = s;
+    }
+    __syncthreads();
     for (int j = 0; j < kNBT; ++j) {
         const cplx tj = (j < nbw) ? w.tau[cb + j] : mk(0.0, 0.0);
-        if (t < j) g[t] = T[j * kNBT + t];
-        __syncthreads();
         cplx v = mk(0.0, 0.0);
         if (j < nbw) {
             if (t < j) {
                 cplx s = mk(0.0, 0.0);
-                for (int k = t; k < j; ++k) cfma(s, T[k * kNBT + t], g[k]);     // row t of T(0:j,0:j) times g
+                for (int k = t; k < j; ++k) cfma(s, T[k * kNBT + t], T[j * kNBT + k]);     // row t of T(0:j,0:j) times G(0:j,j)
                 v = mk(-tj.x, -tj.y) * s;
             } else if (t == j) v = tj;
         }
+        __syncthreads();              // every thread has read column j of G
         T[j * kNBT + t] = v;
         __syncthreads();
     }
+    cplx *Tg = w.Tm + (size_t)b * kNBT * kNBT;
+    for (int e = t; e < kNBT * kNBT; e += kNBT) Tg[e] = T[e];
 }
 
 // VT_b = V_b T_b  (blockIdx.z = b, blockIdx.x = row tile)
@@ -172,6 +187,7 @@ int backherk_init() {
     if (g_bh_init_dev == dev) return 0;
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(cplx) * kNBT * kNBT));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
@@ -193,9 +209,9 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     scale_convert_kernel<<<dim3((n + 1023) / 1024, n), 256, 0, st>>>(n, lam, Zt, ldzt, w.Zc, w.ldz, w.cnt);
     HPSD_LAUNCH_CHECK();
     // compact-WY factors of all blocks (off the dependent chain: batched over blocks)
-    bt_gram_kernel<<<dim3(1, 1, nblocks), BG_THREADS, kSmemKK, st>>>(w);
+    bt_gram_kernel<<<dim3(kSplitK, 1, nblocks), BG_THREADS, kSmemKK, st>>>(w);
     HPSD_LAUNCH_CHECK();
-    bt_tfactor_kernel<<<nblocks, kNBT, 0, st>>>(w);
+    bt_tfactor_kernel<<<nblocks, kNBT, sizeof(cplx) * kNBT * kNBT, st>>>(w);
     HPSD_LAUNCH_CHECK();
     bt_vt_kernel<<<dim3(nt, 1, nblocks), BG_THREADS, kSmemMK, st>>>(w);
     HPSD_LAUNCH_CHECK();

@@ -65,7 +65,7 @@ LargeWs carve(int n, unsigned char *base) {
     w.b.VT = cpx((size_t)N * n);
     w.b.Tm = cpx((size_t)nblocks * kNBT * kNBT);
     w.b.Zc = cpx((size_t)N * n);
-    w.b.Xp = cpx((size_t)kSplitK * kNBT * n);
+    w.b.Xp = cpx((size_t)kSplitK * kNBT * align_up((size_t)n, kNBT));
     w.b.X = cpx((size_t)kNBT * n);
     w.b.cnt = itg(8);
     w.bytes = off;

@@ -79,10 +79,11 @@ __device__ __forceinline__ void householder_scalars(cplx alpha, double xnorm2, d
     } else {
         const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
         beta = -copysign(nrm, alpha.x);
-        tau = mk((beta - alpha.x) / beta, -alpha.y / beta);
+        const double ib = 1.0 / beta;
+        tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
         const cplx den = mk(alpha.x - beta, alpha.y);
-        const double d2 = abs2(den);
-        scale = mk(den.x / d2, -den.y / d2);
+        const double id2 = 1.0 / abs2(den);
+        scale = mk(den.x * id2, -den.y * id2);
     }
 }
 
@@ -131,6 +132,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     constexpr int PSTRIDE = 2 * kNB + 1;
     const int T = p.T, q = p.q;
     const bool streaming = q > kSlots;
+    const bool wide = q <= 2;                       // block-uniform
 
     // ---------------- tile slots: this warp owns slots `warp` and (for warps 0..3) `warp + 8` ---------
     // tile k of this CTA is tiles[g + k G]; it lives in slot k % kSlots, served by warp (k % kSlots) % 8.
@@ -177,6 +179,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             p.part[(size_t)g * PSTRIDE] = mk(t, 0.0);
         }
     }
+    if (wide) cp_async_wait<0>();      // the slots are read by other warps in wide mode
     grid.sync();
 
     for (int i = 0; i < p.nbp; ++i) {
@@ -188,11 +191,21 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         // Tiles are walked forwards on even columns and backwards on odd ones: when they stream, the tail
         // of one pass is the head of the next, so it is still in the slots / in L2.
         const bool fwd = (i & 1) == 0;
+        // wide mode (at most two tiles per CTA): four warps share a tile, eight columns each
+        const int wtile = warp >> 2, wq = warp & 3;
+        const bool wvalid = wide && wtile < q && g + wtile * G < T;
         cplx rawI[2], rawJ[2];
 #pragma unroll
         for (int jj = 0; jj < 2; ++jj) {
             rawI[jj] = mk(0.0, 0.0); rawJ[jj] = mk(0.0, 0.0);
-            if (jj < cnt) {
+            if (wide) {
+                if (jj == 0 && wvalid) {
+                    const int2 ij = p.tiles[g + wtile * G];
+                    const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
+                    if (rI < n && rI > c + 1) rawI[0] = ldcg_(&A[(size_t)c * lda + rI]);
+                    if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[0] = ldcg_(&A[(size_t)c * lda + rJ]);
+                }
+            } else if (jj < cnt) {
                 const int j = fwd ? jj : cnt - 1 - jj;
                 const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
                 const int2 ij = p.tiles[g + k * G];
@@ -230,7 +243,60 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         if (reducer && lane == 0)     // row c+1 term (v = 1 there) plus scale * sum over rows >= c+2
             p.tot[(g / kNB) * kNB + (g % kNB)] = conj_(red_top) + scale * red_s;
         double qacc = 0.0;
-        {
+        if (wide) {
+            cplx *vI = s_v + warp * 2 * kTS, *vJ = vI + kTS;
+            cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0);
+            int2 ij = make_int2(0, 0);
+            if (wvalid) {
+                ij = p.tiles[g + wtile * G];
+                const bool diag = (ij.x == ij.y);
+                const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
+                const cplx a = (rI == c + 1) ? mk(1.0, 0.0) : scale * rawI[0];
+                const cplx b = diag ? a : ((rJ == c + 1) ? mk(1.0, 0.0) : scale * rawJ[0]);
+                vI[lane] = a; vJ[lane] = b;
+                __syncwarp();
+                const cplx *sl = s_slots + (size_t)wtile * kSlotElems;
+                if (!diag) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int cc = wq * 8 + u;
+                        cfma(accR, sl[cc * kTP + lane], vJ[cc]);
+                        cfma_conj(accC, sl[lane * kTP + cc], vI[cc]);
+                    }
+                } else {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int cc = wq * 8 + u;
+                        cplx x = sl[cc * kTP + lane];
+                        x.x = (lane >= cc) ? x.x : 0.0;
+                        x.y = (lane > cc) ? x.y : 0.0;
+                        cfma(accR, x, vJ[cc]);
+                        cplx y = sl[lane * kTP + cc];
+                        y.x = (cc > lane) ? y.x : 0.0;
+                        y.y = (cc > lane) ? y.y : 0.0;
+                        cfma_conj(accC, y, vI[cc]);
+                    }
+                }
+            }
+            s_gV[warp * 32 + lane] = accR;
+            s_gW[warp * 32 + lane] = accC;
+            __syncthreads();
+            if (wvalid && wq == 0) {
+#pragma unroll
+                for (int u = 1; u < 4; ++u) { accR = accR + s_gV[(warp + u) * 32 + lane]; accC = accC + s_gW[(warp + u) * 32 + lane]; }
+                double qterm;
+                if (ij.x == ij.y) {
+                    const cplx sdiag = accR + accC;
+                    p.PR[(size_t)ij.y * ldp + ij.x * kTS + lane] = sdiag;
+                    qterm = vI[lane].x * sdiag.x + vI[lane].y * sdiag.y;
+                } else {
+                    p.PR[(size_t)ij.y * ldp + ij.x * kTS + lane] = accR;
+                    p.PC[(size_t)ij.x * ldp + ij.y * kTS + lane] = accC;
+                    qterm = 2.0 * (vI[lane].x * accR.x + vI[lane].y * accR.y);
+                }
+                qacc = warp_sum(qterm);
+            }
+        } else {
             cplx *vI = s_v + warp * 2 * kTS, *vJ = vI + kTS;
             {
                 for (int jj = 0; jj < cnt; ++jj) {
@@ -372,6 +438,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 double re = 0.0;
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
+                    if (warp + 8 * k >= i) continue;             // warp-uniform
                     // rows c+1 of V and W sit in the helper lane
                     const cplx v1 = mk(__shfl_sync(0xffffffffu, Vr[k].x, 31), __shfl_sync(0xffffffffu, Vr[k].y, 31));
                     const cplx w1 = mk(__shfl_sync(0xffffffffu, Wr[k].x, 31), __shfl_sync(0xffffffffu, Wr[k].y, 31));
