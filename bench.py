@@ -58,7 +58,7 @@ def stage_flops(stage: str, sizes, kpos, jmax: int) -> float:
             tot += 8.0 * n * n * k
         elif stage == "S7S8_herk_pack" and large:
             tot += 4.0 * n * n * k
-        elif stage == "S9S10_jacobi" and 2 <= n <= jmax:
+        elif stage in ("S9_jacobi", "S10_householder_ql") and 2 <= n <= jmax:
             tot += f_alg(n, k)
     return tot
 
@@ -200,7 +200,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     hp.load_library()
-    jmax = 84
+    jmax = 116
 
     def device_inputs(c):
         w = workloads.make(c)

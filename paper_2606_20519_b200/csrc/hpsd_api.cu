@@ -48,11 +48,15 @@ void prof_end_(int stage, cudaStream_t st) {
 namespace {
 
 struct Options {
-    int jacobi_max_n = kJacobiMaxN;   // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
+    int jacobi_max_n = 40;            // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
+    int medium_max_n = kMediumMaxN;   // blocks with jacobi_max_n < n <= this use the one-CTA Householder + QL kernel
 } g_opt;
+
+inline int small_limit(const Options &o) { return o.medium_max_n > o.jacobi_max_n ? o.medium_max_n : o.jacobi_max_n; }
 
 struct JacobiGroup {
     int n, count;
+    bool medium;        // Householder + QL kernel instead of Jacobi
     size_t off_index;   // index (in long long units) of this group's offsets in the descriptor buffer
     size_t idx_index;   // index (in int units) of this group's info indices
 };
@@ -61,7 +65,7 @@ struct LargeBlock { int n; long long off; int idx; };
 
 struct Plan {
     std::vector<int> sizes;
-    int jacobi_max_n;
+    int jacobi_max_n, medium_max_n;
     std::vector<JacobiGroup> groups;
     std::vector<LargeBlock> large;
     int n_scalar = 0;
@@ -97,6 +101,8 @@ int init_device(DeviceState &ds) {
     if (rc) return rc;
     rc = largepath_init();
     if (rc) return rc;
+    rc = medium_init();
+    if (rc) return rc;
     ds.inited = true;
     return 0;
 }
@@ -104,6 +110,8 @@ int init_device(DeviceState &ds) {
 int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     pl.sizes.assign(sizes, sizes + n_blocks);
     pl.jacobi_max_n = g_opt.jacobi_max_n;
+    pl.medium_max_n = g_opt.medium_max_n;
+    const int lim = small_limit(g_opt);
     std::vector<long long> ll;
     std::vector<int> ints;
     std::map<int, std::vector<std::pair<long long, int>>> by_n;
@@ -112,8 +120,8 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     for (int b = 0; b < n_blocks; ++b) {
         const int n = sizes[b];
         if (n == 1) scalars.push_back(off);
-        else if (n >= 2 && n <= pl.jacobi_max_n) by_n[n].push_back({off, b});
-        else if (n > pl.jacobi_max_n) pl.large.push_back({n, off, b});
+        else if (n >= 2 && n <= lim) by_n[n].push_back({off, b});
+        else if (n > lim) pl.large.push_back({n, off, b});
         off += (long long)n * n;
     }
     pl.n_scalar = (int)scalars.size();
@@ -122,6 +130,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     for (auto &kv : by_n) {
         JacobiGroup g;
         g.n = kv.first; g.count = (int)kv.second.size();
+        g.medium = g.n > pl.jacobi_max_n;
         g.off_index = ll.size(); g.idx_index = ints.size();
         for (auto &pr : kv.second) { ll.push_back(pr.first); ints.push_back(pr.second); }
         pl.groups.push_back(g);
@@ -157,7 +166,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
 // synchronises (cudaMalloc/cudaMemcpy); later calls with the same list are launch-only.
 int get_plan(DeviceState &ds, int n_blocks, const int *sizes, Plan **out) {
     for (auto &p : ds.plans) {
-        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n &&
+        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n &&
             (n_blocks == 0 || std::memcmp(p->sizes.data(), sizes, sizeof(int) * n_blocks) == 0)) {
             *out = p.get();
             return 0;
@@ -201,9 +210,10 @@ int run_plan(const Plan &pl, const double *in, double *out, void *ws, int *info_
         if (rc) return rc;
     }
     for (const JacobiGroup &g : pl.groups) {
-        prof_begin(ST_JACOBI, st);
-        rc = launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st);
-        prof_end(ST_JACOBI, st);
+        prof_begin(g.medium ? ST_MEDIUM : ST_JACOBI, st);
+        rc = g.medium ? launch_hhql_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st)
+                      : launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st);
+        prof_end(g.medium ? ST_MEDIUM : ST_JACOBI, st);
         if (rc) return rc;
     }
     for (const LargeBlock &lb : pl.large) {
@@ -245,6 +255,11 @@ int hpsd_set_option(const char *name, int value) {
         g_opt.jacobi_max_n = value;
         return HPSD_OK;
     }
+    if (std::strcmp(name, "medium_max_n") == 0) {
+        if (value < 0 || value > kMediumMaxN) return HPSD_EINVAL;
+        g_opt.medium_max_n = value;
+        return HPSD_OK;
+    }
     return HPSD_EINVAL;
 }
 
@@ -254,7 +269,7 @@ int hpsd_profile_stage_count(void) { return ST_COUNT; }
 
 const char *hpsd_profile_stage_name(int stage) {
     static const char *names[ST_COUNT] = {"S1_unpack", "S2S3_tridiag_panel", "S2_her2k_trailing", "S4_stedc",
-                                          "S5S6_backtransform", "S7S8_herk_pack", "S9S10_jacobi", "n1_clamp"};
+                                          "S5S6_backtransform", "S7S8_herk_pack", "S9_jacobi", "S10_householder_ql", "n1_clamp"};
     return (stage >= 0 && stage < ST_COUNT) ? names[stage] : "";
 }
 
@@ -279,7 +294,7 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     if (rc) return rc;
     size_t ws = 0;
     for (int b = 0; b < n_blocks; ++b)
-        if (sizes[b] > g_opt.jacobi_max_n) {
+        if (sizes[b] > small_limit(g_opt)) {
             const size_t w = largepath_ws_bytes(sizes[b]);
             if (w > ws) ws = w;
         }
@@ -390,10 +405,11 @@ static int single_large_setup(int n, void **ws_out, Plan **pl_out) {
     DeviceState &ds = g_dev[dev];
     int rc = init_device(ds);
     if (rc) return rc;
-    const int saved = g_opt.jacobi_max_n;
+    const Options saved = g_opt;
     g_opt.jacobi_max_n = 1;                 // force the large-path plan for any n >= 2
+    g_opt.medium_max_n = 0;
     rc = get_plan(ds, 1, sizes, pl_out);
-    g_opt.jacobi_max_n = saved;
+    g_opt = saved;
     if (rc) return rc;
     const size_t need = largepath_ws_bytes(n) + 1024;
     if (ds.ws_bytes < need) {

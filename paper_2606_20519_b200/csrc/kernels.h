@@ -20,6 +20,14 @@ int launch_jacobi_project(int n, int count, const long long *offs_dev, const dou
                           int *info_dev, const int *info_idx_dev, cudaStream_t st);
 int jacobi_init();  // set kernel attributes once per device
 
+// ---- medium.cu (S10) ----------------------------------------------------------
+// Batched one-CTA-per-matrix Householder + implicit-QL projection for blocks of one size n,
+// jacobi_max_n < n <= kMediumMaxN (the matrix must fit in shared memory: 16 n (n|1) + O(n) bytes).
+constexpr int kMediumMaxN = 116;
+int launch_hhql_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+                        int *info_dev, const int *info_idx_dev, cudaStream_t st);
+int medium_init();
+
 // ---- peak.cu ---------------------------------------------------------------
 int launch_fp64_probe(int kind, int iters, double *flops_host, cudaStream_t st);
 

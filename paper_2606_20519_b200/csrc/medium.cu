@@ -1,0 +1,409 @@
+// medium.cu -- S10 of SURVEY.md §8(a): medium blocks (jacobi_max_n < n <= kMediumMaxN), batched.
+// One CTA per matrix, the whole matrix in shared memory, one kernel from svec to svec:
+//   S1 unpack -> Householder tridiagonalisation (unblocked, rank-2 updates) -> Q formed IN PLACE over the
+//   reflectors -> implicit QL with Wilkinson shift on (d, e), the real rotations applied to the complex
+//   columns of Q -> S6 clamp/scale -> S7 W W^H -> S8 pack.
+// Operation defined at PAPER.md:1536; layout Eq. (D10) PAPER.md:1220-1222.
+//
+// The serial part of QL (the rotation parameters, ~1.7 n^2/2 of them, each a dependent chain of about
+// 150 cycles) is produced by ONE thread running ahead through a ring buffer in shared memory; the other
+// warps apply the rotations to the rows of Q as the batches become ready.  The generator depends only on
+// (d, e), never on Q, so the two never wait on each other except through the ring.
+//
+// Only one n x n complex array is needed (105 KB at n = 81: two CTAs per SM, so 256 matrices are one wave).
+#include "kernels.h"
+
+namespace hpsd {
+
+constexpr int kMedThreads = 256;
+constexpr int kRing = 128;                 // rotations in flight between generator and appliers
+constexpr int kMedMaxIter = 60;            // QL iterations per eigenvalue before giving up
+
+struct MedSmem {
+    cplx *A;            // n x ld: matrix -> reflectors -> Q
+    cplx *tau;          // n
+    cplx *x;            // n : Householder vector / work row
+    cplx *y;            // n : A v, then w
+    double *d, *e;      // n each
+    double *rc, *rs;    // kRing each
+    int *ri;            // kRing : column index i of the rotation (acts on columns i, i+1)
+    double *red;        // 32
+    volatile int *ctl;  // [0] produced, [1] done flag, [2] info, [3] consumed (min over appliers, lazily)
+};
+
+__host__ __device__ inline int med_ld(int n) { return n | 1; }
+
+__host__ __device__ inline size_t med_smem_bytes(int n) {
+    const size_t ld = med_ld(n);
+    return sizeof(cplx) * ((size_t)n * ld + 3 * (size_t)n) + sizeof(double) * (2 * (size_t)n + 2 * kRing + 32) +
+           sizeof(int) * (kRing + 16) + 64;
+}
+
+__device__ __forceinline__ MedSmem med_carve(unsigned char *base, int n) {
+    MedSmem sm;
+    const int ld = med_ld(n);
+    sm.A = reinterpret_cast<cplx *>(base);
+    sm.tau = sm.A + (size_t)n * ld;
+    sm.x = sm.tau + n;
+    sm.y = sm.x + n;
+    sm.d = reinterpret_cast<double *>(sm.y + n);
+    sm.e = sm.d + n;
+    sm.rc = sm.e + n;
+    sm.rs = sm.rc + kRing;
+    sm.red = sm.rs + kRing;
+    sm.ri = reinterpret_cast<int *>(sm.red + 32);
+    sm.ctl = sm.ri + kRing;
+    return sm;
+}
+
+// block-wide sum of one double (every thread gets the result); red has >= 9 entries
+__device__ __forceinline__ double block_sum(double v, double *red) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < kMedThreads / 32; ++w) t += red[w];
+    return t;
+}
+__device__ __forceinline__ cplx block_sum(cplx v, double *red) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5] = v.x; red[8 + (threadIdx.x >> 5)] = v.y; }
+    __syncthreads();
+    cplx t = mk(0.0, 0.0);
+#pragma unroll
+    for (int w = 0; w < kMedThreads / 32; ++w) { t.x += red[w]; t.y += red[8 + w]; }
+    return t;
+}
+
+// zlarfg semantics (same conventions as tridiag.cu): H^H (alpha; x) = (beta; 0), H = I - tau v v^H, v = (1; scale x)
+__device__ __forceinline__ void med_householder(cplx alpha, double xnorm2, double &beta, cplx &tau, cplx &scale) {
+    if (xnorm2 == 0.0 && alpha.y == 0.0) {
+        beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
+    } else {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        beta = -copysign(nrm, alpha.x);
+        const double ib = 1.0 / beta;
+        tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
+        const cplx den = mk(alpha.x - beta, alpha.y);
+        const double id2 = 1.0 / abs2(den);
+        scale = mk(den.x * id2, -den.y * id2);
+    }
+}
+
+// ---- phase 1: A (full Hermitian, shared memory) -> real tridiagonal (d, e), reflectors in the lower part
+__device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
+    cplx *A = sm.A;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int c = 0; c < n - 1; ++c) {
+        const int m = n - c - 1;
+        double S = 0.0;
+        for (int r = c + 2 + tid; r < n; r += kMedThreads) S += abs2(A[(size_t)c * ld + r]);
+        S = block_sum(S, sm.red);
+        const cplx alpha = A[(size_t)c * ld + c + 1];
+        double beta; cplx tau, scale;
+        med_householder(alpha, S, beta, tau, scale);
+        if (tid == 0) { sm.d[c] = A[(size_t)c * ld + c].x; sm.e[c] = beta; sm.tau[c] = tau; }
+        __syncthreads();                                   // alpha read by everyone before it is overwritten
+        for (int r = c + 1 + tid; r < n; r += kMedThreads) {
+            const cplx v = (r == c + 1) ? mk(1.0, 0.0) : scale * A[(size_t)c * ld + r];
+            sm.x[r] = v;
+            A[(size_t)c * ld + r] = v;
+        }
+        __syncthreads();
+        if (tau.x == 0.0 && tau.y == 0.0) continue;        // H = I (block-uniform)
+        // y = A22 v : 64 rows per pass, 4 column classes per row (lane >> 3), reduced by shuffles
+        cplx q = mk(0.0, 0.0);
+        for (int base = 0; base < m; base += 64) {
+            const int r = c + 1 + base + (lane & 7) + 8 * warp;
+            cplx acc = mk(0.0, 0.0);
+            if (r < n)
+                for (int j = c + 1 + (lane >> 3); j < n; j += 4) cfma(acc, A[(size_t)j * ld + r], sm.x[j]);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+            if (r < n && lane < 8) {
+                sm.y[r] = acc;
+                cfma_conj(q, sm.x[r], acc);                 // conj(v_r) y_r
+            }
+        }
+        q = block_sum(q, sm.red);
+        const double alphap = -0.5 * abs2(tau) * q.x;       // v^H A v is real
+        for (int r = c + 1 + tid; r < n; r += kMedThreads) sm.y[r] = tau * sm.y[r] + alphap * sm.x[r];
+        __syncthreads();
+        // A22 -= v w^H + w v^H on the full trailing block
+        for (int e = tid; e < m * m; e += kMedThreads) {
+            const int rr = e % m, jj = e / m;
+            const int r = c + 1 + rr, j = c + 1 + jj;
+            cplx a = A[(size_t)j * ld + r];
+            const cplx vr = sm.x[r], wr = sm.y[r], vj = sm.x[j], wj = sm.y[j];
+            // v_r conj(w_j) + w_r conj(v_j)
+            a.x -= vr.x * wj.x + vr.y * wj.y + wr.x * vj.x + wr.y * vj.y;
+            a.y -= vr.y * wj.x - vr.x * wj.y + wr.y * vj.x - wr.x * vj.y;
+            if (r == j) a.y = 0.0;
+            A[(size_t)j * ld + r] = a;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) { sm.d[n - 1] = A[(size_t)(n - 1) * ld + n - 1].x; sm.e[n - 1] = 0.0; sm.tau[n - 1] = mk(0.0, 0.0); }
+    __syncthreads();
+}
+
+// ---- phase 2: Q = H_0 H_1 ... H_{n-2} formed in place over the reflectors (backward accumulation)
+__device__ void med_form_q(const MedSmem &sm, int n, int ld) {
+    cplx *A = sm.A;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int k = n - 2; k >= 0; --k) {
+        const cplx tau = sm.tau[k];
+        const int m2 = n - k - 2;                           // size of the already formed block B = A[k+2:, k+2:]
+        // z_j = sum_{r >= k+2} conj(x_r) B[r, j],  x = A[k+2:, k]
+        for (int base = 0; base < m2; base += 64) {
+            const int j = k + 2 + base + (lane & 7) + 8 * warp;
+            cplx acc = mk(0.0, 0.0);
+            if (j < n)
+                for (int r = k + 2 + (lane >> 3); r < n; r += 4) cfma_conj(acc, A[(size_t)k * ld + r], A[(size_t)j * ld + r]);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+            if (j < n && lane < 8) sm.y[j] = acc;
+        }
+        __syncthreads();
+        const cplx mtau = mk(-tau.x, -tau.y);
+        const int m1 = m2 + 1;                              // block C = A[k+1:, k+1:]
+        for (int e = tid; e < m1 * m1; e += kMedThreads) {
+            const int rr = e % m1, jj = e / m1;
+            const int r = k + 1 + rr, j = k + 1 + jj;
+            cplx v;
+            if (rr == 0 && jj == 0) v = mk(1.0 - tau.x, -tau.y);
+            else if (rr == 0) v = mtau * sm.y[j];
+            else if (jj == 0) v = mtau * A[(size_t)k * ld + r];
+            else v = A[(size_t)j * ld + r] + (mtau * A[(size_t)k * ld + r]) * sm.y[j];
+            A[(size_t)j * ld + r] = v;
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < n; e += kMedThreads) {
+        A[(size_t)e * ld] = mk(e == 0 ? 1.0 : 0.0, 0.0);    // row 0
+        A[e] = mk(e == 0 ? 1.0 : 0.0, 0.0);                 // column 0
+    }
+    __syncthreads();
+}
+
+// ---- phase 3: implicit QL (tql2 scheme).  Thread 0 generates the rotations, warps 1.. apply them to Q.
+// ctl[0] = rotations produced, ctl[1] = generator finished, ctl[2] = failure flag, ctl[4 + w] = consumed by warp w
+__device__ void med_ql_generate(const MedSmem &sm, int n) {
+    double *d = sm.d, *e = sm.e;
+    volatile int *ctl = sm.ctl;
+    int produced = 0, safe = kRing;         // slots below `safe` may be written without asking the appliers
+    double an = 0.0;
+    for (int k = 0; k < n; ++k) an = fmax(an, fabs(d[k]) + fabs(e[k]));
+    bool fail = false;
+    for (int l = 0; l < n && !fail; ++l) {
+        int iter = 0;
+        for (;;) {
+            int mm;
+            for (mm = l; mm < n - 1; ++mm) {
+                const double s = fabs(d[mm]) + fabs(d[mm + 1]);
+                if (fabs(e[mm]) <= kEps * s || fabs(e[mm]) <= kEps * an) break;
+            }
+            if (mm == l) break;
+            if (++iter > kMedMaxIter) { fail = true; break; }
+            double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+            double r = sqrt(g * g + 1.0);
+            if (!(fabs(g) < 1e150)) r = fabs(g);
+            g = d[mm] - d[l] + e[l] / (g + copysign(r, g));
+            double s = 1.0, c = 1.0, p = 0.0;
+            int i;
+            bool under = false;
+            // d[i+1] at step i is the (unchanged) d[i] read at step i+1: carried in a register;
+            // e[i], d[i] of the next step are loaded before the dependent chain of this one
+            double dnext = d[mm];
+            double ei = e[mm - 1], di = d[mm - 1];
+            for (i = mm - 1; i >= l; --i) {
+                const double f = s * ei, b = c * ei;
+                const double dcur = di;
+                if (i > l) { ei = e[i - 1]; di = d[i - 1]; }
+                const double h2 = fma(f, f, g * g);
+                double r, ir;
+                if (h2 > 1e-280 && h2 < 1e280) {
+                    ir = rsqrt(h2);
+                    ir = ir * fma(-0.5 * h2 * ir, ir, 1.5);     // one Newton step: 1/sqrt(h2) to working precision
+                    r = h2 * ir;
+                } else {
+                    r = hypot(f, g);
+                    if (r == 0.0) { e[i + 1] = 0.0; d[i + 1] = dnext - p; e[mm] = 0.0; under = true; break; }
+                    ir = 1.0 / r;
+                }
+                e[i + 1] = r;
+                s = f * ir; c = g * ir;
+                g = dnext - p;
+                r = (dcur - g) * s + 2.0 * c * b;
+                p = s * r;
+                d[i + 1] = g + p;
+                g = c * r - b;
+                dnext = dcur;
+                // emit rotation (i, c, s)
+                if (produced >= safe) {
+                    __threadfence_block();
+                    ctl[0] = produced;                     // let the appliers drain everything produced so far
+                    int mn;
+                    do {
+                        mn = ctl[4 + 1];
+                        for (int w = 2; w < kMedThreads / 32; ++w) mn = min(mn, ctl[4 + w]);
+                    } while (produced - mn >= kRing);
+                    safe = mn + kRing;
+                }
+                const int slot = produced & (kRing - 1);
+                sm.ri[slot] = i; sm.rc[slot] = c; sm.rs[slot] = s;
+                ++produced;
+                if ((produced & 15) == 0) { __threadfence_block(); ctl[0] = produced; }
+            }
+            if (!under) { d[l] -= p; e[l] = g; e[mm] = 0.0; }
+            __threadfence_block();
+            ctl[0] = produced;
+        }
+    }
+    __threadfence_block();
+    ctl[0] = produced;
+    if (fail) ctl[2] = 1;
+    __threadfence_block();
+    ctl[1] = 1;
+}
+
+__device__ void med_ql_apply(const MedSmem &sm, int n, int ld) {
+    volatile int *ctl = sm.ctl;
+    const int warp = threadIdx.x >> 5;
+    const int a = threadIdx.x - 32;                   // applier index: (row, component) pairs, 2n of them
+    const int na = kMedThreads - 32;
+    double *Z = reinterpret_cast<double *>(sm.A);
+    int consumed = 0;
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        int done = 0, avail = 0;
+        if (lane == 0) { done = ctl[1]; avail = ctl[0]; }   // done first: if it is set, avail is final
+        done = __shfl_sync(0xffffffffu, done, 0);
+        avail = __shfl_sync(0xffffffffu, avail, 0);
+        if (avail == consumed) {
+            if (done) break;
+            continue;
+        }
+        __threadfence_block();
+        for (; consumed < avail; ++consumed) {
+            const int slot = consumed & (kRing - 1);
+            const int i = sm.ri[slot];
+            const double c = sm.rc[slot], s = sm.rs[slot];
+            for (int t = a; t < 2 * n; t += na) {
+                double *z0 = Z + 2 * (size_t)i * ld + t, *z1 = z0 + 2 * (size_t)ld;
+                const double q = *z0, f = *z1;
+                *z1 = s * q + c * f;
+                *z0 = c * q - s * f;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) ctl[4 + warp] = consumed;
+    }
+}
+
+#ifdef HPSD_PANEL_TRACE
+__device__ long long g_med_trace[8];
+extern "C" int hpsd_debug_medium(long long *out) { cudaMemcpyFromSymbol(out, g_med_trace, sizeof(long long) * 8); return 0; }
+#define MTRACE(k) do { if (threadIdx.x == 0 && blockIdx.x == 0) g_med_trace[k] = clock64(); } while (0)
+#else
+#define MTRACE(k) do {} while (0)
+#endif
+
+__global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const long long *__restrict__ offs,
+                                                                   const double *__restrict__ in, double *__restrict__ out,
+                                                                   int *__restrict__ info, const int *__restrict__ info_idx) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ld = med_ld(n);
+    MedSmem sm = med_carve(smem_raw, n);
+    cplx *A = sm.A;
+    const int tid = threadIdx.x;
+    const double *sv = in + offs[blockIdx.x];
+    double *ov = out + offs[blockIdx.x];
+
+    // ---- S1: unpack into shared memory, both triangles
+    for (int t = tid; t < n * n; t += kMedThreads) {
+        const int j = t / n, i = t % n;
+        if (i < j) continue;
+        const double *c = sv + svec_col_off(n, j);
+        if (i == j) A[(size_t)j * ld + i] = mk(c[0], 0.0);
+        else {
+            const int k = i - j - 1;
+            const cplx v = mk(c[1 + 2 * k] / kSqrt2, c[2 + 2 * k] / kSqrt2);
+            A[(size_t)j * ld + i] = v;
+            A[(size_t)i * ld + j] = conj_(v);
+        }
+    }
+    if (tid < 16) sm.ctl[tid] = 0;
+    __syncthreads();
+
+    MTRACE(0);
+    med_tridiagonalize(sm, n, ld);
+    MTRACE(1);
+    med_form_q(sm, n, ld);
+    MTRACE(2);
+
+    if (tid == 0) { med_ql_generate(sm, n); MTRACE(3); }
+    else if (tid >= 32) med_ql_apply(sm, n, ld);
+    __syncthreads();
+    MTRACE(4);
+#ifdef HPSD_PANEL_TRACE
+    if (tid == 0 && blockIdx.x == 0) g_med_trace[6] = sm.ctl[0];
+#endif
+    if (info != nullptr && tid == 0) info[info_idx[blockIdx.x]] = sm.ctl[2] ? 4 : 0;
+
+    // ---- S6: clamp, W = Q_+ diag(sqrt(lambda_+)); the positive columns are scaled in place
+    int *poslist = reinterpret_cast<int *>(sm.x);            // x, y are dead now (n cplx >= n ints)
+    if (tid == 0) {
+        int k = 0;
+        for (int l = 0; l < n; ++l)
+            if (sm.d[l] > 0.0) poslist[k++] = l;
+        sm.ctl[3] = k;
+    }
+    __syncthreads();
+    const int kpos = sm.ctl[3];
+    for (int t = tid; t < kpos * n; t += kMedThreads) {
+        const int l = poslist[t / n], i = t % n;
+        A[(size_t)l * ld + i] = sqrt(sm.d[l]) * A[(size_t)l * ld + i];
+    }
+    __syncthreads();
+    // ---- S7 + S8: lower triangle of W W^H straight into the svec
+    for (int t = tid; t < n * n; t += kMedThreads) {
+        const int j = t / n, i = t % n;
+        if (i < j) continue;
+        cplx acc = mk(0.0, 0.0);
+        for (int k = 0; k < kpos; ++k) {
+            const int l = poslist[k];
+            const cplx a = A[(size_t)l * ld + i], b = A[(size_t)l * ld + j];
+            acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+            acc.y = fma(a.y, b.x, acc.y); acc.y = fma(-a.x, b.y, acc.y);
+        }
+        double *c = ov + svec_col_off(n, j);
+        if (i == j) c[0] = acc.x;
+        else {
+            const int k = i - j - 1;
+            c[1 + 2 * k] = kSqrt2 * acc.x;
+            c[2 + 2 * k] = kSqrt2 * acc.y;
+        }
+    }
+    MTRACE(5);
+}
+
+int medium_init() {
+    const int maxb = (int)med_smem_bytes(kMediumMaxN);
+    if (cudaFuncSetAttribute(hhql_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, maxb) != cudaSuccess) return HPSD_ECUDA_;
+    return 0;
+}
+
+int launch_hhql_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+                        int *info_dev, const int *info_idx_dev, cudaStream_t st) {
+    if (count <= 0) return 0;
+    if (n < 2 || n > kMediumMaxN) return -1;
+    hhql_project_kernel<<<count, kMedThreads, med_smem_bytes(n), st>>>(n, offs_dev, in, out, info_dev, info_idx_dev);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
+}  // namespace hpsd

@@ -13,7 +13,8 @@ enum Stage {
     ST_STEDC,           // S4
     ST_BACK,            // S5 + S6
     ST_HERK_PACK,       // S7 + S8
-    ST_JACOBI,          // S9 / S10
+    ST_JACOBI,          // S9
+    ST_MEDIUM,          // S10
     ST_SCALAR,          // n = 1 blocks
     ST_COUNT
 };

@@ -27,6 +27,12 @@ def hp():
     return lib
 
 
+def force_large(hp, on):
+    """Route every block through S1..S8 of the multi-kernel path (on) or restore the defaults (off)."""
+    hp.set_option("jacobi_max_n", 1 if on else 40)
+    hp.set_option("medium_max_n", 0 if on else 116)
+
+
 def gpu_project(hp, sizes, sv, **kw):
     import torch
     t = torch.from_numpy(np.ascontiguousarray(sv)).cuda()
@@ -188,11 +194,39 @@ def test_config5_n4096_closed_form_and_invariants(orc, hp):
 
 @pytest.mark.parametrize("n", [2, 3, 4, 15, 31, 32, 33, 63, 64, 65, 83, 84])
 def test_small_path_sizes(orc, hp, n):
+    """S9: the Jacobi kernel on every size it supports (2..84)."""
     rng = np.random.default_rng(200 + n)
+    sizes = [n] * 3
+    sv = pack_all(orc, [herm(rng, n) for _ in sizes])
+    hp.set_option("jacobi_max_n", 84)
+    try:
+        got, _ = check_vs_oracle(orc, hp, sizes, sv)
+        check_invariants(hp, sizes, sv, got)
+    finally:
+        hp.set_option("jacobi_max_n", 40)
+
+
+@pytest.mark.parametrize("n", [41, 47, 64, 65, 81, 84, 100, 115, 116])
+def test_medium_path_sizes(orc, hp, n):
+    """S10: one-CTA Householder + QL kernel (default route for 40 < n <= 116)."""
+    rng = np.random.default_rng(250 + n)
     sizes = [n] * 3
     sv = pack_all(orc, [herm(rng, n) for _ in sizes])
     got, _ = check_vs_oracle(orc, hp, sizes, sv)
     check_invariants(hp, sizes, sv, got)
+
+
+@pytest.mark.parametrize("n", [2, 5, 16, 31])
+def test_medium_kernel_on_small_sizes(orc, hp, n):
+    """The S10 kernel itself has no lower size limit: route small blocks through it."""
+    rng = np.random.default_rng(270 + n)
+    sizes = [n] * 2
+    sv = pack_all(orc, [herm(rng, n) for _ in sizes])
+    hp.set_option("jacobi_max_n", 1)
+    try:
+        check_vs_oracle(orc, hp, sizes, sv)
+    finally:
+        hp.set_option("jacobi_max_n", 40)
 
 
 @pytest.mark.parametrize("n", [2, 3, 31, 32, 33, 63, 64, 65, 85, 96, 127, 128, 129, 200, 257, 320])
@@ -200,12 +234,12 @@ def test_large_path_sizes(orc, hp, n):
     """Force every block through S1..S8 of the Householder/D&C path (ragged tiles, several panels)."""
     rng = np.random.default_rng(300 + n)
     sv = orc.pack(herm(rng, n))
-    hp.set_option("jacobi_max_n", 1)
+    force_large(hp, True)
     try:
         got, _ = check_vs_oracle(orc, hp, [n], sv, nthreads=orc.max_threads() if n > 150 else 1)
         check_invariants(hp, [n], sv, got)
     finally:
-        hp.set_option("jacobi_max_n", 84)
+        force_large(hp, False)
 
 
 # ------------------------------------------------------------------ degenerate inputs
@@ -237,12 +271,12 @@ def _special_cases(rng, n):
     }
 
 
-@pytest.mark.parametrize("n,force_large", [(24, False), (24, True), (81, False), (150, True)])
-def test_degenerate_inputs(orc, hp, n, force_large):
+@pytest.mark.parametrize("n,large", [(24, False), (24, True), (81, False), (150, True)])
+def test_degenerate_inputs(orc, hp, n, large):
     rng = np.random.default_rng(500 + n)
     cases = _special_cases(rng, n)
-    if force_large:
-        hp.set_option("jacobi_max_n", 1)
+    if large:
+        force_large(hp, True)
     try:
         for name, X in cases.items():
             X = 0.5 * (X + X.conj().T)
@@ -256,7 +290,7 @@ def test_degenerate_inputs(orc, hp, n, force_large):
             if name in ("diagonal", "identity"):       # closed form: clamp the diagonal
                 np.testing.assert_allclose(got, np.maximum(sv, 0), rtol=8 * EPS, atol=0, err_msg=name)
     finally:
-        hp.set_option("jacobi_max_n", 84)
+        force_large(hp, False)
 
 
 def test_n0_n1_and_empty_list(orc, hp):
@@ -372,7 +406,7 @@ def test_covariances(orc, hp):
     rng = np.random.default_rng(11)
     for n, force in ((40, False), (140, True)):
         if force:
-            hp.set_option("jacobi_max_n", 1)
+            force_large(hp, True)
         try:
             X = herm(rng, n)
             sv = orc.pack(X)
@@ -381,4 +415,4 @@ def test_covariances(orc, hp):
             pc = gpu_project(hp, [n], orc.pack(X.conj()))
             assert rel_err(pc, orc.pack(orc.unpack(p, n).conj())) <= TOL * n
         finally:
-            hp.set_option("jacobi_max_n", 84)
+            force_large(hp, False)

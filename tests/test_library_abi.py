@@ -56,6 +56,9 @@ def test_argument_errors_without_gpu(lib):
     assert lib.hpsd_set_option(b"no_such_option", 1) == -1
     assert lib.hpsd_set_option(b"jacobi_max_n", 0) == -1
     assert lib.hpsd_set_option(b"jacobi_max_n", 84) == 0
+    assert lib.hpsd_set_option(b"medium_max_n", 117) == -1
+    assert lib.hpsd_set_option(b"medium_max_n", 116) == 0
+    assert lib.hpsd_set_option(b"jacobi_max_n", 40) == 0
     assert lib.hpsd_project(0, None, None, None, None) == 0       # empty list: nothing to do
 
 
