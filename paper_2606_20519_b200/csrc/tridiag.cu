@@ -325,12 +325,15 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     cp_async_wait_dyn(issued - ready_seq[h]);
                     __syncwarp();
                     const cplx *sl = s_slots + (size_t)(k % kSlots) * kSlotElems;
-                    cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0);
+                    // two independent accumulator sets (even / odd columns) halve the dependent DFMA chains
+                    cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0), accR1 = mk(0.0, 0.0), accC1 = mk(0.0, 0.0);
                     if (!diag) {
 #pragma unroll 8
-                        for (int cc = 0; cc < kTS; ++cc) {
-                            cfma(accR, sl[cc * kTP + lane], vJ[cc]);          // lane = row
-                            cfma_conj(accC, sl[lane * kTP + cc], vI[cc]);     // lane = column, cc = row
+                        for (int cc = 0; cc < kTS; cc += 2) {
+                            cfma(accR, sl[cc * kTP + lane], vJ[cc]);              // lane = row
+                            cfma(accR1, sl[(cc + 1) * kTP + lane], vJ[cc + 1]);
+                            cfma_conj(accC, sl[lane * kTP + cc], vI[cc]);         // lane = column, cc = row
+                            cfma_conj(accC1, sl[lane * kTP + cc + 1], vI[cc + 1]);
                         }
                     } else {
 #pragma unroll 8
@@ -342,9 +345,10 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                             cplx b = sl[lane * kTP + cc];                      // col = lane, row = cc
                             b.x = (cc > lane) ? b.x : 0.0;
                             b.y = (cc > lane) ? b.y : 0.0;
-                            cfma_conj(accC, b, vI[cc]);
+                            cfma_conj(accC1, b, vI[cc]);
                         }
                     }
+                    accR = accR + accR1; accC = accC + accC1;
                     double qterm;
                     if (diag) {
                         const cplx s = accR + accC;
