@@ -63,6 +63,30 @@ def stage_flops(stage: str, sizes, kpos, jmax: int) -> float:
     return tot
 
 
+def panel_bytes(n: int) -> float:
+    """Algorithmic bytes of the panel kernel for one n x n block: per column c the Hermitian mat-vec reads the
+    stored lower triangle (diagonal included) of the (n-c-1) x (n-c-1) trailing matrix once, 16 B per entry."""
+    return float(sum(16 * (m * (m + 1) // 2) for m in range(1, n)))
+
+
+def measured_hbm_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy bandwidth, burst)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback 6.65 TB/s of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu
+# --set full captures (profiles/r1_tuned_ncu_full.md); None where no capture exists for that workload
+NCU_TRAFFIC = {
+    ("S2S3_tridiag_panel", 3): {"bytes_per_launch": 2.82e6, "source": "profiles/r1_tuned_ncu_full.md (first panel, n=625)"},
+    ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.24e9, "source": "profiles/r1_tuned_ncu_full.md (first panels, n=4096)"},
+    ("S10_householder_ql", 2): {"bytes_per_launch": 1.35e7, "source": "profiles/r1_tuned_ncu_full.md (256 x n=81)"},
+}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -306,21 +330,40 @@ def main():
     dom_ms = stages[dom]["ms_per_step"]
     dom_spans = max(stages[dom]["launch_spans_per_step"], 1)
     dom_flops = stage_flops(dom, sizes, kpos, jmax)
-    achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     F = sum(f_alg(n, k) for n, k in zip(sizes, kpos))
-    roofline = {
-        "kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-        "frac": achieved / fp64_peak if fp64_peak else None, "traffic": None,
+    hbm_peak, hbm_src = measured_hbm_gbs()
+    fp64_src = (f"measured in this run by hpsd_fp64_peak_probe: DFMA {peak_dfma:.1f}, DMMA {peak_dmma:.1f} TFLOP/s "
+                "(MEASURED_PEAKS.json has no FP64 figure)")
+    if dom in ("S2S3_tridiag_panel", "S1_unpack"):
+        # memory-bound stages: the one-stage reduction streams the stored lower triangle of the trailing
+        # matrix through the SMs once per column; unpack reads 8n^2 and writes 8n^2 bytes
+        if dom == "S1_unpack":
+            dom_bytes = sum(16.0 * n * n for n in sizes if n > jmax)
+        else:
+            dom_bytes = sum(panel_bytes(n) for n in sizes if n > jmax)
+        achieved = dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": achieved / hbm_peak, "traffic": (NCU_TRAFFIC.get((dom, cfg)) or {}).get("bytes_per_launch"),
+                    "traffic_source": (NCU_TRAFFIC.get((dom, cfg)) or {}).get("source"),
+                    "peak_source": hbm_src, "algorithmic_bytes_per_step": dom_bytes,
+                    "algorithmic_flops_per_step": dom_flops,
+                    "flop_fraction_of_fp64_peak": dom_flops / (dom_ms * 1e-3) / 1e12 / fp64_peak if fp64_peak else None}
+    else:
+        achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+        bound = "alu" if dom in ("S9_jacobi", "S10_householder_ql") else "tensor"     # tensor = FP64 DMMA pipe
+        roofline = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+                    "frac": achieved / fp64_peak if fp64_peak else None, "traffic": (NCU_TRAFFIC.get((dom, cfg)) or {}).get("bytes_per_launch"),
+                    "traffic_source": (NCU_TRAFFIC.get((dom, cfg)) or {}).get("source"),
+                    "peak_source": fp64_src, "algorithmic_flops_per_step": dom_flops}
+    roofline.update({
         "avg_launch_ms": dom_ms / dom_spans, "launches_per_step": dom_spans,
         "share_of_step": dom_ms / sum(s["ms_per_step"] for s in stages.values()),
-        "peak_source": f"measured in this run by hpsd_fp64_peak_probe: DFMA {peak_dfma:.1f}, DMMA {peak_dmma:.1f} TFLOP/s "
-                       "(MEASURED_PEAKS.json has no FP64 figure)",
-        "algorithmic_flops_per_step": dom_flops,
+        "fp64_peak_tflops": fp64_peak, "fp64_peak_source": fp64_src,
         "whole_path": {"f_alg_flops": F, "achieved_tflops": F / (ms_per_step * 1e-3) / 1e12,
                        "frac_of_fp64_peak": F / (ms_per_step * 1e-3) / 1e12 / fp64_peak if fp64_peak else None,
-                       "hbm_floor_ms": 16.0 * sum(n * n for n in sizes) / 6553.9e9 * 1e3},
+                       "hbm_floor_ms": 16.0 * sum(n * n for n in sizes) / (hbm_peak * 1e9) * 1e3},
         "stages": stages,
-    }
+    })
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     h_in = sv.cpu().pin_memory()
