@@ -113,11 +113,13 @@ __global__ void __launch_bounds__(BG_THREADS) bt_vt_kernel(BackWs w) {
     gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, blockIdx.x, 0, smem_raw, epi);
 }
 
-// X_part[s] = V_b^H Z over the s-th chunk of rows (blockIdx.x = column tile, blockIdx.y = s)
+// X_part[s] = V_b^H Z over the s-th chunk of rows (blockIdx.x = column tile, blockIdx.y = s, blockIdx.z = row tile)
+template <int MI, int NI>
 __global__ void __launch_bounds__(BG_THREADS) bt_vhz_kernel(BackWs w, int b) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
-    if ((int)blockIdx.x * 64 >= kpos) return;
+    if ((int)blockIdx.x * BN >= kpos) return;
     const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
     const int chunk = (((m + kSplitK - 1) / kSplitK) + 15) & ~15;
     const int k0 = blockIdx.y * chunk;
@@ -127,7 +129,7 @@ __global__ void __launch_bounds__(BG_THREADS) bt_vhz_kernel(BackWs w, int b) {
     p.B = w.Zc + cb + 1 + k0; p.ldb = w.ldz;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = kpos; p.K = klen > 0 ? klen : 0; p.K2 = 0;
     StoreEpi epi{w.Xp + (size_t)blockIdx.y * kNBT * w.n, kNBT};
-    gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, 0, blockIdx.x, smem_raw, epi);
+    gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, MI, NI, BG_WM, BG_WN, false>(p, blockIdx.z, blockIdx.x, smem_raw, epi);
 }
 
 __global__ void __launch_bounds__(256) bt_reduce_kernel(BackWs w) {
@@ -142,17 +144,19 @@ __global__ void __launch_bounds__(256) bt_reduce_kernel(BackWs w) {
 }
 
 // Z[cb+1:, :] -= VT_b X
+template <int MI, int NI>
 __global__ void __launch_bounds__(BG_THREADS) bt_update_kernel(BackWs w, int b) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int BM = BG_WM * MI * 8, BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
     const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
-    if ((int)blockIdx.y * 64 >= kpos || (int)blockIdx.x * 64 >= m) return;
+    if ((int)blockIdx.y * BN >= kpos || (int)blockIdx.x * BM >= m) return;
     GemmProblem<cplx, cplx> p;
     p.A = w.VT + (size_t)cb * w.lda + cb + 1; p.lda = w.lda;
     p.B = w.X; p.ldb = kNBT;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = m; p.N = kpos; p.K = nbw; p.K2 = 0;
     SubEpi epi{w.Zc + cb + 1, w.ldz};
-    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, MI, NI, BG_WM, BG_WN, false>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
 // ---- S7 + S8: lower triangle of W W^H packed as vec_R (Eq. D10) --------------------------------
@@ -179,6 +183,8 @@ __global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, double 
 static int g_bh_init_dev = -1;
 constexpr size_t kSmemKK = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
 constexpr size_t kSmemMK = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
+constexpr size_t kSmemKKs = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, 2, 2, BG_WM, BG_WN>();
+constexpr size_t kSmemMKs = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, 2, 2, BG_WM, BG_WN>();
 constexpr size_t kSmemMM = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
 
 int backherk_init() {
@@ -188,9 +194,11 @@ int backherk_init() {
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(cplx) * kNBT * kNBT));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKKs);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMKs);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(herk_pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMM);
     if (e != cudaSuccess) return HPSD_ECUDA_;
     g_bh_init_dev = dev;
@@ -203,6 +211,7 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     if (rc) return rc;
     const int nblocks = (n + kNBT - 1) / kNBT;
     const int nt = (n + 63) / 64;
+    const bool small = n <= 1536;          // 32 x 32 CTA tiles keep the grid wide and the CTAs short
     prof_begin(ST_BACK, st);
     count_pos_kernel<<<1, 32, 0, st>>>(n, lam, w.cnt);
     HPSD_LAUNCH_CHECK();
@@ -218,11 +227,13 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     for (int b = nblocks - 1; b >= 0; --b) {
         const int m = n - b * kNBT - 1;
         if (m <= 0) continue;
-        bt_vhz_kernel<<<dim3(nt, kSplitK), BG_THREADS, kSmemKK, st>>>(w, b);
+        if (small) bt_vhz_kernel<2, 2><<<dim3((n + 31) / 32, kSplitK, 2), BG_THREADS, kSmemKKs, st>>>(w, b);
+        else bt_vhz_kernel<4, 4><<<dim3(nt, kSplitK, 1), BG_THREADS, kSmemKK, st>>>(w, b);
         HPSD_LAUNCH_CHECK();
         bt_reduce_kernel<<<(kNBT * n + 255) / 256 < 1184 ? (kNBT * n + 255) / 256 : 1184, 256, 0, st>>>(w);
         HPSD_LAUNCH_CHECK();
-        bt_update_kernel<<<dim3((m + 63) / 64, nt), BG_THREADS, kSmemMK, st>>>(w, b);
+        if (small) bt_update_kernel<2, 2><<<dim3((m + 31) / 32, (n + 31) / 32), BG_THREADS, kSmemMKs, st>>>(w, b);
+        else bt_update_kernel<4, 4><<<dim3((m + 63) / 64, nt), BG_THREADS, kSmemMK, st>>>(w, b);
         HPSD_LAUNCH_CHECK();
     }
     prof_end(ST_BACK, st);

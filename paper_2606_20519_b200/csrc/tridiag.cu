@@ -537,6 +537,13 @@ __global__ void __launch_bounds__(H2_WM *H2_WN * 32) her2k_kernel(GemmProblem<cp
     gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, H2_MI, H2_NI, H2_WM, H2_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
+// small trailing matrices: 32 x 32 CTA tiles, so that the grid still covers the SMs and each CTA is short
+__global__ void __launch_bounds__(H2_WM *H2_WN * 32) her2k_small_kernel(GemmProblem<cplx, cplx> p, Her2kEpi epi) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (blockIdx.y > blockIdx.x) return;
+    gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, 2, 2, H2_WM, H2_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+}
+
 // After the reduction: zero the (unused) diagonal and upper part so that V blocks are plain dense
 // sub-matrices for the back-transformation (S5).
 __global__ void clean_v_kernel(int n, cplx *A, int lda) {
@@ -554,6 +561,8 @@ int tridiag_init() {
     if (cudaFuncSetAttribute(tridiag_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)panel_smem_bytes()) != cudaSuccess) return HPSD_ECUDA_;
     constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
     if (cudaFuncSetAttribute(her2k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h2) != cudaSuccess) return HPSD_ECUDA_;
+    constexpr size_t h2s = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2_WM, H2_WN>();
+    if (cudaFuncSetAttribute(her2k_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h2s) != cudaSuccess) return HPSD_ECUDA_;
     g_panel_init_dev = dev;
     return 0;
 }
@@ -622,10 +631,16 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
             gp.A2 = Wp; gp.lda2 = w.ldw; gp.B2 = V; gp.ldb2 = w.lda;
             gp.M = m2; gp.N = m2; gp.K = kNB; gp.K2 = kNB;
             Her2kEpi epi{w.A + (size_t)(j0 + kNB) * w.lda + (j0 + kNB), w.lda};
-            const int nt = (m2 + 63) / 64;
             constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
+            constexpr size_t h2s = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2_WM, H2_WN>();
             prof_begin(ST_HER2K, st);
-            her2k_kernel<<<dim3(nt, nt), H2_WM * H2_WN * 32, h2, st>>>(gp, epi);
+            if (m2 <= 1536) {
+                const int nt = (m2 + 31) / 32;
+                her2k_small_kernel<<<dim3(nt, nt), H2_WM * H2_WN * 32, h2s, st>>>(gp, epi);
+            } else {
+                const int nt = (m2 + 63) / 64;
+                her2k_kernel<<<dim3(nt, nt), H2_WM * H2_WN * 32, h2, st>>>(gp, epi);
+            }
             prof_end(ST_HER2K, st);
             HPSD_LAUNCH_CHECK();
         }
