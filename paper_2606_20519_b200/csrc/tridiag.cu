@@ -52,15 +52,17 @@ struct PanelArgs {
 
 #ifdef HPSD_PANEL_TRACE
 // dev-only: per-column phase timestamps of CTA 0 and CTA G/2 (clock64), first traced launch only
-__device__ long long g_trace[2 * 32 * 8];
+__device__ long long g_trace[2 * 32 * 16];
 __device__ int g_trace_armed = 0;
 #define TRACE(slot)                                                                                   \
     do {                                                                                              \
         if (trace_on)                                                                                 \
-            g_trace[((g == 0 ? 0 : 1) * 32 + i) * 8 + (slot)] = clock64();                             \
+            g_trace[((g == 0 ? 0 : 1) * 32 + i) * 16 + (slot)] = clock64();                             \
     } while (0)
+#define TRACE_USE(val) do { if (trace_on && (val) == 1.2345e300) g_trace[0] = 0; } while (0)
 #else
 #define TRACE(slot) do {} while (0)
+#define TRACE_USE(val) do {} while (0)
 #endif
 
 __device__ __forceinline__ cplx group8_sum(cplx v) {
@@ -89,8 +91,12 @@ __device__ __forceinline__ void householder_scalars(cplx alpha, double xnorm2, d
 
 // Phase-B row distribution: 31 rows per CTA (one per 8-lane group; group 31 is the helper), more
 // only when the rows outnumber 31 G.  Few producers keep the cross-CTA reductions small.
-__device__ __forceinline__ int rows_per_cta(int rows, int G) { const int l = (rows + G - 1) / G; return l > 31 ? l : 31; }
-__device__ __forceinline__ int producers(int rows, int G) { const int l = rows_per_cta(rows, G); return (rows + l - 1) / l; }
+// (runtime integer divisions are ~100 cycles on the critical path: only taken when the rows outnumber 31 G)
+__device__ __forceinline__ int rows_per_cta(int rows, int G) { return rows <= 31 * G ? 31 : (rows + G - 1) / G; }
+__device__ __forceinline__ int producers(int rows, int G) {
+    const int l = rows_per_cta(rows, G);
+    return l == 31 ? (rows + 30) / 31 : (rows + l - 1) / l;
+}
 
 // One warp copies tile (I, J) of A into a shared-memory slot (zero fill outside the matrix).
 __device__ __forceinline__ void warp_load_tile(cplx *slot, const cplx *__restrict__ A, int lda, int n, int2 ij, int lane) {
@@ -157,6 +163,11 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         cnt = j + 1;
     }
 
+    // tile coordinates of this warp's first two tiles (all of them in the resident regimes), read once
+    int2 ijc[2] = {make_int2(0, 0), make_int2(0, 0)};
+    if (wide) { if ((warp >> 2) < q && g + (warp >> 2) * G < T) ijc[0] = p.tiles[g + (warp >> 2) * G]; }
+    else { for (int j = 0; j < 2 && j < cnt; ++j) ijc[j] = p.tiles[g + ((j / nsl) * kSlots + warp + 8 * (j % nsl)) * G]; }
+
     // ---------------- panel start: d[j0] and the partial norm of column j0 (already fully updated) -----
     {
         const int cn = p.j0;
@@ -200,7 +211,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             rawI[jj] = mk(0.0, 0.0); rawJ[jj] = mk(0.0, 0.0);
             if (wide) {
                 if (jj == 0 && wvalid) {
-                    const int2 ij = p.tiles[g + wtile * G];
+                    const int2 ij = ijc[0];
                     const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
                     if (rI < n && rI > c + 1) rawI[0] = ldcg_(&A[(size_t)c * lda + rI]);
                     if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[0] = ldcg_(&A[(size_t)c * lda + rJ]);
@@ -208,7 +219,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             } else if (jj < cnt) {
                 const int j = fwd ? jj : cnt - 1 - jj;
                 const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
-                const int2 ij = p.tiles[g + k * G];
+                const int2 ij = (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
                 const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
                 if (rI < n && rI > c + 1) rawI[jj] = ldcg_(&A[(size_t)c * lda + rI]);
                 if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[jj] = ldcg_(&A[(size_t)c * lda + rJ]);
@@ -248,7 +259,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0);
             int2 ij = make_int2(0, 0);
             if (wvalid) {
-                ij = p.tiles[g + wtile * G];
+                ij = ijc[0];
                 const bool diag = (ij.x == ij.y);
                 const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
                 const cplx a = (rI == c + 1) ? mk(1.0, 0.0) : scale * rawI[0];
@@ -303,7 +314,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     const int j = fwd ? jj : cnt - 1 - jj;
                     const int h = j % nsl;
                     const int k = (j / nsl) * kSlots + warp + 8 * h;
-                    const int2 ij = p.tiles[g + k * G];
+                    const int2 ij = (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
                     const int r0 = ij.x * kTS, c0 = ij.y * kTS;
                     const bool diag = (ij.x == ij.y);
                     // v pieces (formed on the fly; zero outside the trailing matrix)
@@ -411,6 +422,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 // ---- every global load of the pass is issued before the first shared-memory write
                 const cplx ar = okr ? ldcg_(&A[(size_t)c * lda + r]) : mk(0.0, 0.0);
                 const cplx anx = (okr && do_next) ? ldcg_(&A[(size_t)(c + 1) * lda + r]) : mk(0.0, 0.0);
+                TRACE(8);
                 cplx Vr[kNB / 8], Wr[kNB / 8], cv[kNB / 8], cw[kNB / 8];
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
@@ -428,10 +440,23 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 cplx p1 = mk(0.0, 0.0);
                 if (ok) {
                     const int R = r / kTS;
-#pragma unroll 4
-                    for (int bb = J0 + warp; bb < p.nblk; bb += 8)
-                        p1 = p1 + ((bb <= R) ? ldcg_(&p.PR[(size_t)bb * ldp + r]) : ldcg_(&p.PC[(size_t)bb * ldp + r]));
+                    // eight independent loads in flight per group (no load -> add -> load chains)
+                    for (int b0 = J0 + warp; b0 < p.nblk; b0 += 64) {
+                        cplx v[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const int bb = b0 + 8 * u;
+                            v[u] = mk(0.0, 0.0);
+                            if (bb < p.nblk) v[u] = (bb <= R) ? ldcg_(&p.PR[(size_t)bb * ldp + r]) : ldcg_(&p.PC[(size_t)bb * ldp + r]);
+                        }
+                        p1 = p1 + (((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7])));
+                    }
                 }
+                TRACE(9);
+                TRACE_USE(ar.x + anx.x);
+                TRACE(10);
+                TRACE_USE(p1.x);
+                TRACE(11);
                 double qv = 0.0;
                 if (warp == 1) {
                     for (int k = lane; k < (T < G ? T : G); k += 32) qv += ldcg_(&p.qpart[k]);
@@ -570,7 +595,7 @@ int tridiag_init() {
 #ifdef HPSD_PANEL_TRACE
 extern "C" int hpsd_debug_trace(int arm, long long *out) {
     if (arm >= 0) cudaMemcpyToSymbol(g_trace_armed, &arm, sizeof(int));
-    if (out) cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 2 * 32 * 8);
+    if (out) cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 2 * 32 * 16);
     return 0;
 }
 #endif
