@@ -74,6 +74,12 @@ __device__ __forceinline__ cplx group8_sum(cplx v) {
     return v;
 }
 
+// Loads of data another CTA wrote before the last grid barrier.  The barrier's fence invalidates this SM's L1
+// (CCTL.IVALL, which is how grid.sync makes ordinary loads safe), so plain loads are correct here, and they are
+// much cheaper to issue than ld.global.cg, which ptxas turns into LDG.STRONG.GPU (~170 cycles of issue each).
+__device__ __forceinline__ double ldx_(const double *p) { return *p; }
+__device__ __forceinline__ cplx ldx_(const cplx *p) { return *p; }
+
 // Householder scalars of column c from alpha = a[c+1] and xnorm2 = ||a[c+2:]||^2 (zlarfg semantics)
 __device__ __forceinline__ void householder_scalars(cplx alpha, double xnorm2, double &beta, cplx &tau, cplx &scale) {
     if (xnorm2 == 0.0 && alpha.y == 0.0) {
@@ -213,24 +219,24 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 if (jj == 0 && wvalid) {
                     const int2 ij = ijc[0];
                     const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
-                    if (rI < n && rI > c + 1) rawI[0] = ldcg_(&A[(size_t)c * lda + rI]);
-                    if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[0] = ldcg_(&A[(size_t)c * lda + rJ]);
+                    if (rI < n && rI > c + 1) rawI[0] = ldx_(&A[(size_t)c * lda + rI]);
+                    if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[0] = ldx_(&A[(size_t)c * lda + rJ]);
                 }
             } else if (jj < cnt) {
                 const int j = fwd ? jj : cnt - 1 - jj;
                 const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
                 const int2 ij = (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
                 const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
-                if (rI < n && rI > c + 1) rawI[jj] = ldcg_(&A[(size_t)c * lda + rI]);
-                if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[jj] = ldcg_(&A[(size_t)c * lda + rJ]);
+                if (rI < n && rI > c + 1) rawI[jj] = ldx_(&A[(size_t)c * lda + rI]);
+                if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[jj] = ldx_(&A[(size_t)c * lda + rJ]);
             }
         }
         const int nprod = producers(n - c, G);          // CTAs that left partials for this column
         // warp 0: Householder scalars from the partial norms
         if (warp == 0) {
             double S = 0.0;
-            for (int k = lane; k < nprod; k += 32) S += ldcg_(&p.part[(size_t)k * PSTRIDE].x);
-            const cplx alpha = ldcg_(&A[(size_t)c * lda + c + 1]);
+            for (int k = lane; k < nprod; k += 32) S += ldx_(&p.part[(size_t)k * PSTRIDE].x);
+            const cplx alpha = ldx_(&A[(size_t)c * lda + c + 1]);
             S = warp_sum(S);
             double beta; cplx tau0, scale0;
             householder_scalars(alpha, S, beta, tau0, scale0);
@@ -244,8 +250,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         const bool reducer = (warp == 7 && i > 0 && g < 2 * kNB && (g % kNB) < i);
         if (reducer) {
             const int t = g % kNB, which = g / kNB;
-            for (int k = lane; k < nprod; k += 32) red_s = red_s + ldcg_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
-            red_top = which == 0 ? ldcg_(&A[(size_t)(p.j0 + t) * lda + c + 1]) : ldcg_(&W[(size_t)t * ldw + c + 1]);
+            for (int k = lane; k < nprod; k += 32) red_s = red_s + ldx_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
+            red_top = which == 0 ? ldx_(&A[(size_t)(p.j0 + t) * lda + c + 1]) : ldx_(&W[(size_t)t * ldw + c + 1]);
             red_s = warp_sum(red_s);
         }
         __syncthreads();
@@ -325,8 +331,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         else if (jj == 1) { a = rawI[1]; b = rawJ[1]; }
                         else {
                             a = mk(0.0, 0.0); b = mk(0.0, 0.0);
-                            if (rI < n && rI > c + 1) a = ldcg_(&A[(size_t)c * lda + rI]);
-                            if (!diag && rJ < n && rJ > c + 1) b = ldcg_(&A[(size_t)c * lda + rJ]);
+                            if (rI < n && rI > c + 1) a = ldx_(&A[(size_t)c * lda + rI]);
+                            if (!diag && rJ < n && rJ > c + 1) b = ldx_(&A[(size_t)c * lda + rJ]);
                         }
                         a = (rI == c + 1) ? mk(1.0, 0.0) : scale * a;
                         b = diag ? a : ((rJ == c + 1) ? mk(1.0, 0.0) : scale * b);
@@ -420,8 +426,18 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 const bool ok = helper ? do_next : (rr < L && r < n);
                 const bool okr = ok && !helper;
                 // ---- every global load of the pass is issued before the first shared-memory write
-                const cplx ar = okr ? ldcg_(&A[(size_t)c * lda + r]) : mk(0.0, 0.0);
-                const cplx anx = (okr && do_next) ? ldcg_(&A[(size_t)(c + 1) * lda + r]) : mk(0.0, 0.0);
+                const cplx ar = okr ? ldx_(&A[(size_t)c * lda + r]) : mk(0.0, 0.0);
+                const cplx anx = (okr && do_next) ? ldx_(&A[(size_t)(c + 1) * lda + r]) : mk(0.0, 0.0);
+                // warp 1 also gathers the v^H y partials of phase A; issued here so that they share the round trip
+                double qv = 0.0, qv0 = 0.0, qv1 = 0.0, qv2 = 0.0, qv3 = 0.0, qv4 = 0.0;
+                if (warp == 1) {
+                    const int nq = T < G ? T : G;
+                    if (lane < nq) qv0 = ldx_(&p.qpart[lane]);
+                    if (lane + 32 < nq) qv1 = ldx_(&p.qpart[lane + 32]);
+                    if (lane + 64 < nq) qv2 = ldx_(&p.qpart[lane + 64]);
+                    if (lane + 96 < nq) qv3 = ldx_(&p.qpart[lane + 96]);
+                    for (int k = lane + 128; k < nq; k += 32) qv4 += ldx_(&p.qpart[k]);
+                }
                 TRACE(8);
                 cplx Vr[kNB / 8], Wr[kNB / 8], cv[kNB / 8], cw[kNB / 8];
 #pragma unroll
@@ -430,11 +446,11 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     Vr[k] = mk(0.0, 0.0); Wr[k] = mk(0.0, 0.0); cv[k] = mk(0.0, 0.0); cw[k] = mk(0.0, 0.0);
                     if (t < i) {
                         if (ok) {
-                            Vr[k] = ldcg_(&A[(size_t)(p.j0 + t) * lda + r]);
-                            Wr[k] = ldcg_(&W[(size_t)t * ldw + r]);
+                            Vr[k] = ldx_(&A[(size_t)(p.j0 + t) * lda + r]);
+                            Wr[k] = ldx_(&W[(size_t)t * ldw + r]);
                         }
-                        cv[k] = ldcg_(&p.tot[t]);
-                        cw[k] = ldcg_(&p.tot[kNB + t]);
+                        cv[k] = ldx_(&p.tot[t]);
+                        cw[k] = ldx_(&p.tot[kNB + t]);
                     }
                 }
                 cplx p1 = mk(0.0, 0.0);
@@ -447,7 +463,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         for (int u = 0; u < 8; ++u) {
                             const int bb = b0 + 8 * u;
                             v[u] = mk(0.0, 0.0);
-                            if (bb < p.nblk) v[u] = (bb <= R) ? ldcg_(&p.PR[(size_t)bb * ldp + r]) : ldcg_(&p.PC[(size_t)bb * ldp + r]);
+                            if (bb < p.nblk) v[u] = (bb <= R) ? ldx_(&p.PR[(size_t)bb * ldp + r]) : ldx_(&p.PC[(size_t)bb * ldp + r]);
                         }
                         p1 = p1 + (((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7])));
                     }
@@ -457,11 +473,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 TRACE(10);
                 TRACE_USE(p1.x);
                 TRACE(11);
-                double qv = 0.0;
-                if (warp == 1) {
-                    for (int k = lane; k < (T < G ? T : G); k += 32) qv += ldcg_(&p.qpart[k]);
-                    qv = warp_sum(qv);
-                }
+                if (warp == 1) qv = warp_sum((qv0 + qv1) + (qv2 + qv3) + qv4);
                 // ---- partial sums of this warp: y - V cW - W cV,  V conj(W[c+1,:]) + W conj(V[c+1,:]),  Re(cV^H cW)
                 cplx p2 = mk(0.0, 0.0);
                 double re = 0.0;
