@@ -116,11 +116,19 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
                     bool under = false;
                     for (i = mm - 1; i >= l; --i) {
                         const double f = s * ee[i], b = c * ee[i];
-                        r = sqrt(f * f + g * g);
-                        if (r < 1e-140) r = hypot(f, g);        // squares underflowed: take the safe route
+                        const double h2 = fma(f, f, g * g);
+                        double ir;
+                        if (h2 > 1e-280) {                      // T is scaled to unit max-norm: no overflow
+                            ir = rsqrt(h2);
+                            ir = ir * fma(-0.5 * h2 * ir, ir, 1.5);
+                            r = h2 * ir;
+                        } else {                                // squares underflowed: take the safe route
+                            r = hypot(f, g);
+                            ir = (r != 0.0) ? 1.0 / r : 0.0;
+                        }
                         ee[i + 1] = r;
                         if (r == 0.0) { dd[i + 1] -= p; ee[mm] = 0.0; under = true; break; }
-                        { const double ir = 1.0 / r; s = f * ir; c = g * ir; }
+                        s = f * ir; c = g * ir;
                         g = dd[i + 1] - p;
                         r = (dd[i] - g) * s + 2.0 * c * b;
                         p = s * r;
@@ -186,6 +194,22 @@ __device__ __forceinline__ int upper_bound_d(const double *a, int len, double v)
     return lo;
 }
 
+// exclusive prefix sum of one int per thread over a 256-thread block (every thread gets its offset and the total)
+__device__ __forceinline__ int block_excl_scan256(int v, int *s_w, int &total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    __syncthreads();
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    int base = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { const int t = s_w[w]; if (w < warp) base += t; tot += t; }
+    total = tot;
+    return base + inc - v;
+}
+
 __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int node = blockIdx.x;
@@ -224,9 +248,62 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
     }
     if ((tid & 31) == 0) { s_red[tid >> 5] = dmax; s_red[8 + (tid >> 5)] = zmax; }
     __syncthreads();
+    __shared__ double s_tol;
+    __shared__ int s_w[8];
     if (tid == 0) {
         for (int w = 1; w < 8; ++w) { dmax = fmax(dmax, s_red[w]); zmax = fmax(zmax, s_red[8 + w]); }
-        const double tol = 8.0 * kEps * fmax(dmax, zmax);
+        s_tol = 8.0 * kEps * fmax(dmax, zmax);
+    }
+    __syncthreads();
+    const double tol = s_tol;
+    // ---- parallel fast path: deflate the negligible weights; if no two surviving neighbours are close poles
+    // (the usual case) nothing sequential is left.  Otherwise thread 0 redoes the scan with rotations below.
+    bool fast;
+    {
+        const int chunk = (N + 255) / 256;
+        const int r_lo = min(N, tid * chunk), r_hi = min(N, r_lo + chunk);
+        int mine = 0;
+        for (int r = r_lo; r < r_hi; ++r) mine += !(rho * fabs(zs[r]) <= tol);
+        int ns;
+        const int off = block_excl_scan256(mine, s_w, ns);
+        int qs = off, it = r_lo - off;                       // next survivor slot, next deflated rank
+        for (int r = r_lo; r < r_hi; ++r) {
+            if (rho * fabs(zs[r]) <= tol) list[N - 1 - it++] = r;   // ascending r = ascending pole: i-th smallest at N-1-i
+            else list[qs++] = r;
+        }
+        __syncthreads();
+        int close = 0;
+        for (int q = tid; q + 1 < ns; q += 256) {
+            const int pj = list[q], r = list[q + 1];
+            const double sv = zs[pj], cv = zs[r], t = ds[r] - ds[pj];
+            close |= (fabs(t) * fabs(cv * sv) <= tol * (cv * cv + sv * sv));
+        }
+        fast = !__syncthreads_or(close);
+        if (fast) {
+            const int K = ns;
+            const int ch2 = (K + 255) / 256;
+            const int q_lo = min(K, tid * ch2), q_hi = min(K, q_lo + ch2);
+            int n1 = 0, n2 = 0, n3 = 0;
+            for (int q = q_lo; q < q_hi; ++q) { const int ty = src[list[q]] >> 28; n1 += (ty == 1); n2 += (ty == 2); n3 += (ty == 3); }
+            int k1, k2, k3;
+            int c1 = block_excl_scan256(n1, s_w, k1);
+            int c2 = block_excl_scan256(n2, s_w, k2) + k1;
+            int c3 = block_excl_scan256(n3, s_w, k3) + k1 + k2;
+            for (int q = q_lo; q < q_hi; ++q) {
+                const int ty = src[list[q]] >> 28;
+                const int g = (ty == 1) ? c1++ : (ty == 2) ? c2++ : c3++;
+                a.grow[lo + q] = g;
+                a.gsrc[lo + g] = src[list[q]] & 0x0fffffff;
+            }
+            if (tid == 0) {
+                int *ni = a.nodeinfo + 8 * node;
+                ni[0] = K; ni[1] = k1; ni[2] = k2; ni[3] = k3; ni[4] = 0; ni[5] = N - K;
+                a.rho[node] = rho;
+                s_cnt[0] = K; s_cnt[1] = N - K;
+            }
+        }
+    }
+    if (!fast && tid == 0) {
         int K = 0, ndefl = 0, nrot = 0, pj = -1;
         // deflated sorted indices live at list[N-ndefl .. N-1], ascending value towards lower index reversed:
         // the i-th smallest deflated value is list[N-1-i]
