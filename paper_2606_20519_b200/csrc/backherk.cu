@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(256) bt_reduce_kernel(BackWs w) {
 
 // Z[cb+1:, :] -= VT_b X
 template <int MI, int NI>
-__global__ void __launch_bounds__(BG_THREADS) bt_update_kernel(BackWs w, int b) {
+__global__ void __launch_bounds__(BG_THREADS, 3) bt_update_kernel(BackWs w, int b) {      // K = 64: two stages, 3 CTAs/SM
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int BM = BG_WM * MI * 8, BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(BG_THREADS) bt_update_kernel(BackWs w, int b) 
     p.B = w.X; p.ldb = kNBT;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = m; p.N = kpos; p.K = nbw; p.K2 = 0;
     SubEpi epi{w.Zc + cb + 1, w.ldz};
-    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, MI, NI, BG_WM, BG_WN, false>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, MI, NI, BG_WM, BG_WN, false, 2>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
 // ---- S7 + S8: lower triangle of W W^H packed as vec_R (Eq. D10) --------------------------------
@@ -183,8 +183,9 @@ __global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, double 
 static int g_bh_init_dev = -1;
 constexpr size_t kSmemKK = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
 constexpr size_t kSmemMK = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
+constexpr size_t kSmemMK2 = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN, 2>();
 constexpr size_t kSmemKKs = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, 2, 2, BG_WM, BG_WN>();
-constexpr size_t kSmemMKs = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, 2, 2, BG_WM, BG_WN>();
+constexpr size_t kSmemMKs = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, 2, 2, BG_WM, BG_WN, 2>();
 constexpr size_t kSmemMM = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
 
 int backherk_init() {
@@ -198,7 +199,7 @@ int backherk_init() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKKs);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMKs);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK2);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(herk_pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMM);
     if (e != cudaSuccess) return HPSD_ECUDA_;
     g_bh_init_dev = dev;
@@ -233,7 +234,7 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
         bt_reduce_kernel<<<(kNBT * n + 255) / 256 < 1184 ? (kNBT * n + 255) / 256 : 1184, 256, 0, st>>>(w);
         HPSD_LAUNCH_CHECK();
         if (small) bt_update_kernel<2, 2><<<dim3((m + 31) / 32, (n + 31) / 32), BG_THREADS, kSmemMKs, st>>>(w, b);
-        else bt_update_kernel<4, 4><<<dim3((m + 63) / 64, nt), BG_THREADS, kSmemMK, st>>>(w, b);
+        else bt_update_kernel<4, 4><<<dim3((m + 63) / 64, nt), BG_THREADS, kSmemMK2, st>>>(w, b);
         HPSD_LAUNCH_CHECK();
     }
     prof_end(ST_BACK, st);

@@ -101,14 +101,14 @@ struct Acc {
 
 // Epilogue interface:  epi(row, col, re, im) called for every in-range element of the tile.
 // LOWER: only tiles with (tile row block) >= (tile col block) are computed; the epilogue masks i<j.
-template <typename TA, typename TB, int LA, int LB, bool CONJA, bool CONJB, int MI, int NI, int WM, int WN, bool LOWER, class Epi>
+template <typename TA, typename TB, int LA, int LB, bool CONJA, bool CONJB, int MI, int NI, int WM, int WN, bool LOWER, int STAGES = kGemmStages, class Epi>
 __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int tile_m, int tile_n, unsigned char *smem_raw, Epi &epi) {
     constexpr bool CA = is_cplx<TA>::v, CB = is_cplx<TB>::v, CC = CA || CB;
     constexpr int BM = WM * MI * 8, BN = WN * NI * 8, NT = WM * WN * 32;
     using GA = TileGeom<TA, LA, BM>;
     using GB = TileGeom<TB, LB, BN>;
     TA *smA = reinterpret_cast<TA *>(smem_raw);
-    TB *smB = reinterpret_cast<TB *>(smem_raw + sizeof(TA) * GA::elems * kGemmStages);
+    TB *smB = reinterpret_cast<TB *>(smem_raw + sizeof(TA) * GA::elems * STAGES);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp % WM, wn = warp / WM;
@@ -128,7 +128,7 @@ __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int
 
     auto issue = [&](int kt) {
         if (kt < KT) {
-            const int slot = kt % kGemmStages;
+            const int slot = kt % STAGES;
             if (kt < KT1) {
                 load_tile<TA, LA, BM, NT>(smA + slot * GA::elems, p.A, p.lda, m0, kt * kGemmBK, p.M, p.K, tid);
                 load_tile<TB, LB, BN, NT>(smB + slot * GB::elems, p.B, p.ldb, n0, kt * kGemmBK, p.N, p.K, tid);
@@ -141,15 +141,15 @@ __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int
     };
 
 #pragma unroll
-    for (int s = 0; s < kGemmStages - 1; ++s) issue(s);
+    for (int s = 0; s < STAGES - 1; ++s) issue(s);
 
     const int fr = lane >> 2, fk = lane & 3;
     for (int kt = 0; kt < KT; ++kt) {
-        cp_async_wait<kGemmStages - 2>();
+        cp_async_wait<STAGES - 2>();
         __syncthreads();
-        issue(kt + kGemmStages - 1);
-        const TA *sa = smA + (kt % kGemmStages) * GA::elems;
-        const TB *sb = smB + (kt % kGemmStages) * GB::elems;
+        issue(kt + STAGES - 1);
+        const TA *sa = smA + (kt % STAGES) * GA::elems;
+        const TB *sb = smB + (kt % STAGES) * GB::elems;
 #pragma unroll
         for (int k4 = 0; k4 < kGemmBK; k4 += 4) {
             double ar[MI], ai[MI], br[NI], bi[NI];
@@ -194,9 +194,9 @@ __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int
             }
 }
 
-template <typename TA, typename TB, int LA, int LB, int MI, int NI, int WM, int WN>
+template <typename TA, typename TB, int LA, int LB, int MI, int NI, int WM, int WN, int STAGES = kGemmStages>
 constexpr size_t gemm_smem_bytes() {
-    return (size_t)kGemmStages * (sizeof(TA) * TileGeom<TA, LA, WM * MI * 8>::elems + sizeof(TB) * TileGeom<TB, LB, WN * NI * 8>::elems);
+    return (size_t)STAGES * (sizeof(TA) * TileGeom<TA, LA, WM * MI * 8>::elems + sizeof(TB) * TileGeom<TB, LB, WN * NI * 8>::elems);
 }
 
 }  // namespace hpsd

@@ -568,10 +568,12 @@ struct Her2kEpi {
 
 constexpr int H2_MI = 4, H2_NI = 4, H2_WM = 2, H2_WN = 2;   // 64 x 64 CTA tile, 4 warps
 
-__global__ void __launch_bounds__(H2_WM *H2_WN * 32) her2k_kernel(GemmProblem<cplx, cplx> p, Her2kEpi epi) {
+// K is only 64 per output tile, so prologue and epilogue weigh as much as the main loop: two stages and
+// three CTAs per SM let one CTA's loads and read-modify-write overlap another's DMMAs
+__global__ void __launch_bounds__(H2_WM *H2_WN * 32, 3) her2k_kernel(GemmProblem<cplx, cplx> p, Her2kEpi epi) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (blockIdx.y > blockIdx.x) return;   // lower triangle of tiles only
-    gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, H2_MI, H2_NI, H2_WM, H2_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+    gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, H2_MI, H2_NI, H2_WM, H2_WN, true, 2>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
 // small trailing matrices: 32 x 32 CTA tiles, so that the grid still covers the SMs and each CTA is short
@@ -596,7 +598,7 @@ int tridiag_init() {
     cudaGetDevice(&dev);
     if (g_panel_init_dev == dev) return 0;
     if (cudaFuncSetAttribute(tridiag_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)panel_smem_bytes()) != cudaSuccess) return HPSD_ECUDA_;
-    constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
+    constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN, 2>();
     if (cudaFuncSetAttribute(her2k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h2) != cudaSuccess) return HPSD_ECUDA_;
     constexpr size_t h2s = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2_WM, H2_WN>();
     if (cudaFuncSetAttribute(her2k_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h2s) != cudaSuccess) return HPSD_ECUDA_;
@@ -668,7 +670,7 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
             gp.A2 = Wp; gp.lda2 = w.ldw; gp.B2 = V; gp.ldb2 = w.lda;
             gp.M = m2; gp.N = m2; gp.K = kNB; gp.K2 = kNB;
             Her2kEpi epi{w.A + (size_t)(j0 + kNB) * w.lda + (j0 + kNB), w.lda};
-            constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN>();
+            constexpr size_t h2 = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2_MI, H2_NI, H2_WM, H2_WN, 2>();
             constexpr size_t h2s = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2_WM, H2_WN>();
             prof_begin(ST_HER2K, st);
             if (m2 <= 1536) {
