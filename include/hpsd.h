@@ -79,6 +79,14 @@ int hpsd_project_ws(int n_blocks, const int *sizes,
                     const double *in_svec, double *out_svec,
                     void *ws, size_t ws_bytes, int *info_dev, void *stream);
 
+/* One ADMM cone step, Eqs. (D33)-(D34), fused into the projection:
+ *     u = Pi_C(u~ - v),      v <- v - u~ + u
+ * on the PSD part of the cone.  utilde (read only), v (read and updated in place) and u (written) are DEVICE
+ * svec vectors of sum_b n_b^2 doubles; u may alias utilde.  The difference u~ - v is formed while unpacking (S1)
+ * and the v update is written by the same epilogue that packs u (S8), so neither costs a pass over memory.
+ * Same workspace, stream and error conventions as hpsd_project. */
+int hpsd_admm_step(int n_blocks, const int *sizes, const double *utilde, double *v, double *u, void *stream);
+
 /* The same projection through HOST buffers: copies in_host to the device,
  * projects, copies the result back and synchronises `stream` before
  * returning.  This is the end-to-end call bench.py's "e2e" times; the paper

@@ -125,3 +125,12 @@ def project(sizes: Sequence[int], in_svec: np.ndarray, nthreads: int = 1) -> np.
     if rc != 0:
         raise RuntimeError(f"oracle projection failed (code {rc})")
     return out
+
+
+def admm_step(sizes: Sequence[int], utilde: np.ndarray, v: np.ndarray, nthreads: int = 1):
+    """The cone step of the SCS iteration exactly as the paper writes it, Eqs. (D33)-(D34)
+    (PAPER.md:1466-1472):  u = Pi_C(u~ - v),  v_new = v - u~ + u.  Returns (u, v_new)."""
+    utilde = np.ascontiguousarray(utilde, dtype=np.float64)
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    u = project(sizes, utilde - v, nthreads=nthreads)
+    return u, v - utilde + u

@@ -7,6 +7,7 @@ CUDA extension is missing or no GPU is present, calls raise.
 """
 from .binding import (  # noqa: F401
     HpsdError,
+    admm_step_,
     eigvalsh,
     fp64_peak_probe,
     last_launch_count,

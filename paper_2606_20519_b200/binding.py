@@ -16,7 +16,7 @@ EXPORTS = [
     "hpsd_version", "hpsd_strerror", "hpsd_project", "hpsd_workspace_size", "hpsd_project_ws",
     "hpsd_project_host", "hpsd_pack", "hpsd_unpack", "hpsd_tridiagonalize", "hpsd_eigvalsh",
     "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
-    "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read",
+    "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
 ]
 
 
@@ -42,6 +42,7 @@ def load_library():
         lib.hpsd_strerror.restype = ctypes.c_char_p
         lib.hpsd_strerror.argtypes = [c_int]
         lib.hpsd_project.argtypes = [c_int, ip, c_vp, c_vp, c_vp]
+        lib.hpsd_admm_step.argtypes = [c_int, ip, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_workspace_size.argtypes = [c_int, ip, ctypes.POINTER(c_sz)]
         lib.hpsd_project_ws.argtypes = [c_int, ip, c_vp, c_vp, c_vp, c_sz, c_vp, c_vp]
         lib.hpsd_project_host.argtypes = [c_int, ip, c_vp, c_vp, c_vp]
@@ -121,6 +122,21 @@ def project_(sizes: Sequence[int], in_svec: torch.Tensor, out_svec: torch.Tensor
 
 def project(sizes: Sequence[int], in_svec: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     return project_(sizes, in_svec, torch.empty_like(in_svec), stream)
+
+
+def admm_step_(sizes: Sequence[int], utilde: torch.Tensor, v: torch.Tensor, u: torch.Tensor,
+               stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_admm_step: u = Pi_C(utilde - v), v <- v - utilde + u (v updated in place); returns u."""
+    lib = load_library()
+    for t, name in ((utilde, "utilde"), (v, "v"), (u, "u")):
+        _need_cuda_f64(t, name)
+    total = svec_len(sizes)
+    if utilde.numel() != total or v.numel() != total or u.numel() != total:
+        raise HpsdError(f"svec lengths != sum n^2 = {total}")
+    arr, nb = _sizes(sizes)
+    with torch.cuda.device(utilde.device):
+        _check(lib.hpsd_admm_step(nb, arr, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)), "hpsd_admm_step")
+    return u
 
 
 def workspace_size(sizes: Sequence[int]) -> int:

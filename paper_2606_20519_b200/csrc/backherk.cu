@@ -161,21 +161,21 @@ __global__ void __launch_bounds__(BG_THREADS, 3) bt_update_kernel(BackWs w, int 
 
 // ---- S7 + S8: lower triangle of W W^H packed as vec_R (Eq. D10) --------------------------------
 struct PackEpi {
-    double *sv; int n;
+    SvecIo io; int n;
     __device__ __forceinline__ void operator()(int i, int j, double re, double im) const {
-        double *c = sv + svec_col_off(n, j);
-        if (i == j) c[0] = re;
-        else { const int k = i - j - 1; c[1 + 2 * k] = kSqrt2 * re; c[2 + 2 * k] = kSqrt2 * im; }
+        const size_t c = svec_col_off(n, j);
+        if (i == j) io_store(io, c, re);
+        else { const int k = i - j - 1; io_store(io, c + 1 + 2 * k, kSqrt2 * re); io_store(io, c + 2 + 2 * k, kSqrt2 * im); }
     }
 };
 
-__global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, double *out) {
+__global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, SvecIo io) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (blockIdx.y > blockIdx.x) return;
     GemmProblem<cplx, cplx> p;
     p.A = w.Zc; p.lda = w.ldz; p.B = w.Zc; p.ldb = w.ldz;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = w.n; p.N = w.n; p.K = w.cnt[1]; p.K2 = 0;
-    PackEpi epi{out, w.n};
+    PackEpi epi{io, w.n};
     gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, BG_MI, BG_NI, BG_WM, BG_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
@@ -206,7 +206,7 @@ int backherk_init() {
     return 0;
 }
 
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, double *out, cudaStream_t st) {
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st) {
     const int n = w.n;
     int rc = backherk_init();
     if (rc) return rc;
@@ -239,7 +239,7 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     }
     prof_end(ST_BACK, st);
     prof_begin(ST_HERK_PACK, st);
-    herk_pack_kernel<<<dim3(nt, nt), BG_THREADS, kSmemMM, st>>>(w, out);
+    herk_pack_kernel<<<dim3(nt, nt), BG_THREADS, kSmemMM, st>>>(w, io);
     prof_end(ST_HERK_PACK, st);
     HPSD_LAUNCH_CHECK();
     return 0;

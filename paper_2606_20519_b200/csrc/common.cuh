@@ -40,6 +40,31 @@ constexpr double kEps = 2.220446049250313e-16;     // 2^-52
 // svec layout (include/hpsd.h): start of column j of the lower triangle
 __host__ __device__ __forceinline__ size_t svec_col_off(int n, int j) { return (size_t)j * (size_t)(2 * n - j); }
 
+// svec input/output of one call.  Plain projection: x = in, out = P(x).  ADMM step, Eqs. (D33)-(D34)
+// (PAPER.md:1466-1472): x = in - sub with in = u~ and sub = v;  out = u = P(x);  vout = sub - in + u.
+// vout may alias sub, out may alias in: every element is read before it is written, by the same thread.
+struct SvecIo {
+    const double *in;
+    const double *sub;     // nullptr for a plain projection
+    double *out;
+    double *vout;
+};
+__device__ __forceinline__ double io_load(const SvecIo &io, size_t i) {
+    double x = io.in[i];
+    if (io.sub) x -= io.sub[i];
+    return x;
+}
+__device__ __forceinline__ void io_store(const SvecIo &io, size_t i, double u) {
+    if (io.sub) io.vout[i] = (io.sub[i] - io.in[i]) + u;
+    io.out[i] = u;
+}
+inline SvecIo io_offset(const SvecIo &io, long long off) {
+    SvecIo r = io;
+    r.in += off; r.out += off;
+    if (io.sub) { r.sub += off; r.vout += off; }
+    return r;
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -194,7 +194,7 @@ int check_args(int n_blocks, const int *sizes, const void *in, const void *out, 
     return 0;
 }
 
-int run_plan(const Plan &pl, const double *in, double *out, void *ws, int *info_dev, cudaStream_t st) {
+int run_plan(const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStream_t st) {
     // info lives at the start of the workspace when the caller gave none
     int *info = info_dev ? info_dev : reinterpret_cast<int *>(ws);
     unsigned char *scratch = reinterpret_cast<unsigned char *>(ws) + align_up(pl.sizes.size() * sizeof(int) + 4, 256);
@@ -205,19 +205,19 @@ int run_plan(const Plan &pl, const double *in, double *out, void *ws, int *info_
     if (g_profile) prof_reset();
     if (pl.n_scalar) {
         prof_begin(ST_SCALAR, st);
-        rc = launch_clamp_scalars(pl.n_scalar, pl.ll(pl.scalar_off_index), in, out, st);
+        rc = launch_clamp_scalars(pl.n_scalar, pl.ll(pl.scalar_off_index), io, st);
         prof_end(ST_SCALAR, st);
         if (rc) return rc;
     }
     for (const JacobiGroup &g : pl.groups) {
         prof_begin(g.medium ? ST_MEDIUM : ST_JACOBI, st);
-        rc = g.medium ? launch_hhql_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st)
-                      : launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), in, out, info, pl.ii(g.idx_index), st);
+        rc = g.medium ? launch_hhql_project(g.n, g.count, pl.ll(g.off_index), io, info, pl.ii(g.idx_index), st)
+                      : launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), io, info, pl.ii(g.idx_index), st);
         prof_end(g.medium ? ST_MEDIUM : ST_JACOBI, st);
         if (rc) return rc;
     }
     for (const LargeBlock &lb : pl.large) {
-        rc = largepath_project(lb.n, in + lb.off, out + lb.off, scratch, pl.tiles_dev.at(lb.n), info + lb.idx, st);
+        rc = largepath_project(lb.n, io_offset(io, lb.off), scratch, pl.tiles_dev.at(lb.n), info + lb.idx, st);
         if (rc) return rc;
     }
     return 0;
@@ -302,15 +302,11 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     return HPSD_OK;
 }
 
-int hpsd_project_ws(int n_blocks, const int *sizes, const double *in_svec, double *out_svec,
-                    void *ws, size_t ws_bytes, int *info_dev, void *stream) {
+static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void *ws, size_t ws_bytes, int *info_dev, void *stream) {
     g_launches = 0;
-    size_t total;
-    int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
-    if (rc) return rc;
     if (n_blocks == 0) return HPSD_OK;
     size_t need;
-    rc = hpsd_workspace_size(n_blocks, sizes, &need);
+    int rc = hpsd_workspace_size(n_blocks, sizes, &need);
     if (rc) return rc;
     if (ws == nullptr || ws_bytes < need || (reinterpret_cast<uintptr_t>(ws) & 255u)) return HPSD_EWORKSPACE;
     int dev;
@@ -322,7 +318,48 @@ int hpsd_project_ws(int n_blocks, const int *sizes, const double *in_svec, doubl
     Plan *pl;
     rc = get_plan(ds, n_blocks, sizes, &pl);
     if (rc) return rc;
-    return run_plan(*pl, in_svec, out_svec, ws, info_dev, (cudaStream_t)stream);
+    return run_plan(*pl, io, ws, info_dev, (cudaStream_t)stream);
+}
+
+// library-owned workspace of the current device, grown on demand
+static int library_workspace(int n_blocks, const int *sizes, void **ws, size_t *bytes) {
+    size_t need;
+    int rc = hpsd_workspace_size(n_blocks, sizes, &need);
+    if (rc) return rc;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    if (ds.ws_bytes < need) {
+        if (ds.ws) cudaFree(ds.ws);   // synchronises; only when the workspace grows
+        ds.ws = nullptr; ds.ws_bytes = 0;
+        if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
+        ds.ws_bytes = need;
+    }
+    *ws = ds.ws; *bytes = ds.ws_bytes;
+    return 0;
+}
+
+int hpsd_project_ws(int n_blocks, const int *sizes, const double *in_svec, double *out_svec,
+                    void *ws, size_t ws_bytes, int *info_dev, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
+    if (rc) return rc;
+    const SvecIo io{in_svec, nullptr, out_svec, nullptr};
+    return project_io_ws(n_blocks, sizes, io, ws, ws_bytes, info_dev, stream);
+}
+
+int hpsd_admm_step(int n_blocks, const int *sizes, const double *utilde, double *v, double *u, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, utilde, u, &total);
+    if (rc) return rc;
+    if (total > 0 && v == nullptr) return HPSD_EINVAL;
+    if (n_blocks == 0) { g_launches = 0; return HPSD_OK; }
+    void *ws; size_t bytes;
+    rc = library_workspace(n_blocks, sizes, &ws, &bytes);
+    if (rc) return rc;
+    const SvecIo io{utilde, v, u, v};
+    return project_io_ws(n_blocks, sizes, io, ws, bytes, nullptr, stream);
 }
 
 int hpsd_project(int n_blocks, const int *sizes, const double *in_svec, double *out_svec, void *stream) {
@@ -330,25 +367,10 @@ int hpsd_project(int n_blocks, const int *sizes, const double *in_svec, double *
     int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
     if (rc) return rc;
     if (n_blocks == 0) { g_launches = 0; return HPSD_OK; }
-    size_t need;
-    rc = hpsd_workspace_size(n_blocks, sizes, &need);
+    void *ws; size_t bytes;
+    rc = library_workspace(n_blocks, sizes, &ws, &bytes);
     if (rc) return rc;
-    int dev;
-    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
-    void *ws;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        DeviceState &ds = g_dev[dev];
-        if (ds.ws_bytes < need) {
-            if (ds.ws) cudaFree(ds.ws);   // synchronises; only when the workspace grows
-            ds.ws = nullptr; ds.ws_bytes = 0;
-            if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
-            ds.ws_bytes = need;
-        }
-        ws = ds.ws;
-        need = ds.ws_bytes;
-    }
-    return hpsd_project_ws(n_blocks, sizes, in_svec, out_svec, ws, need, nullptr, stream);
+    return hpsd_project_ws(n_blocks, sizes, in_svec, out_svec, ws, bytes, nullptr, stream);
 }
 
 int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, double *out_host, void *stream) {
@@ -390,7 +412,7 @@ int hpsd_pack(int n, const void *A, int lda, double *svec, void *stream) {
 int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream) {
     if (n < 0 || (n > 0 && (!A || !svec || lda < n))) return HPSD_EINVAL;
     g_launches = 0;
-    return launch_unpack(n, svec, reinterpret_cast<cplx *>(A), lda, 1, (cudaStream_t)stream);
+    return launch_unpack(n, svec, nullptr, reinterpret_cast<cplx *>(A), lda, 1, (cudaStream_t)stream);
 }
 
 // S2+S3 alone: real symmetric tridiagonal (d[n], e[n-1]) unitarily similar to the block.

@@ -46,7 +46,7 @@ static size_t jacobi_smem_bytes(int m) {
 
 template <int THREADS>
 __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const long long *__restrict__ offs,
-                                                                 const double *__restrict__ in, double *__restrict__ out,
+                                                                 SvecIo io,
                                                                  int *__restrict__ info, const int *__restrict__ info_idx) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int m = (n + 1) & ~1;
@@ -54,8 +54,7 @@ __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const lo
     JacobiSmem sm = carve(smem_raw, m);
     cplx *A = sm.A, *V = sm.V;
     const int tid = threadIdx.x;
-    const double *sv = in + offs[blockIdx.x];
-    double *ov = out + offs[blockIdx.x];
+    const size_t base = (size_t)offs[blockIdx.x];
 
     // ---- S1: unpack into shared memory (both triangles), V = I -------------
     for (int t = tid; t < m * m; t += THREADS) {
@@ -67,14 +66,14 @@ __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const lo
     for (int t = tid; t < n * n; t += THREADS) {
         const int j = t / n, i = t % n;
         if (i < j) continue;
-        const double *c = sv + svec_col_off(n, j);
+        const size_t c = base + svec_col_off(n, j);
         if (i == j) {
-            const double d = c[0];
+            const double d = io_load(io, c);
             A[(size_t)j * m + i] = mk(d, 0.0);
             ss += d * d;
         } else {
             const int k = i - j - 1;
-            const cplx v = mk(c[1 + 2 * k] / kSqrt2, c[2 + 2 * k] / kSqrt2);
+            const cplx v = mk(io_load(io, c + 1 + 2 * k) / kSqrt2, io_load(io, c + 2 + 2 * k) / kSqrt2);
             A[(size_t)j * m + i] = v;
             A[(size_t)i * m + j] = conj_(v);
             ss += 2.0 * abs2(v);
@@ -196,12 +195,12 @@ __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const lo
             acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
             acc.y = fma(a.y, b.x, acc.y); acc.y = fma(-a.x, b.y, acc.y);
         }
-        double *c = ov + svec_col_off(n, j);
-        if (i == j) c[0] = acc.x;
+        const size_t c = base + svec_col_off(n, j);
+        if (i == j) io_store(io, c, acc.x);
         else {
             const int k = i - j - 1;
-            c[1 + 2 * k] = kSqrt2 * acc.x;
-            c[2 + 2 * k] = kSqrt2 * acc.y;
+            io_store(io, c + 1 + 2 * k, kSqrt2 * acc.x);
+            io_store(io, c + 2 + 2 * k, kSqrt2 * acc.y);
         }
     }
 }
@@ -214,15 +213,15 @@ int jacobi_init() {
     return 0;
 }
 
-int launch_jacobi_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+int launch_jacobi_project(int n, int count, const long long *offs_dev, const SvecIo &io,
                           int *info_dev, const int *info_idx_dev, cudaStream_t st) {
     if (count <= 0) return 0;
     if (n < 2 || n > kJacobiMaxN) return -1;
     const int m = (n + 1) & ~1;
     const size_t smem = jacobi_smem_bytes(m);
-    if (m <= 32) jacobi_project_kernel<256><<<count, 256, smem, st>>>(n, offs_dev, in, out, info_dev, info_idx_dev);
-    else if (m <= 56) jacobi_project_kernel<512><<<count, 512, smem, st>>>(n, offs_dev, in, out, info_dev, info_idx_dev);
-    else jacobi_project_kernel<1024><<<count, 1024, smem, st>>>(n, offs_dev, in, out, info_dev, info_idx_dev);
+    if (m <= 32) jacobi_project_kernel<256><<<count, 256, smem, st>>>(n, offs_dev, io, info_dev, info_idx_dev);
+    else if (m <= 56) jacobi_project_kernel<512><<<count, 512, smem, st>>>(n, offs_dev, io, info_dev, info_idx_dev);
+    else jacobi_project_kernel<1024><<<count, 1024, smem, st>>>(n, offs_dev, io, info_dev, info_idx_dev);
     HPSD_LAUNCH_CHECK();
     return 0;
 }

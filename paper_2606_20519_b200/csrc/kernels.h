@@ -6,17 +6,18 @@ namespace hpsd {
 
 // ---- pack.cu (S1 / S8) ------------------------------------
 // svec -> column-major complex.  full=0: lower triangle incl. diagonal only.
-int launch_unpack(int n, const double *svec, cplx *A, int lda, int full, cudaStream_t st);
+// sub != nullptr: unpack svec - sub (the ADMM argument u~ - v of Eq. D33)
+int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st);
 int launch_pack(int n, const cplx *A, int lda, double *svec, cudaStream_t st);
 // n = 1 blocks: out = max(in, 0) for `count` scattered scalars
-int launch_clamp_scalars(int count, const long long *offs_dev, const double *in, double *out, cudaStream_t st);
+int launch_clamp_scalars(int count, const long long *offs_dev, const SvecIo &io, cudaStream_t st);
 
 // ---- jacobi.cu (S9 / S10) --------------------------------------------------
 // Batched one-CTA-per-matrix cyclic Jacobi projection for blocks of one size n
 // (2 <= n <= kJacobiMaxN).  offs_dev[i] = svec offset (doubles) of matrix i;
 // info_dev may be NULL; info_idx_dev[i] = index into info_dev.
 constexpr int kJacobiMaxN = 84;
-int launch_jacobi_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+int launch_jacobi_project(int n, int count, const long long *offs_dev, const SvecIo &io,
                           int *info_dev, const int *info_idx_dev, cudaStream_t st);
 int jacobi_init();  // set kernel attributes once per device
 
@@ -24,7 +25,7 @@ int jacobi_init();  // set kernel attributes once per device
 // Batched one-CTA-per-matrix Householder + implicit-QL projection for blocks of one size n,
 // jacobi_max_n < n <= kMediumMaxN (the matrix must fit in shared memory: 16 n (n|1) + O(n) bytes).
 constexpr int kMediumMaxN = 116;
-int launch_hhql_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+int launch_hhql_project(int n, int count, const long long *offs_dev, const SvecIo &io,
                         int *info_dev, const int *info_idx_dev, cudaStream_t st);
 int medium_init();
 

@@ -71,7 +71,7 @@ struct BackWs {
     int *cnt;          // [0] = p0 (#lambda <= 0), [1] = kpos
 };
 int backherk_init();
-// lam ascending (n), Zt real eigenvectors of T (ldzt x n); writes the projection's svec to out.
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, double *out, cudaStream_t st);
+// lam ascending (n), Zt real eigenvectors of T (ldzt x n); writes the projection's svec (and the ADMM v update) through io.
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st);
 
 }  // namespace hpsd

@@ -72,11 +72,11 @@ LargeWs carve(int n, unsigned char *base) {
     return w;
 }
 
-int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, cudaStream_t st) {
+int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, const double *sub, cudaStream_t st) {
     if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     prof_begin(ST_UNPACK, st);
-    int rc = launch_unpack(n, in, w.t.A, w.t.lda, 0, st);
+    int rc = launch_unpack(n, in, sub, w.t.A, w.t.lda, 0, st);
     prof_end(ST_UNPACK, st);
     if (rc) return rc;
     return launch_tridiag(w.t, st);
@@ -98,7 +98,7 @@ size_t largepath_ws_bytes(int n) { return carve(n, nullptr).bytes; }
 int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsigned char *scratch, const int2 *tiles, cudaStream_t st) {
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
-    int rc = reduce_to_tridiagonal(w, n, in, st);
+    int rc = reduce_to_tridiagonal(w, n, in, nullptr, st);
     if (rc) return rc;
     if (cudaMemcpyAsync(d, w.t.d, sizeof(double) * n, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return HPSD_ECUDA_;
     if (n > 1 && cudaMemcpyAsync(e, w.t.e, sizeof(double) * (n - 1), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return HPSD_ECUDA_;
@@ -108,7 +108,7 @@ int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsign
 int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *scratch, const int2 *tiles, cudaStream_t st) {
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
-    int rc = reduce_to_tridiagonal(w, n, in, st);
+    int rc = reduce_to_tridiagonal(w, n, in, nullptr, st);
     if (rc) return rc;
     double *lam, *Z;
     rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
@@ -117,18 +117,18 @@ int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *sc
     return 0;
 }
 
-int largepath_project(int n, const double *in, double *out, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st) {
+int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st) {
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
     w.s.info = info;
-    int rc = reduce_to_tridiagonal(w, n, in, st);
+    int rc = reduce_to_tridiagonal(w, n, io.in, io.sub, st);
     if (rc) return rc;
     double *lam, *Z;
     prof_begin(ST_STEDC, st);
     rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
     prof_end(ST_STEDC, st);
     if (rc) return rc;
-    return launch_back_herk(w.b, lam, Z, w.s.ldz, out, st);
+    return launch_back_herk(w.b, lam, Z, w.s.ldz, io, st);
 }
 
 }  // namespace hpsd

@@ -6,7 +6,7 @@ namespace hpsd {
 int largepath_init();
 size_t largepath_ws_bytes(int n);
 // One block: svec in -> svec out.  scratch >= largepath_ws_bytes(n), 256-byte aligned.
-int largepath_project(int n, const double *in, double *out, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st);
+int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st);
 // S1+S2+S3 only (diagnostic / eigenvalue-only entry points).
 int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsigned char *scratch, const int2 *tiles, cudaStream_t st);
 // S1..S4: ascending eigenvalues only.

@@ -313,25 +313,24 @@ extern "C" int hpsd_debug_medium(long long *out) { cudaMemcpyFromSymbol(out, g_m
 #endif
 
 __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const long long *__restrict__ offs,
-                                                                   const double *__restrict__ in, double *__restrict__ out,
+                                                                   SvecIo io,
                                                                    int *__restrict__ info, const int *__restrict__ info_idx) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ld = med_ld(n);
     MedSmem sm = med_carve(smem_raw, n);
     cplx *A = sm.A;
     const int tid = threadIdx.x;
-    const double *sv = in + offs[blockIdx.x];
-    double *ov = out + offs[blockIdx.x];
+    const size_t base = (size_t)offs[blockIdx.x];
 
     // ---- S1: unpack into shared memory, both triangles
     for (int t = tid; t < n * n; t += kMedThreads) {
         const int j = t / n, i = t % n;
         if (i < j) continue;
-        const double *c = sv + svec_col_off(n, j);
-        if (i == j) A[(size_t)j * ld + i] = mk(c[0], 0.0);
+        const size_t c = base + svec_col_off(n, j);
+        if (i == j) A[(size_t)j * ld + i] = mk(io_load(io, c), 0.0);
         else {
             const int k = i - j - 1;
-            const cplx v = mk(c[1 + 2 * k] / kSqrt2, c[2 + 2 * k] / kSqrt2);
+            const cplx v = mk(io_load(io, c + 1 + 2 * k) / kSqrt2, io_load(io, c + 2 + 2 * k) / kSqrt2);
             A[(size_t)j * ld + i] = v;
             A[(size_t)i * ld + j] = conj_(v);
         }
@@ -380,12 +379,12 @@ __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const 
             acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
             acc.y = fma(a.y, b.x, acc.y); acc.y = fma(-a.x, b.y, acc.y);
         }
-        double *c = ov + svec_col_off(n, j);
-        if (i == j) c[0] = acc.x;
+        const size_t c = base + svec_col_off(n, j);
+        if (i == j) io_store(io, c, acc.x);
         else {
             const int k = i - j - 1;
-            c[1 + 2 * k] = kSqrt2 * acc.x;
-            c[2 + 2 * k] = kSqrt2 * acc.y;
+            io_store(io, c + 1 + 2 * k, kSqrt2 * acc.x);
+            io_store(io, c + 2 + 2 * k, kSqrt2 * acc.y);
         }
     }
     MTRACE(5);
@@ -397,11 +396,11 @@ int medium_init() {
     return 0;
 }
 
-int launch_hhql_project(int n, int count, const long long *offs_dev, const double *in, double *out,
+int launch_hhql_project(int n, int count, const long long *offs_dev, const SvecIo &io,
                         int *info_dev, const int *info_idx_dev, cudaStream_t st) {
     if (count <= 0) return 0;
     if (n < 2 || n > kMediumMaxN) return -1;
-    hhql_project_kernel<<<count, kMedThreads, med_smem_bytes(n), st>>>(n, offs_dev, in, out, info_dev, info_idx_dev);
+    hhql_project_kernel<<<count, kMedThreads, med_smem_bytes(n), st>>>(n, offs_dev, io, info_dev, info_idx_dev);
     HPSD_LAUNCH_CHECK();
     return 0;
 }

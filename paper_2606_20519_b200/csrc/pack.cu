@@ -8,17 +8,20 @@ namespace hpsd {
 // One CTA handles a chunk of one column j: rows i = j .. n-1.
 // svec column j: [X_jj, s Re X_{j+1,j}, s Im X_{j+1,j}, ...]
 template <int FULL>
-__global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__restrict__ sv, cplx *__restrict__ A, int lda) {
+__global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__restrict__ sv, const double *__restrict__ sub, cplx *__restrict__ A, int lda) {
     const int j = blockIdx.y;
     const double *c = sv + svec_col_off(n, j);
+    const double *cs = sub ? sub + svec_col_off(n, j) : nullptr;
     for (int i = j + blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         cplx v;
         if (i == j) {
-            v = mk(c[0], 0.0);
+            v = mk(cs ? c[0] - cs[0] : c[0], 0.0);
         } else {
             const int k = i - j - 1;
+            double re = c[1 + 2 * k], im = c[2 + 2 * k];
+            if (cs) { re -= cs[1 + 2 * k]; im -= cs[2 + 2 * k]; }     // u~ - v of Eq. (D33)
             // division, not multiplication by 1/sqrt2: bit-identical to vec_R^-1 as defined
-            v = mk(c[1 + 2 * k] / kSqrt2, c[2 + 2 * k] / kSqrt2);
+            v = mk(re / kSqrt2, im / kSqrt2);
         }
         A[(size_t)j * lda + i] = v;
         if (FULL && i != j) A[(size_t)i * lda + j] = conj_(v);
@@ -40,11 +43,11 @@ __global__ void __launch_bounds__(256) pack_kernel(int n, const cplx *__restrict
     }
 }
 
-__global__ void clamp_scalars_kernel(int count, const long long *__restrict__ offs, const double *__restrict__ in, double *__restrict__ out) {
+__global__ void clamp_scalars_kernel(int count, const long long *__restrict__ offs, SvecIo io) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < count) {
-        double v = in[offs[i]];
-        out[offs[i]] = v > 0.0 ? v : (v != v ? v : 0.0);   // NaN propagates
+        const double v = io_load(io, offs[i]);
+        io_store(io, offs[i], v > 0.0 ? v : (v != v ? v : 0.0));   // NaN propagates
     }
 }
 
@@ -54,11 +57,11 @@ static dim3 col_grid(int n) {
     return dim3(gx, n, 1);
 }
 
-int launch_unpack(int n, const double *svec, cplx *A, int lda, int full, cudaStream_t st) {
+int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st) {
     if (n <= 0) return 0;
     if (n > 65535) return -1;
-    if (full) unpack_kernel<1><<<col_grid(n), 256, 0, st>>>(n, svec, A, lda);
-    else unpack_kernel<0><<<col_grid(n), 256, 0, st>>>(n, svec, A, lda);
+    if (full) unpack_kernel<1><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda);
+    else unpack_kernel<0><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda);
     HPSD_LAUNCH_CHECK();
     return 0;
 }
@@ -71,9 +74,9 @@ int launch_pack(int n, const cplx *A, int lda, double *svec, cudaStream_t st) {
     return 0;
 }
 
-int launch_clamp_scalars(int count, const long long *offs_dev, const double *in, double *out, cudaStream_t st) {
+int launch_clamp_scalars(int count, const long long *offs_dev, const SvecIo &io, cudaStream_t st) {
     if (count <= 0) return 0;
-    clamp_scalars_kernel<<<(count + 127) / 128, 128, 0, st>>>(count, offs_dev, in, out);
+    clamp_scalars_kernel<<<(count + 127) / 128, 128, 0, st>>>(count, offs_dev, io);
     HPSD_LAUNCH_CHECK();
     return 0;
 }

@@ -416,3 +416,32 @@ def test_covariances(orc, hp):
             assert rel_err(pc, orc.pack(orc.unpack(p, n).conj())) <= TOL * n
         finally:
             force_large(hp, False)
+
+
+def test_admm_step_fused(orc, hp):
+    """NEXT-2: u = Pi_C(u~ - v), v <- v - u~ + u (Eqs. D33-D34) fused into
+    S1 and S8, against the oracle's unfused version; every size class in one list; u aliasing u~."""
+    import torch
+    rng = np.random.default_rng(12)
+    sizes = [1, 24, 81, 150, 1, 36]
+    ut = pack_all(orc, [herm(rng, n) for n in sizes])
+    v = pack_all(orc, [herm(rng, n) for n in sizes])
+    want_u, want_v = orc.admm_step(sizes, ut, v, nthreads=orc.max_threads())
+    t_ut, t_v = torch.from_numpy(ut).cuda(), torch.from_numpy(v.copy()).cuda()
+    t_u = torch.empty_like(t_ut)
+    hp.admm_step_(sizes, t_ut, t_v, t_u)
+    torch.cuda.synchronize()
+    off = 0
+    for n in sizes:
+        sl = slice(off, off + n * n)
+        assert parity_err(t_u.cpu().numpy()[sl], want_u[sl], (ut - v)[sl], n) <= TOL * n, n
+        assert parity_err(t_v.cpu().numpy()[sl], want_v[sl], (ut - v)[sl], n) <= TOL * n, n
+        off += n * n
+    # the plain projection of the difference gives the same u bit for bit (same kernels, same arithmetic)
+    assert np.array_equal(t_u.cpu().numpy(), gpu_project(hp, sizes, (torch.from_numpy(ut) - torch.from_numpy(v)).numpy()))
+    # in place: u written over u~
+    t_ut2, t_v2 = torch.from_numpy(ut.copy()).cuda(), torch.from_numpy(v.copy()).cuda()
+    hp.admm_step_(sizes, t_ut2, t_v2, t_ut2)
+    torch.cuda.synchronize()
+    assert np.array_equal(t_ut2.cpu().numpy(), t_u.cpu().numpy())
+    assert np.array_equal(t_v2.cpu().numpy(), t_v.cpu().numpy())

@@ -345,3 +345,21 @@ def test_thread_count_does_not_change_result(orc):
     a = orc.project(w.sizes, sv, nthreads=1)
     b = orc.project(w.sizes, sv, nthreads=4)
     assert np.array_equal(a, b)
+
+
+def test_admm_step_moreau_pin(orc):
+    """Eqs. (D33)-(D34).  Pin by the Moreau decomposition:
+    with x = u~ - v, u = P(x) and v_new = u - x = P(x) - x = P(-x), so u >= 0, v_new >= 0 (the PSD cone is
+    self-dual), <u, v_new> = 0 and u - v_new = x; and for a closed-form input the values are known."""
+    rng = np.random.default_rng(77)
+    b = workloads.from_spectrum(rng, np.array([2.0, -1.0, 0.5, -0.25, 3.0, -4.0]))
+    n = b.n
+    x = orc.pack(b.X)
+    v = orc.pack(herm(rng, n))
+    ut = x + v
+    u, vn = orc.admm_step([n], ut, v)
+    want_u = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
+    want_v = orc.pack((b.Q * np.maximum(-b.lam, 0)[None, :]) @ b.Q.conj().T)
+    assert rel_err(u, want_u) <= 1e-13 and rel_err(vn, want_v) <= 1e-13
+    assert abs(u @ vn) <= 1e-13 * np.linalg.norm(u) * np.linalg.norm(vn)
+    np.testing.assert_allclose(u - vn, ut - v, rtol=0, atol=1e-13 * np.linalg.norm(x))
