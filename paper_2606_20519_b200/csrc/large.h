@@ -33,11 +33,12 @@ constexpr int kMaxLargeN = 8192;  // shared-memory bound of the deflation scan (
 
 struct StedcWs {
     int n, ldz, depth;
+    int blk, d0;                       // batched use: n = blk 2^d0 and the top d0 levels are never merged (single: blk = n, d0 = 0)
     double *Za, *Zb, *Qw, *U;          // ldz x n each (eigenvector ping-pong, gathered copy, secular vectors)
     double *lamA, *lamB;               // n: eigenvalue ping-pong
     double *dmod;                      // n: scaled diagonal with the rank-one tears removed
     double *es;                        // n: scaled sub-diagonal
-    double *scal;                      // [sigma, 1/sigma]: power-of-two scaling of T
+    double *scal;                      // [sigma, 1/sigma] per top-level block: power-of-two scaling of T
     double *dt, *zt;                   // n: sorted non-deflated poles / weights per node segment
     double *mu, *lamroot, *zhat;       // n
     double *dval;                      // n: deflated eigenvalues (ascending) per node segment

@@ -48,7 +48,7 @@ LargeWs carve(int n, unsigned char *base) {
     w.t.qpart = dbl(G);
     w.t.tiles = nullptr;
     // ---- S4
-    w.s.n = n; w.s.ldz = N; w.s.depth = stedc_depth(n);
+    w.s.n = n; w.s.ldz = N; w.s.depth = stedc_depth(n); w.s.blk = n; w.s.d0 = 0;
     w.s.Za = dbl((size_t)N * n); w.s.Zb = dbl((size_t)N * n); w.s.Qw = dbl((size_t)N * n); w.s.U = dbl((size_t)N * n);
     w.s.lamA = dbl(N); w.s.lamB = dbl(N); w.s.dmod = dbl(N); w.s.es = dbl(N); w.s.scal = dbl(2); w.s.dt = dbl(N); w.s.zt = dbl(N);
     w.s.mu = dbl(N); w.s.lamroot = dbl(N); w.s.zhat = dbl(N); w.s.dval = dbl(N); w.s.rc = dbl(N); w.s.rs = dbl(N);

@@ -21,6 +21,11 @@ namespace hpsd {
 // node j at depth k owns indices [bound(k,j), bound(k,j+1))
 __host__ __device__ __forceinline__ int node_bound(int n, int k, int j) { return (int)(((long long)j * n) >> k); }
 
+// Batched use: a batch of 2^d0 tridiagonals of size blk is treated as one virtual problem of size n = blk 2^d0 whose
+// top d0 tree levels are never merged; eigenvector blocks are then stored compactly (ldz >= blk rows, n columns):
+// the ROW offset of a node is taken inside its top-level block.  Single matrix: blk = n, row offset = lo.
+__host__ __device__ __forceinline__ int row_off(int lo, int blk) { return lo - (lo / blk) * blk; }
+
 int stedc_depth(int n) {
     int D = 0;
     while (((n + (1 << D) - 1) >> D) > kLeaf) ++D;
@@ -29,13 +34,16 @@ int stedc_depth(int n) {
 
 // ---- K0: scale T to unit max-norm by an exact power of two (the deflation tolerances below
 // assume ||T|| ~ 1, as LAPACK's dstedc does) and remove the rank-one tears from the diagonal -----
-__global__ void __launch_bounds__(1024) stedc_prepare_kernel(int n, int depth, const double *__restrict__ d, const double *__restrict__ e,
+// (one CTA per top-level block: every matrix of a batch gets its own scale)
+__global__ void __launch_bounds__(1024) stedc_prepare_kernel(int n, int depth, int blk, const double *__restrict__ d, const double *__restrict__ e,
                                                              double *__restrict__ dmod, double *__restrict__ es, double *__restrict__ scal) {
     __shared__ double s_max[32];
     __shared__ double s_sigma;
     const int tid = threadIdx.x;
+    const int b0 = blockIdx.x * blk, b1 = b0 + blk;
+    scal += 2 * blockIdx.x;
     double m = 0.0;
-    for (int i = tid; i < n; i += 1024) {
+    for (int i = b0 + tid; i < b1; i += 1024) {
         m = fmax(m, fabs(d[i]));
         if (i < n - 1) m = fmax(m, fabs(e[i]));
     }
@@ -63,7 +71,7 @@ __global__ void __launch_bounds__(1024) stedc_prepare_kernel(int n, int depth, c
         const int j = (int)((num + n - 1) / n);
         return node_bound(n, depth, j) == x;
     };
-    for (int i = tid; i < n; i += 1024) {
+    for (int i = b0 + tid; i < b1; i += 1024) {
         double v = d[i] * sigma;
         const double ei = (i < n - 1) ? e[i] * sigma : 0.0;
         es[i] = ei;
@@ -75,14 +83,14 @@ __global__ void __launch_bounds__(1024) stedc_prepare_kernel(int n, int depth, c
     }
 }
 
-__global__ void stedc_unscale_kernel(int n, double *__restrict__ lam, const double *__restrict__ scal) {
+__global__ void stedc_unscale_kernel(int n, int blk, double *__restrict__ lam, const double *__restrict__ scal) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) lam[i] *= scal[1];
+    if (i < n) lam[i] *= scal[2 * (i / blk) + 1];
 }
 
 // ---- K1: leaves -- implicit QL with Wilkinson shift in one warp -----------------------------
 __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const double *__restrict__ dmod, const double *__restrict__ e,
-                                                        double *__restrict__ Z, int ldz, double *__restrict__ lam, int *info) {
+                                                        double *__restrict__ Z, int ldz, double *__restrict__ lam, int *info, int blk) {
     __shared__ double dd[kLeaf], ee[kLeaf], cs[kLeaf], sn[kLeaf];
     __shared__ double Zs[kLeaf * (kLeaf + 1)];
     __shared__ int ctrl[4];
@@ -168,7 +176,7 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
     __syncwarp();
     for (int c = 0; c < m; ++c) {
         const int rk = __shfl_sync(0xffffffffu, rank, c);
-        if (lane < m) Z[(size_t)(lo + rk) * ldz + lo + lane] = Zs[c * (kLeaf + 1) + lane];
+        if (lane < m) Z[(size_t)(lo + rk) * ldz + row_off(lo, blk) + lane] = Zs[c * (kLeaf + 1) + lane];
     }
 }
 
@@ -176,6 +184,7 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
 // nodeinfo[8*node + {0:K, 1:k1, 2:k2, 3:k3, 4:nrot, 5:ndefl}]
 struct MergeArgs {
     int n, ldz, depth;                 // depth = depth of the PARENT nodes being formed
+    int blk;                           // top-level block size (= n for a single matrix)
     const double *e;
     const double *Zin; double *Zout; double *Qw; double *U;
     const double *lam_in; double *lam_out;
@@ -216,6 +225,7 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
     const int lo = node_bound(a.n, a.depth, node), hi = node_bound(a.n, a.depth, node + 1);
     const int mid = node_bound(a.n, a.depth + 1, 2 * node + 1);
     const int N = hi - lo, n1 = mid - lo, n2 = hi - mid;
+    const int ro = row_off(lo, a.blk);
     double *ds = reinterpret_cast<double *>(smem_raw);    // N: poles in ascending order
     double *zs = ds + N;                                   // N: weights in the same order
     int *src = reinterpret_cast<int *>(zs + N);            // N: source column (local) | type << 28
@@ -231,10 +241,10 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
     for (int t = tid; t < N; t += 256) {
         double z, v; int rank, typ;
         if (t < n1) {
-            z = a.Zin[(size_t)(lo + t) * a.ldz + (mid - 1)];
+            z = a.Zin[(size_t)(lo + t) * a.ldz + (mid - 1 - lo + ro)];
             v = l1[t]; rank = t + lower_bound_d(l2, n2, v); typ = 1;
         } else {
-            z = sgn * a.Zin[(size_t)(lo + t) * a.ldz + mid];
+            z = sgn * a.Zin[(size_t)(lo + t) * a.ldz + (mid - lo + ro)];
             v = l2[t - n1]; rank = (t - n1) + upper_bound_d(l1, n1, v); typ = 3;
         }
         z *= 0.7071067811865476;
@@ -370,7 +380,7 @@ __global__ void __launch_bounds__(256) stedc_rotate_kernel(MergeArgs a) {
     const int r = blockIdx.x * 256 + threadIdx.x;
     const int nrot = a.nodeinfo[8 * node + 4];
     if (r >= N || nrot == 0) return;
-    double *Z = const_cast<double *>(a.Zin) + (size_t)lo * a.ldz + lo + r;    // row r of the node block
+    double *Z = const_cast<double *>(a.Zin) + (size_t)lo * a.ldz + row_off(lo, a.blk) + r;    // row r of the node block
     for (int t = 0; t < nrot; ++t) {
         const int p = a.rp[lo + t], q = a.rq[lo + t];
         const double c = a.rc[lo + t], s = a.rs[lo + t];
@@ -390,8 +400,8 @@ __global__ void __launch_bounds__(256) stedc_gather_kernel(MergeArgs a) {
     const int g0 = blockIdx.y * kGatherCols;
     const int r = blockIdx.x * 256 + threadIdx.x;
     if (g0 >= K || r >= N) return;
-    const double *__restrict__ Z = a.Zin + (size_t)lo * a.ldz + lo + r;
-    double *__restrict__ Q = a.Qw + (size_t)lo * a.ldz + lo + r;
+    const double *__restrict__ Z = a.Zin + (size_t)lo * a.ldz + row_off(lo, a.blk) + r;
+    double *__restrict__ Q = a.Qw + (size_t)lo * a.ldz + row_off(lo, a.blk) + r;
     double v[kGatherCols];
 #pragma unroll
     for (int cc = 0; cc < kGatherCols; ++cc) {
@@ -563,12 +573,12 @@ __global__ void __launch_bounds__(256) stedc_form_u_kernel(MergeArgs a) {
         for (int j = lane; j < K; j += 32) { const double u = a.zhat[lo + j] / ((d[j] - dorg) - mu); ss += u * u; }
         ss = warp_sum(ss);
         const double inv = 1.0 / sqrt(ss);
-        double *Ucol = a.U + (size_t)(lo + i) * a.ldz + lo;
+        double *Ucol = a.U + (size_t)(lo + i) * a.ldz + row_off(lo, a.blk);
         for (int j = lane; j < K; j += 32) Ucol[a.grow[lo + j]] = inv * (a.zhat[lo + j] / ((d[j] - dorg) - mu));
     } else if (w - K < ndefl && w < N) {
         const int m = w - K;
-        const double *src = a.Zin + (size_t)(lo + a.dcol[lo + m]) * a.ldz + lo;
-        double *dst = a.Zout + (size_t)(lo + a.dest_defl[lo + m]) * a.ldz + lo;
+        const double *src = a.Zin + (size_t)(lo + a.dcol[lo + m]) * a.ldz + row_off(lo, a.blk);
+        double *dst = a.Zout + (size_t)(lo + a.dest_defl[lo + m]) * a.ldz + row_off(lo, a.blk);
         for (int r = lane; r < N; r += 32) dst[r] = src[r];
     }
 }
@@ -592,8 +602,9 @@ __global__ void __launch_bounds__(DG_WM *DG_WN * 32) stedc_gemm_kernel(MergeArgs
     const int K = ni[0], k1 = ni[1], k2 = ni[2], k3 = ni[3];
     GemmProblem<double, double> p;
     int rowbase;
-    if (half == 0) { p.M = mid - lo; p.K = k1 + k2; rowbase = lo; p.A = a.Qw + (size_t)lo * a.ldz + lo; p.B = a.U + (size_t)lo * a.ldz + lo; }
-    else { p.M = hi - mid; p.K = k2 + k3; rowbase = mid; p.A = a.Qw + (size_t)(lo + k1) * a.ldz + mid; p.B = a.U + (size_t)lo * a.ldz + lo + k1; }
+    const int ro = row_off(lo, a.blk);
+    if (half == 0) { p.M = mid - lo; p.K = k1 + k2; rowbase = ro; p.A = a.Qw + (size_t)lo * a.ldz + ro; p.B = a.U + (size_t)lo * a.ldz + ro; }
+    else { p.M = hi - mid; p.K = k2 + k3; rowbase = mid - lo + ro; p.A = a.Qw + (size_t)(lo + k1) * a.ldz + (mid - lo + ro); p.B = a.U + (size_t)lo * a.ldz + ro + k1; }
     p.N = K; p.K2 = 0; p.A2 = nullptr; p.B2 = nullptr; p.lda = a.ldz; p.ldb = a.ldz; p.lda2 = 0; p.ldb2 = 0;
     if ((int)blockIdx.x * 64 >= p.M || (int)blockIdx.y * 64 >= p.N) return;
     ScatterEpi epi{a.Zout + (size_t)lo * a.ldz + rowbase, a.ldz, a.dest_root + lo};
@@ -618,21 +629,22 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
     const int n = w.n;
     int rc = stedc_init();
     if (rc) return rc;
-    const int D = w.depth;
+    const int D = w.depth, d0 = w.d0, blk = w.blk;      // single matrix: d0 = 0, blk = n
     // zero both eigenvector buffers: the off-diagonal quadrants of every node block are structural zeros
     if (cudaMemsetAsync(w.Za, 0, sizeof(double) * (size_t)w.ldz * n, st) != cudaSuccess) return HPSD_ECUDA_;
-    if (D > 0 && cudaMemsetAsync(w.Zb, 0, sizeof(double) * (size_t)w.ldz * n, st) != cudaSuccess) return HPSD_ECUDA_;
-    stedc_prepare_kernel<<<1, 1024, 0, st>>>(n, D, d, e, w.dmod, w.es, w.scal);
+    if (D > d0 && cudaMemsetAsync(w.Zb, 0, sizeof(double) * (size_t)w.ldz * n, st) != cudaSuccess) return HPSD_ECUDA_;
+    stedc_prepare_kernel<<<n / blk, 1024, 0, st>>>(n, D, blk, d, e, w.dmod, w.es, w.scal);
     HPSD_LAUNCH_CHECK();
     e = w.es;    // everything below works on the scaled tridiagonal
-    stedc_leaf_kernel<<<1 << D, 32, 0, st>>>(n, D, w.dmod, e, w.Za, w.ldz, w.lamA, w.info);
+    stedc_leaf_kernel<<<1 << D, 32, 0, st>>>(n, D, w.dmod, e, w.Za, w.ldz, w.lamA, w.info, blk);
     HPSD_LAUNCH_CHECK();
     double *Zin = w.Za, *Zout = w.Zb, *lin = w.lamA, *lout = w.lamB;
-    for (int k = D - 1; k >= 0; --k) {
+    for (int k = D - 1; k >= d0; --k) {
         const int nodes = 1 << k;
-        const int maxN = (n + nodes - 1) / nodes + 1;
+        const int per = 1 << (k - d0);                   // nodes per top-level block at this depth
+        const int maxN = (blk + per - 1) / per + 1;
         MergeArgs a;
-        a.n = n; a.ldz = w.ldz; a.depth = k; a.e = e;
+        a.n = n; a.ldz = w.ldz; a.depth = k; a.e = e; a.blk = blk;
         a.Zin = Zin; a.Zout = Zout; a.Qw = w.Qw; a.U = w.U; a.lam_in = lin; a.lam_out = lout;
         a.dt = w.dt; a.zt = w.zt; a.mu = w.mu; a.lamroot = w.lamroot; a.zhat = w.zhat; a.dval = w.dval;
         a.rc = w.rc; a.rs = w.rs; a.rho = w.rho;
@@ -656,7 +668,7 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
         double *t = Zin; Zin = Zout; Zout = t;
         t = lin; lin = lout; lout = t;
     }
-    stedc_unscale_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, lin, w.scal);
+    stedc_unscale_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, blk, lin, w.scal);
     HPSD_LAUNCH_CHECK();
     *lam_out = lin; *Z_out = Zin;
     return 0;
