@@ -116,12 +116,15 @@ int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void
 int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
 
 /* Tuning/testing knobs.
- *   "jacobi_max_n" (1..84, default 40): blocks with 2 <= n <= value use the one-CTA
+ *   "jacobi_max_n" (1..84, default 32): blocks with 2 <= n <= value use the one-CTA
  *       cyclic Jacobi kernel (S9).
  *   "medium_max_n" (0..116, default 116): blocks with jacobi_max_n < n <= value use the
  *       one-CTA Householder + implicit-QL kernel (S10); larger ones the multi-kernel
  *       Householder / divide-and-conquer path.  jacobi_max_n = 1 with medium_max_n = 0
  *       forces every block through the large path (used by the edge-case tests).
+ *   "medium_dc" (0/1, default 1): medium blocks with n <= 83 solve their tridiagonal eigenproblems with
+ *       the batched device-side divide & conquer (whole group as one virtual problem) instead of the
+ *       in-CTA implicit QL.
  *   "profile" (0/1): record CUDA events on the caller's stream around every stage
  *       of the path (S1..S10) for hpsd_profile_read.  Off by default. */
 int hpsd_set_option(const char *name, int value);

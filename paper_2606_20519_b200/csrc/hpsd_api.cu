@@ -2,6 +2,7 @@
 // size class per block, svec offsets sum n_k^2, workspace carve-up, launches on the caller's stream.
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <map>
 #include <memory>
 #include <mutex>
@@ -48,15 +49,19 @@ void prof_end_(int stage, cudaStream_t st) {
 namespace {
 
 struct Options {
-    int jacobi_max_n = 40;            // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
-    int medium_max_n = kMediumMaxN;   // blocks with jacobi_max_n < n <= this use the one-CTA Householder + QL kernel
+    int jacobi_max_n = 32;            // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
+    int medium_max_n = kMediumMaxN;   // blocks with jacobi_max_n < n <= this use the one-CTA Householder kernels
+    int medium_dc = 1;                // medium blocks with n <= kMedDcMaxN: batched divide & conquer instead of in-CTA QL
 } g_opt;
+
+inline bool use_meddc(const Options &o, int n) { return o.medium_dc && n > o.jacobi_max_n && n <= o.medium_max_n && n <= kMedDcMaxN; }
 
 inline int small_limit(const Options &o) { return o.medium_max_n > o.jacobi_max_n ? o.medium_max_n : o.jacobi_max_n; }
 
 struct JacobiGroup {
     int n, count;
     bool medium;        // Householder + QL kernel instead of Jacobi
+    bool dc;            // ... with the batched divide & conquer instead of in-CTA QL
     size_t off_index;   // index (in long long units) of this group's offsets in the descriptor buffer
     size_t idx_index;   // index (in int units) of this group's info indices
 };
@@ -65,7 +70,7 @@ struct LargeBlock { int n; long long off; int idx; };
 
 struct Plan {
     std::vector<int> sizes;
-    int jacobi_max_n, medium_max_n;
+    int jacobi_max_n, medium_max_n, medium_dc;
     std::vector<JacobiGroup> groups;
     std::vector<LargeBlock> large;
     int n_scalar = 0;
@@ -111,6 +116,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     pl.sizes.assign(sizes, sizes + n_blocks);
     pl.jacobi_max_n = g_opt.jacobi_max_n;
     pl.medium_max_n = g_opt.medium_max_n;
+    pl.medium_dc = g_opt.medium_dc;
     const int lim = small_limit(g_opt);
     std::vector<long long> ll;
     std::vector<int> ints;
@@ -131,6 +137,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
         JacobiGroup g;
         g.n = kv.first; g.count = (int)kv.second.size();
         g.medium = g.n > pl.jacobi_max_n;
+        g.dc = use_meddc(g_opt, g.n);
         g.off_index = ll.size(); g.idx_index = ints.size();
         for (auto &pr : kv.second) { ll.push_back(pr.first); ints.push_back(pr.second); }
         pl.groups.push_back(g);
@@ -145,6 +152,8 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
         if (cudaMemcpy(pl.desc_dev, host.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) return HPSD_ECUDA;
     }
     size_t ws = 0;
+    for (const JacobiGroup &g : pl.groups)
+        if (g.dc) ws = std::max(ws, meddc_ws_bytes(g.n, g.count));
     for (auto &lb : pl.large) {
         if (!pl.tiles_dev.count(lb.n)) {
             const size_t nt = tridiag_tile_count(lb.n);
@@ -166,7 +175,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
 // synchronises (cudaMalloc/cudaMemcpy); later calls with the same list are launch-only.
 int get_plan(DeviceState &ds, int n_blocks, const int *sizes, Plan **out) {
     for (auto &p : ds.plans) {
-        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n &&
+        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n && p->medium_dc == g_opt.medium_dc &&
             (n_blocks == 0 || std::memcmp(p->sizes.data(), sizes, sizeof(int) * n_blocks) == 0)) {
             *out = p.get();
             return 0;
@@ -211,7 +220,8 @@ int run_plan(const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStre
     }
     for (const JacobiGroup &g : pl.groups) {
         prof_begin(g.medium ? ST_MEDIUM : ST_JACOBI, st);
-        rc = g.medium ? launch_hhql_project(g.n, g.count, pl.ll(g.off_index), io, info, pl.ii(g.idx_index), st)
+        rc = g.dc ? launch_meddc_project(g.n, g.count, pl.ll(g.off_index), io, scratch, info, pl.ii(g.idx_index), st)
+           : g.medium ? launch_hhql_project(g.n, g.count, pl.ll(g.off_index), io, info, pl.ii(g.idx_index), st)
                       : launch_jacobi_project(g.n, g.count, pl.ll(g.off_index), io, info, pl.ii(g.idx_index), st);
         prof_end(g.medium ? ST_MEDIUM : ST_JACOBI, st);
         if (rc) return rc;
@@ -255,6 +265,10 @@ int hpsd_set_option(const char *name, int value) {
         g_opt.jacobi_max_n = value;
         return HPSD_OK;
     }
+    if (std::strcmp(name, "medium_dc") == 0) {
+        g_opt.medium_dc = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "medium_max_n") == 0) {
         if (value < 0 || value > kMediumMaxN) return HPSD_EINVAL;
         g_opt.medium_max_n = value;
@@ -293,11 +307,14 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     int rc = check_args(n_blocks, sizes, (void *)1, (void *)1, &total);
     if (rc) return rc;
     size_t ws = 0;
-    for (int b = 0; b < n_blocks; ++b)
+    std::map<int, int> dc_count;
+    for (int b = 0; b < n_blocks; ++b) {
         if (sizes[b] > small_limit(g_opt)) {
             const size_t w = largepath_ws_bytes(sizes[b]);
             if (w > ws) ws = w;
-        }
+        } else if (use_meddc(g_opt, sizes[b])) dc_count[sizes[b]]++;
+    }
+    for (auto &kv : dc_count) ws = std::max(ws, meddc_ws_bytes(kv.first, kv.second));
     *bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int) + 4, 256) + 256;
     return HPSD_OK;
 }

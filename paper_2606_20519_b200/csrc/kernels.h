@@ -28,6 +28,12 @@ constexpr int kMediumMaxN = 116;
 int launch_hhql_project(int n, int count, const long long *offs_dev, const SvecIo &io,
                         int *info_dev, const int *info_idx_dev, cudaStream_t st);
 int medium_init();
+// Batched divide-and-conquer variant (n <= kMedDcMaxN: reflectors and kept eigenvectors both fit in shared memory);
+// scratch >= meddc_ws_bytes(n, count), 256-byte aligned.
+constexpr int kMedDcMaxN = 83;
+size_t meddc_ws_bytes(int n, int count);
+int launch_meddc_project(int n, int count, const long long *offs_dev, const SvecIo &io, unsigned char *scratch,
+                         int *info_dev, const int *info_idx_dev, cudaStream_t st);
 
 // ---- peak.cu ---------------------------------------------------------------
 int launch_fp64_probe(int kind, int iters, double *flops_host, cudaStream_t st);

@@ -12,6 +12,7 @@
 //
 // Only one n x n complex array is needed (105 KB at n = 81: two CTAs per SM, so 256 matrices are one wave).
 #include "kernels.h"
+#include "large.h"
 
 namespace hpsd {
 
@@ -390,9 +391,199 @@ __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const 
     MTRACE(5);
 }
 
+// =====================================================================================================
+// Batched divide-and-conquer variant of S10 (n <= kMedDcMaxN): the serial QL generator above costs ~480 cycles
+// per rotation; here the tridiagonal eigenproblems of a whole group of equal-size blocks are solved by the
+// device-side D&C of stedc.cu, the group being ONE virtual tridiagonal of size blk 2^d0 whose top d0 levels are
+// never merged.  Kernel A: unpack + Householder tridiagonalisation per CTA (reflectors, tau, d, e to global);
+// stedc; kernel C: W = Q Z_+ diag(sqrt(lambda_+)) by applying the reflectors to the kept columns in shared
+// memory, then HERK + pack.
+// =====================================================================================================
+struct MedDcWs {
+    int n, count, B, ld;          // block size, blocks, padded batch (power of two), leading dimension of the reflectors
+    cplx *Ar;                     // count x (n x ld): reflectors (column c rows c+1.. = v_c)
+    cplx *tau;                    // B n
+    double *d, *e;                // B n
+    int *info;                    // 1: D&C failure flag of the group
+    StedcWs s;
+};
+
+__global__ void __launch_bounds__(kMedThreads) meddc_tridiag_kernel(int n, const long long *__restrict__ offs, SvecIo io, MedDcWs w) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ld = med_ld(n);
+    MedSmem sm = med_carve(smem_raw, n);
+    cplx *A = sm.A;
+    const int tid = threadIdx.x, t = blockIdx.x;
+    const size_t base = (size_t)offs[t];
+    for (int q = tid; q < n * n; q += kMedThreads) {
+        const int j = q / n, i = q % n;
+        if (i < j) continue;
+        const size_t c = base + svec_col_off(n, j);
+        if (i == j) A[(size_t)j * ld + i] = mk(io_load(io, c), 0.0);
+        else {
+            const int k = i - j - 1;
+            const cplx v = mk(io_load(io, c + 1 + 2 * k) / kSqrt2, io_load(io, c + 2 + 2 * k) / kSqrt2);
+            A[(size_t)j * ld + i] = v;
+            A[(size_t)i * ld + j] = conj_(v);
+        }
+    }
+    __syncthreads();
+    med_tridiagonalize(sm, n, ld);
+    cplx *Ag = w.Ar + (size_t)t * n * w.ld;
+    for (int q = tid; q < n * n; q += kMedThreads) {
+        const int j = q / n, i = q % n;
+        if (i > j) Ag[(size_t)j * w.ld + i] = A[(size_t)j * ld + i];
+    }
+    for (int i = tid; i < n; i += kMedThreads) {
+        w.tau[(size_t)t * n + i] = sm.tau[i];
+        w.d[(size_t)t * n + i] = sm.d[i];
+        w.e[(size_t)t * n + i] = sm.e[i];
+    }
+}
+
+__global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const long long *__restrict__ offs, SvecIo io, MedDcWs w,
+                                                                 const double *__restrict__ lam, const double *__restrict__ Z, int ldz,
+                                                                 int *__restrict__ info, const int *__restrict__ info_idx) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ld = med_ld(n);
+    cplx *A = reinterpret_cast<cplx *>(smem_raw);               // n x ld reflectors
+    cplx *Wm = A + (size_t)n * ld;                               // n x ld kept eigenvectors
+    cplx *tau = Wm + (size_t)n * ld;                             // n
+    cplx *sv = tau + n;                                          // n : v^H W
+    double *lm = reinterpret_cast<double *>(sv + n);             // n
+    __shared__ int s_p0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, t = blockIdx.x;
+    const cplx *Ag = w.Ar + (size_t)t * n * w.ld;
+    for (int q = tid; q < n * n; q += kMedThreads) {
+        const int j = q / n, i = q % n;
+        if (i > j) A[(size_t)j * ld + i] = Ag[(size_t)j * w.ld + i];
+    }
+    for (int i = tid; i < n; i += kMedThreads) { tau[i] = w.tau[(size_t)t * n + i]; lm[i] = lam[(size_t)t * n + i]; }
+    __syncthreads();
+    if (tid == 0) {
+        int lo = 0, hi = n;                                      // eigenvalues ascending: first index with lam > 0
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (lm[mid] > 0.0) hi = mid; else lo = mid + 1; }
+        s_p0 = lo;
+        if (info != nullptr) info[info_idx[t]] = (w.info != nullptr && *w.info) ? *w.info : 0;
+    }
+    __syncthreads();
+    const int p0 = s_p0, kpos = n - p0;
+    // S6: W = Z_+ diag(sqrt(lambda_+)), real -> complex
+    const double *Zt = Z + (size_t)t * n * ldz;
+    for (int q = tid; q < kpos * n; q += kMedThreads) {
+        const int j = q / n, r = q % n;
+        Wm[(size_t)j * ld + r] = mk(sqrt(lm[p0 + j]) * Zt[(size_t)(p0 + j) * ldz + r], 0.0);
+    }
+    __syncthreads();
+    // S5: W <- H_0 H_1 ... H_{n-2} W, last reflector first
+    for (int k = n - 2; k >= 0; --k) {
+        const cplx tk = tau[k];
+        if (tk.x == 0.0 && tk.y == 0.0) continue;                // block-uniform
+        for (int base = 0; base < kpos; base += 64) {
+            const int j = base + (lane & 7) + 8 * warp;
+            cplx acc = mk(0.0, 0.0);
+            if (j < kpos)
+                for (int r = k + 1 + (lane >> 3); r < n; r += 4) cfma_conj(acc, A[(size_t)k * ld + r], Wm[(size_t)j * ld + r]);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+            if (j < kpos && lane < 8) sv[j] = tk * acc;
+        }
+        __syncthreads();
+        const int m = n - k - 1;
+        for (int q = tid; q < m * kpos; q += kMedThreads) {
+            const int rr = q % m, j = q / m;
+            const int r = k + 1 + rr;
+            const cplx v = A[(size_t)k * ld + r], s = sv[j];
+            cplx x = Wm[(size_t)j * ld + r];
+            x.x -= v.x * s.x - v.y * s.y;
+            x.y -= v.x * s.y + v.y * s.x;
+            Wm[(size_t)j * ld + r] = x;
+        }
+        __syncthreads();
+    }
+    // S7 + S8
+    const size_t obase = (size_t)offs[t];
+    for (int q = tid; q < n * n; q += kMedThreads) {
+        const int j = q / n, i = q % n;
+        if (i < j) continue;
+        cplx acc = mk(0.0, 0.0);
+        for (int l = 0; l < kpos; ++l) {
+            const cplx a = Wm[(size_t)l * ld + i], b = Wm[(size_t)l * ld + j];
+            acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+            acc.y = fma(a.y, b.x, acc.y); acc.y = fma(-a.x, b.y, acc.y);
+        }
+        const size_t c = obase + svec_col_off(n, j);
+        if (i == j) io_store(io, c, acc.x);
+        else {
+            const int k = i - j - 1;
+            io_store(io, c + 1 + 2 * k, kSqrt2 * acc.x);
+            io_store(io, c + 2 + 2 * k, kSqrt2 * acc.y);
+        }
+    }
+}
+
+static size_t meddc_back_smem(int n) {
+    return sizeof(cplx) * (2 * (size_t)n * med_ld(n) + 2 * (size_t)n) + sizeof(double) * n + 64;
+}
+
+static int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+// Carve the scratch of one group (base may be nullptr: size query).
+static size_t meddc_carve(int n, int count, unsigned char *base, MedDcWs &w) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> unsigned char * { unsigned char *p = base ? base + off : nullptr; off += align_up(bytes, 256); return p; };
+    auto dbl = [&](size_t c) { return reinterpret_cast<double *>(take(sizeof(double) * c)); };
+    auto itg = [&](size_t c) { return reinterpret_cast<int *>(take(sizeof(int) * c)); };
+    const int B = next_pow2(count);
+    int d0 = 0; while ((1 << d0) < B) ++d0;
+    const size_t N = (size_t)B * n;
+    const int ldz = (int)align_up((size_t)n, 8);
+    w.n = n; w.count = count; w.B = B; w.ld = n;
+    w.Ar = reinterpret_cast<cplx *>(take(sizeof(cplx) * (size_t)count * n * n));
+    w.tau = reinterpret_cast<cplx *>(take(sizeof(cplx) * N));
+    w.d = dbl(N); w.e = dbl(N);
+    w.info = itg(4);
+    StedcWs &s = w.s;
+    s.n = (int)N; s.ldz = ldz; s.blk = n; s.d0 = d0; s.depth = d0 + stedc_depth(n);
+    s.Za = dbl((size_t)ldz * N); s.Zb = dbl((size_t)ldz * N); s.Qw = dbl((size_t)ldz * N); s.U = dbl((size_t)ldz * N);
+    s.lamA = dbl(N); s.lamB = dbl(N); s.dmod = dbl(N); s.es = dbl(N); s.scal = dbl(2 * (size_t)B);
+    s.dt = dbl(N); s.zt = dbl(N); s.mu = dbl(N); s.lamroot = dbl(N); s.zhat = dbl(N); s.dval = dbl(N); s.rc = dbl(N); s.rs = dbl(N);
+    s.org = itg(N); s.grow = itg(N); s.gsrc = itg(N); s.dcol = itg(N);
+    s.dest_root = itg(N); s.dest_defl = itg(N); s.rp = itg(N); s.rq = itg(N);
+    const size_t maxnodes = (size_t)1 << (s.depth > 0 ? s.depth - 1 : 0);
+    s.nodeinfo = itg(8 * maxnodes);
+    s.rho = dbl(maxnodes);
+    s.info = w.info;
+    return off;
+}
+
+size_t meddc_ws_bytes(int n, int count) { MedDcWs w; return meddc_carve(n, count, nullptr, w); }
+
+int launch_meddc_project(int n, int count, const long long *offs_dev, const SvecIo &io, unsigned char *scratch,
+                         int *info_dev, const int *info_idx_dev, cudaStream_t st) {
+    if (count <= 0) return 0;
+    if (n < 2 || n > kMedDcMaxN || (long long)next_pow2(count) * n > kMaxLargeN * 64LL) return -1;
+    MedDcWs w;
+    meddc_carve(n, count, scratch, w);
+    const size_t N = (size_t)w.B * n;
+    if (cudaMemsetAsync(w.d, 0, sizeof(double) * N, st) != cudaSuccess) return HPSD_ECUDA_;   // padding blocks: zero matrices
+    if (cudaMemsetAsync(w.e, 0, sizeof(double) * N, st) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaMemsetAsync(w.info, 0, sizeof(int) * 4, st) != cudaSuccess) return HPSD_ECUDA_;
+    meddc_tridiag_kernel<<<count, kMedThreads, med_smem_bytes(n), st>>>(n, offs_dev, io, w);
+    HPSD_LAUNCH_CHECK();
+    double *lam, *Z;
+    int rc = launch_stedc(w.s, w.d, w.e, &lam, &Z, st);
+    if (rc) return rc;
+    meddc_back_kernel<<<count, kMedThreads, meddc_back_smem(n), st>>>(n, offs_dev, io, w, lam, Z, w.s.ldz, info_dev, info_idx_dev);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
 int medium_init() {
     const int maxb = (int)med_smem_bytes(kMediumMaxN);
     if (cudaFuncSetAttribute(hhql_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, maxb) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(meddc_tridiag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)med_smem_bytes(kMedDcMaxN)) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(meddc_back_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)meddc_back_smem(kMedDcMaxN)) != cudaSuccess) return HPSD_ECUDA_;
     return 0;
 }
 

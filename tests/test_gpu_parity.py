@@ -29,7 +29,7 @@ def hp():
 
 def force_large(hp, on):
     """Route every block through S1..S8 of the multi-kernel path (on) or restore the defaults (off)."""
-    hp.set_option("jacobi_max_n", 1 if on else 40)
+    hp.set_option("jacobi_max_n", 1 if on else 32)
     hp.set_option("medium_max_n", 0 if on else 116)
 
 
@@ -203,12 +203,12 @@ def test_small_path_sizes(orc, hp, n):
         got, _ = check_vs_oracle(orc, hp, sizes, sv)
         check_invariants(hp, sizes, sv, got)
     finally:
-        hp.set_option("jacobi_max_n", 40)
+        hp.set_option("jacobi_max_n", 32)
 
 
-@pytest.mark.parametrize("n", [41, 47, 64, 65, 81, 84, 100, 115, 116])
+@pytest.mark.parametrize("n", [33, 36, 47, 64, 65, 81, 83, 84, 100, 115, 116])
 def test_medium_path_sizes(orc, hp, n):
-    """S10: one-CTA Householder + QL kernel (default route for 40 < n <= 116)."""
+    """S10 (default route for 32 < n <= 116): batched divide & conquer up to n = 83, in-CTA QL above."""
     rng = np.random.default_rng(250 + n)
     sizes = [n] * 3
     sv = pack_all(orc, [herm(rng, n) for _ in sizes])
@@ -216,9 +216,25 @@ def test_medium_path_sizes(orc, hp, n):
     check_invariants(hp, sizes, sv, got)
 
 
+@pytest.mark.parametrize("n,count", [(33, 1), (36, 5), (64, 2), (81, 7), (83, 1)])
+def test_medium_path_in_cta_ql(orc, hp, n, count):
+    """The in-CTA QL variant of S10 on sizes the batched D&C normally takes (option medium_dc = 0), and batch
+    counts that are not powers of two for the D&C variant (the batch is padded with zero matrices)."""
+    rng = np.random.default_rng(260 + n)
+    sizes = [n] * count
+    sv = pack_all(orc, [herm(rng, n) for _ in sizes])
+    got_dc, _ = check_vs_oracle(orc, hp, sizes, sv)
+    hp.set_option("medium_dc", 0)
+    try:
+        got_ql, _ = check_vs_oracle(orc, hp, sizes, sv)
+    finally:
+        hp.set_option("medium_dc", 1)
+    assert rel_err(got_ql, got_dc) <= TOL * n
+
+
 @pytest.mark.parametrize("n", [2, 5, 16, 31])
 def test_medium_kernel_on_small_sizes(orc, hp, n):
-    """The S10 kernel itself has no lower size limit: route small blocks through it."""
+    """The S10 kernels have no lower size limit: route small blocks through them (D&C with a single leaf)."""
     rng = np.random.default_rng(270 + n)
     sizes = [n] * 2
     sv = pack_all(orc, [herm(rng, n) for _ in sizes])
@@ -226,7 +242,7 @@ def test_medium_kernel_on_small_sizes(orc, hp, n):
     try:
         check_vs_oracle(orc, hp, sizes, sv)
     finally:
-        hp.set_option("jacobi_max_n", 40)
+        hp.set_option("jacobi_max_n", 32)
 
 
 @pytest.mark.parametrize("n", [2, 3, 31, 32, 33, 63, 64, 65, 85, 96, 127, 128, 129, 200, 257, 320])

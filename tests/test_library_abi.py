@@ -49,16 +49,20 @@ def test_argument_errors_without_gpu(lib):
     ok = (ctypes.c_int * 3)(16, 625, 36)
     assert lib.hpsd_workspace_size(3, ok, ctypes.byref(sz)) == 0
     assert sz.value > 16 * 625 * 625          # at least one complex copy of the large block
-    small = (ctypes.c_int * 2)(16, 36)
+    small = (ctypes.c_int * 2)(16, 30)
     sz2 = ctypes.c_size_t(0)
     assert lib.hpsd_workspace_size(2, small, ctypes.byref(sz2)) == 0
     assert sz2.value < 4096                   # Jacobi blocks need no scratch, only the info words
+    med = (ctypes.c_int * 3)(81, 81, 16)
+    sz3 = ctypes.c_size_t(0)
+    assert lib.hpsd_workspace_size(3, med, ctypes.byref(sz3)) == 0
+    assert 16 * 2 * 81 * 81 < sz3.value < 1 << 22   # batched D&C scratch of the two n=81 blocks
     assert lib.hpsd_set_option(b"no_such_option", 1) == -1
     assert lib.hpsd_set_option(b"jacobi_max_n", 0) == -1
     assert lib.hpsd_set_option(b"jacobi_max_n", 84) == 0
     assert lib.hpsd_set_option(b"medium_max_n", 117) == -1
     assert lib.hpsd_set_option(b"medium_max_n", 116) == 0
-    assert lib.hpsd_set_option(b"jacobi_max_n", 40) == 0
+    assert lib.hpsd_set_option(b"jacobi_max_n", 32) == 0
     assert lib.hpsd_project(0, None, None, None, None) == 0       # empty list: nothing to do
 
 
