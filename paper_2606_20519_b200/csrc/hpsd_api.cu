@@ -269,6 +269,10 @@ int hpsd_set_option(const char *name, int value) {
         g_opt.medium_dc = (value != 0);
         return HPSD_OK;
     }
+    if (std::strcmp(name, "cluster_tridiag") == 0) {
+        g_cluster_tridiag = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "medium_max_n") == 0) {
         if (value < 0 || value > kMediumMaxN) return HPSD_EINVAL;
         g_opt.medium_max_n = value;

@@ -73,6 +73,7 @@ LargeWs carve(int n, unsigned char *base) {
 }
 
 int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, const double *sub, cudaStream_t st) {
+    if (g_cluster_tridiag && tridiag_cluster_fits(n)) return launch_tridiag_cluster(w.t, in, sub, st);
     if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     prof_begin(ST_UNPACK, st);

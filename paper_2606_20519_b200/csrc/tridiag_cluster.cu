@@ -1,0 +1,456 @@
+// tridiag_cluster.cu -- S1 + S2 + S3 of SURVEY.md §8(a) for blocks whose lower triangle fits in the
+// shared memory of ONE 16-CTA thread-block cluster (n <= ~640: the paper's d = 5, n = 625 block).
+// svec -> REAL symmetric tridiagonal (d, e) + reflectors V, tau, same conventions as tridiag.cu:
+// A = Q T Q^H, Q = H_0 ... H_{n-2}, H_c = I - tau_c v_c v_c^H (zlarfg: complex tau, real beta).
+// "Eigendecomposition" of PAPER.md:1536 starts here; the design is ours (the paper calls a library).
+//
+// Why: at n = 625 the grid-wide panel kernel is bound by two grid barriers per column (1.1-1.5 us
+// each on B200).  A cluster barrier costs ~0.2 us, and 16 x 227 KB of distributed
+// shared memory hold the whole packed lower triangle (3.1 MB at n = 625), so the matrix is read from
+// HBM exactly once (straight from the svec: S1 is fused) and every column step runs out of shared memory.
+//
+// Layout: column j belongs to CTA j mod 16 and is stored packed (rows j..n-1, contiguous).
+// Rows are owned by threads: row i = 32 (8 s + warp) + lane for register slot s < 3; each thread
+// keeps v_i, w_i, u_i of its rows in registers.
+//
+// Step c (unblocked, LAPACK zhetd2 arithmetic, one fused pass per column):
+//   [A] every CTA (redundantly, bit-identically) forms column c of the current matrix from the raw
+//       column the owner exported, a' = raw - v conj(w_c) - w, its Householder vector u = v_c, tau, beta;
+//   [B] one pass over the CTA's own columns j >= c+1: A_ij -= v_i conj(w_j) + w_i conj(v_j) (the
+//       rank-2 update of step c-1, applied late) and, in the same sweep, z_i += A_ij u_j,
+//       t_j += conj(A_ij) u_i (the Hermitian mat-vec of step c from the stored half);
+//   [C] contributions z_i (+ t_i) are pushed through DSMEM to CTA i mod 16, partial v^H y to everybody;
+//       cluster barrier 1;
+//   [D] CTA i mod 16 sums the 16 contributions of its rows and broadcasts tau y_i; cluster barrier 2;
+//       w_i = tau y_i - 1/2 |tau|^2 (v^H y) u_i is completed by every receiver.
+// The raw next column travels through a two-entry ring in global memory (L2): one writer, 16 readers,
+// ordered by the release/acquire of cluster barrier 1.
+#include <cooperative_groups.h>
+#include "kernels.h"
+#include "large.h"
+#include "prof.h"
+
+namespace cg = cooperative_groups;
+
+namespace hpsd {
+
+constexpr int kCl = 16;            // CTAs per cluster (non-portable size)
+constexpr int kClThreads = 512;
+constexpr int kClWarps = kClThreads / 32;
+constexpr int kClR = 2;            // row slots per thread: n <= 1024
+constexpr int kClMaxN = 32 * kClWarps * kClR;
+constexpr int kKT = 2;             // own columns per trip of the pass
+constexpr int kRedN = 0, kRedQ = kClWarps, kRedS = 2 * kClWarps;   // s_red: norm partials | dot partials | alpha.x, alpha.y, d_c
+// 32-row chunk of (slot, warp): odd slots run backwards so that every warp gets a light and a heavy chunk
+__device__ __forceinline__ int cl_chunk(int s, int wp) { return kClWarps * s + ((s & 1) ? kClWarps - 1 - wp : wp); }
+__device__ __forceinline__ void cl_barrier() {
+    // release/acquire at CLUSTER scope (cooperative_groups' cluster.sync() fences at gpu scope: MEMBAR.ALL.GPU)
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+struct ClusterArgs {
+    int n, lda;
+    const double *in, *sub;        // svec (and the ADMM subtrahend, or null)
+    cplx *A;                       // lda x n: reflectors out (zero on and above the diagonal)
+    cplx *raw;                     // 2 x lda ring of exported raw columns
+    double *d, *e;
+    cplx *tau;
+};
+
+__host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + kCl - 1) / kCl : 0; }
+__host__ __device__ inline size_t cl_col_off(int n, int r, int jl) { return (size_t)jl * (n - r) - (size_t)8 * jl * (jl - 1); }
+
+struct ClusterSmem {
+    size_t colv, q, red, ysum, rbuf, wbuf, stor, total;
+};
+__host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
+    ClusterSmem s;
+    const int nc = cl_ncols(n, 0);                 // widest CTA
+    const int rs = (n + kCl - 1) / kCl;
+    size_t off = 0;
+    s.colv = off; off += sizeof(cplx) * 3 * nc;
+    s.q = off; off += sizeof(double) * kCl;
+    s.red = off; off += sizeof(double) * (2 * kClWarps + 4);   // block-reduction scratch + alpha, d_c
+    s.ysum = off; off += sizeof(cplx) * rs;        // tau y of the rows this CTA reduces
+    s.rbuf = off; off += sizeof(cplx) * kCl * (rs | 1);
+    s.wbuf = off;
+    const size_t wb = sizeof(cplx) * n, tp = sizeof(cplx) * kClWarps * nc;
+    off += wb > tp ? wb : tp;                      // wbuf is dead during the pass: aliased with the t_j partials
+    s.stor = off;
+    off += sizeof(cplx) * cl_col_off(n, r, cl_ncols(n, r));
+    s.total = off;
+    return s;
+}
+
+__device__ __forceinline__ void cl_householder(cplx alpha, double xnorm2, double &beta, cplx &tau, cplx &scale) {
+    if (xnorm2 == 0.0 && alpha.y == 0.0) {
+        beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
+    } else {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        beta = -copysign(nrm, alpha.x);
+        const double ib = 1.0 / beta;
+        tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
+        const cplx den = mk(alpha.x - beta, alpha.y);
+        const double id2 = 1.0 / abs2(den);
+        scale = mk(den.x * id2, -den.y * id2);
+    }
+}
+
+// element (i, j), i >= j, of the input matrix from the svec (Eq. D10 inverted; same arithmetic as unpack_kernel)
+__device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, const double *__restrict__ sub, int n, int i, int j) {
+    const size_t o = svec_col_off(n, j);
+    if (i == j) return mk(sub ? sv[o] - sub[o] : sv[o], 0.0);
+    const size_t k = o + 1 + 2 * (size_t)(i - j - 1);
+    double re = sv[k], im = sv[k + 1];
+    if (sub) { re -= sub[k]; im -= sub[k + 1]; }
+    return mk(re / kSqrt2, im / kSqrt2);
+}
+
+#ifdef HPSD_PANEL_TRACE
+// dev-only: clock64 at eight points of every 8th column step, CTA 0 / thread 0
+__device__ long long g_cltrace[128 * 8];
+__device__ long long g_cltrace2[8 * 16 * 4];
+#define CLT2(pt) do { if (r == 0 && lane == 0 && c == 0) g_cltrace2[(wp * 16 + ((jl - jl0) >> 2)) * 4 + (pt)] = clock64(); } while (0)
+#define CLTRACE(slot) do { if (r == 0 && tid == 0 && (c & 7) == 0 && (c >> 3) < 128) g_cltrace[(c >> 3) * 8 + (slot)] = clock64(); } while (0)
+#else
+#define CLTRACE(slot) do {} while (0)
+#define CLT2(pt) do {} while (0)
+#endif
+
+__global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterArgs p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const int r = (int)cluster.block_rank();
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int n = p.n, lda = p.lda;
+    const ClusterSmem L = cl_smem(n, r);
+    cplx *colv_v = reinterpret_cast<cplx *>(smem_raw + L.colv);
+    const int ncw = cl_ncols(n, 0);
+    cplx *colv_w = colv_v + ncw, *colv_u = colv_w + ncw;
+    double *s_q = reinterpret_cast<double *>(smem_raw + L.q);
+    double *s_red = reinterpret_cast<double *>(smem_raw + L.red);   // kRedN.. norm, kRedQ.. dot, kRedS.. alpha, d_c
+    cplx *ysum = reinterpret_cast<cplx *>(smem_raw + L.ysum);
+    cplx *rbuf = reinterpret_cast<cplx *>(smem_raw + L.rbuf);                 // [sender][RSP]
+    const int RS = (n + kCl - 1) / kCl, RSP = RS | 1;
+    cplx *wbuf = reinterpret_cast<cplx *>(smem_raw + L.wbuf);
+    cplx *tpart = wbuf;                                               // [warp][ncw], alive only inside a step
+    cplx *stor = reinterpret_cast<cplx *>(smem_raw + L.stor);
+    const int nc = cl_ncols(n, r);
+
+    // ---- S1 fused: own columns straight from the svec into shared memory (one warp per column)
+    for (int jl = wp; jl < nc; jl += kClWarps) {
+        const int j = r + kCl * jl;
+        cplx *col = stor + cl_col_off(n, r, jl);
+        for (int i = j + lane; i < n; i += 32) col[i - j] = cl_load_svec(p.in, p.sub, n, i, j);
+    }
+    int row[kClR], dest[kClR], dslot[kClR];
+    cplx v[kClR], w[kClR], u[kClR], z[kClR], raw[kClR];
+#pragma unroll
+    for (int s = 0; s < kClR; ++s) {
+        row[s] = 32 * cl_chunk(s, wp) + lane;
+        dest[s] = row[s] / RS; dslot[s] = row[s] - dest[s] * RS;       // reducer CTA of the row and its slot there
+        v[s] = w[s] = u[s] = z[s] = mk(0.0, 0.0);
+        raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0) : mk(0.0, 0.0);
+    }
+    cplx wc = mk(0.0, 0.0);
+    cl_barrier();       // every CTA of the cluster is resident before the first DSMEM access
+
+    for (int c = 0; c < n; ++c) {
+        // ================= [A] column c of the current matrix, Householder vector =================
+        CLTRACE(0);
+        cplx a[kClR];
+        double xn = 0.0;
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) {
+            const int i = row[s];
+            cplx t = mk(0.0, 0.0);
+            if (i >= c && i < n) {
+                t = raw[s] - w[s];
+                t.x -= v[s].x * wc.x + v[s].y * wc.y;       // v conj(wc)
+                t.y -= v[s].y * wc.x - v[s].x * wc.y;
+            }
+            a[s] = t;
+            if (i == c) s_red[kRedS + 2] = t.x;
+            if (i == c + 1) { s_red[kRedS] = t.x; s_red[kRedS + 1] = t.y; }
+            if (i >= c + 2) xn += abs2(t);
+        }
+        xn = warp_sum(xn);
+        if (lane == 0) s_red[kRedN + wp] = xn;
+        __syncthreads();
+        CLTRACE(1);
+        const double dc = s_red[kRedS + 2];
+        if (c == n - 1) {
+            if (r == (c & (kCl - 1))) {
+                if (tid == 0) { p.d[c] = dc; p.e[c] = 0.0; p.tau[c] = mk(0.0, 0.0); }
+#pragma unroll
+                for (int s = 0; s < kClR; ++s) if (row[s] < n) p.A[(size_t)c * lda + row[s]] = mk(0.0, 0.0);
+            }
+            break;
+        }
+        double xnorm2 = 0.0;
+#pragma unroll
+        for (int k = 0; k < kClWarps; ++k) xnorm2 += s_red[kRedN + k];
+        const cplx alpha = mk(s_red[kRedS], s_red[kRedS + 1]);
+        double beta; cplx tau, scale;
+        cl_householder(alpha, xnorm2, beta, tau, scale);
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) {
+            const int i = row[s];
+            u[s] = (i == c + 1) ? mk(1.0, 0.0) : ((i > c + 1 && i < n) ? scale * a[s] : mk(0.0, 0.0));
+            if (i < n && (i & (kCl - 1)) == r && i >= c + 1) {
+                const int jl = i >> 4;
+                colv_v[jl] = v[s]; colv_w[jl] = w[s]; colv_u[jl] = u[s];
+            }
+        }
+        if (r == (c & (kCl - 1))) {
+            if (tid == 0) { p.d[c] = dc; p.e[c] = beta; p.tau[c] = tau; }
+#pragma unroll
+            for (int s = 0; s < kClR; ++s) if (row[s] < n) p.A[(size_t)c * lda + row[s]] = u[s];   // zero for rows <= c
+        }
+        __syncthreads();
+        CLTRACE(2);
+
+        // ================= [B] fused rank-2 update (step c-1) + Hermitian mat-vec (step c) =================
+        // Four own columns per trip: twelve independent element chains per thread hide the shared-memory
+        // and DFMA latencies; the four t_j are reduced over the warp by one halving butterfly.
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) z[s] = mk(0.0, 0.0);
+        const int jl0 = (c + 1 > r) ? (c + 1 - r + kCl - 1) / kCl : 0;
+        cplx *rawn = p.raw + (size_t)((c + 1) & 1) * lda;
+        for (int jl = jl0; jl < nc; jl += kKT) {
+            const int j0 = r + kCl * jl;
+            CLT2(0);
+            cplx cv[kKT], cw[kKT], cu[kKT], tj[kKT];
+            cplx *col[kKT];
+#pragma unroll
+            for (int k = 0; k < kKT; ++k) {
+                const bool okc = jl + k < nc;
+                const int jk = okc ? jl + k : jl;
+                cv[k] = colv_v[jk]; cw[k] = colv_w[jk];
+                cu[k] = okc ? colv_u[jk] : mk(0.0, 0.0);
+                col[k] = stor + cl_col_off(n, r, jk) - (r + kCl * jk);   // col[k][i] = A(i, j_k)
+                tj[k] = mk(0.0, 0.0);
+            }
+            const bool exp_col = (j0 == c + 1);                   // only the first column of a trip can be column c+1
+            cplx x[kClR][kKT];
+            bool ok[kClR][kKT];
+#pragma unroll
+            for (int s = 0; s < kClR; ++s) {
+                const int i0 = 32 * cl_chunk(s, wp);
+                const bool slot_on = !(i0 + 31 < j0 || i0 >= n);   // warp-uniform
+#pragma unroll
+                for (int k = 0; k < kKT; ++k) {
+                    const int i = i0 + lane;
+                    ok[s][k] = slot_on && (jl + k < nc) && i >= j0 + kCl * k && i < n;
+#if defined(HPSD_CLX) && HPSD_CLX == 3
+                    x[s][k] = mk(1.0 * i, 0.5);
+#else
+                    x[s][k] = ok[s][k] ? col[k][i] : mk(0.0, 0.0);
+#endif
+                }
+            }
+            CLT2(1);
+#pragma unroll
+            for (int s = 0; s < kClR; ++s) {
+                const int i = 32 * cl_chunk(s, wp) + lane;
+#pragma unroll
+                for (int k = 0; k < kKT; ++k) {
+                    if (!ok[s][k]) continue;
+                    cplx xx = x[s][k];
+                    // xx -= v_i conj(w_j) + w_i conj(v_j)
+                    xx.x = fma(-v[s].x, cw[k].x, xx.x); xx.x = fma(-v[s].y, cw[k].y, xx.x);
+                    xx.x = fma(-w[s].x, cv[k].x, xx.x); xx.x = fma(-w[s].y, cv[k].y, xx.x);
+                    xx.y = fma(-v[s].y, cw[k].x, xx.y); xx.y = fma(v[s].x, cw[k].y, xx.y);
+                    xx.y = fma(-w[s].y, cv[k].x, xx.y); xx.y = fma(w[s].x, cv[k].y, xx.y);
+                    const int j = j0 + kCl * k;
+                    if (i == j) xx.y = 0.0;
+#if defined(HPSD_CLX) && HPSD_CLX == 2
+                    if (k == 0 && exp_col) rawn[i] = xx;
+#else
+                    if (k == 0 && exp_col) rawn[i] = xx; else col[k][i] = xx;
+#endif
+                    cfma(z[s], xx, cu[k]);
+                    if (i > j) cfma_conj(tj[k], xx, u[s]);
+                }
+            }
+            CLT2(2);
+            // halving butterfly: kKT values x 32 lanes -> lane 32 q / kKT holds the total of column q
+            {
+                cplx kp;
+                if constexpr (kKT == 4) {
+                    const bool hi = (lane & 16) != 0, b8 = (lane & 8) != 0;
+                    const cplx s0 = hi ? tj[0] : tj[2], s1 = hi ? tj[1] : tj[3];
+                    cplx k0 = hi ? tj[2] : tj[0], k1 = hi ? tj[3] : tj[1];
+                    k0.x += __shfl_xor_sync(0xffffffffu, s0.x, 16); k0.y += __shfl_xor_sync(0xffffffffu, s0.y, 16);
+                    k1.x += __shfl_xor_sync(0xffffffffu, s1.x, 16); k1.y += __shfl_xor_sync(0xffffffffu, s1.y, 16);
+                    const cplx snd = b8 ? k0 : k1;
+                    kp = b8 ? k1 : k0;
+                    kp.x += __shfl_xor_sync(0xffffffffu, snd.x, 8); kp.y += __shfl_xor_sync(0xffffffffu, snd.y, 8);
+                } else {
+                    static_assert(kKT == 2 || kKT == 4, "butterfly written for 2 or 4 columns per trip");
+                    const bool hi = (lane & 16) != 0;
+                    const cplx snd = hi ? tj[0] : tj[kKT - 1];
+                    kp = hi ? tj[kKT - 1] : tj[0];
+                    kp.x += __shfl_xor_sync(0xffffffffu, snd.x, 16); kp.y += __shfl_xor_sync(0xffffffffu, snd.y, 16);
+                    kp.x += __shfl_xor_sync(0xffffffffu, kp.x, 8); kp.y += __shfl_xor_sync(0xffffffffu, kp.y, 8);
+                }
+#pragma unroll
+                for (int o = 4; o > 0; o >>= 1) {
+                    kp.x += __shfl_xor_sync(0xffffffffu, kp.x, o); kp.y += __shfl_xor_sync(0xffffffffu, kp.y, o);
+                }
+                const int idx = lane / (32 / kKT);
+                if ((lane & (32 / kKT - 1)) == 0 && jl + idx < nc) tpart[wp * ncw + jl + idx] = kp;
+            }
+            CLT2(3);
+        }
+        __syncthreads();
+        CLTRACE(3);
+
+        // ================= [C] contributions to y = A v: reduce-scatter through DSMEM =================
+        // Rows [rho RS, (rho+1) RS) are summed by CTA rho, so a warp's 32 consecutive rows go to at most two
+        // destinations as contiguous segments (scattered 16-byte remote stores cost ~6 cycles each).
+        double qp = 0.0;
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) {
+            const int i = row[s];
+            if (i >= c + 1 && i < n) {
+                cplx y = z[s];
+                if ((i & (kCl - 1)) == r) {
+                    const int slot = i >> 4;
+#pragma unroll
+                    for (int k = 0; k < kClWarps; ++k) y = y + tpart[k * ncw + slot];
+                }
+                qp += u[s].x * y.x + u[s].y * y.y;               // Re(conj(u_i) y_i): v^H A v is real
+                cplx *dst = cluster.map_shared_rank(rbuf, dest[s]);
+                dst[r * RSP + dslot[s]] = y;
+            }
+        }
+        qp = warp_sum(qp);
+        if (lane == 0) s_red[kRedQ + wp] = qp;
+        __syncthreads();
+        if (tid < kCl) {
+            double q = 0.0;
+#pragma unroll
+            for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
+            double *dst = cluster.map_shared_rank(s_q, tid);
+            dst[r] = q;
+        }
+        CLTRACE(4);
+        cl_barrier();                                             // barrier 1
+        CLTRACE(5);
+
+        // ================= [D] sum the contributions of my rows, broadcast tau y =================
+        const cplx *rawc = p.raw + (size_t)((c + 1) & 1) * lda;
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) raw[s] = (row[s] >= c + 1 && row[s] < n) ? rawc[row[s]] : mk(0.0, 0.0);
+        double q = 0.0;
+#pragma unroll
+        for (int k = 0; k < kCl; ++k) q += s_q[k];
+        const double alphap = -0.5 * abs2(tau) * q;
+        {
+            // slot t = tid / 4 (row i = r RS + t); the four threads of a slot sum four contributions each
+            const int t = tid >> 2, part = tid & 3;
+            const int i = r * RS + t;
+            const bool on = (t < RS && i >= c + 1 && i < n);      // uniform over the four threads of a slot
+            cplx y = mk(0.0, 0.0);
+            if (on) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y = y + rbuf[(4 * part + k) * RSP + t];
+            }
+            y.x += __shfl_xor_sync(0xffffffffu, y.x, 1); y.y += __shfl_xor_sync(0xffffffffu, y.y, 1);
+            y.x += __shfl_xor_sync(0xffffffffu, y.x, 2); y.y += __shfl_xor_sync(0xffffffffu, y.y, 2);
+            if (on && part == 0) ysum[t] = tau * y;
+        }
+        __syncthreads();
+        {
+            // kClThreads / 16 threads per destination CTA, contiguous rows
+            constexpr int kPer = kClThreads / kCl;
+            cplx *dst = cluster.map_shared_rank(wbuf, tid / kPer);
+            for (int t = tid % kPer; t < RS; t += kPer) {
+                const int i = r * RS + t;
+                if (i >= c + 1 && i < n) dst[i] = ysum[t];
+            }
+        }
+        CLTRACE(6);
+        cl_barrier();                                             // barrier 2
+        CLTRACE(7);
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) {
+            const int i = row[s];
+            v[s] = u[s];
+            w[s] = (i >= c + 1 && i < n) ? wbuf[i] + alphap * u[s] : mk(0.0, 0.0);
+        }
+        wc = wbuf[c + 1] + alphap * mk(1.0, 0.0);
+    }
+}
+
+// ---------------------------------------------------------------- host side
+#ifdef HPSD_PANEL_TRACE
+extern "C" int hpsd_debug_cltrace2(long long *out) {
+    return cudaMemcpyFromSymbol(out, g_cltrace2, sizeof(long long) * 8 * 16 * 4) == cudaSuccess ? 0 : -1;
+}
+extern "C" int hpsd_debug_cltrace(long long *out) {
+    return cudaMemcpyFromSymbol(out, g_cltrace, sizeof(long long) * 128 * 8) == cudaSuccess ? 0 : -1;
+}
+#endif
+int g_cluster_tridiag = 0;     // experimental until it beats the grid-wide panel kernel
+static int g_cl_init_dev = -1;
+static int g_cl_ok = 0;            // 1: 16-CTA clusters with the maximum shared memory are launchable on this device
+
+static size_t cl_smem_max(int n) {
+    size_t m = 0;
+    for (int r = 0; r < kCl; ++r) { const size_t t = cl_smem(n, r).total; if (t > m) m = t; }
+    return m;
+}
+
+int tridiag_cluster_init() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (g_cl_init_dev == dev) return 0;
+    g_cl_ok = 0;
+    int maxsm = 0;
+    cudaDeviceGetAttribute(&maxsm, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (cudaFuncSetAttribute(tridiag_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, maxsm) == cudaSuccess &&
+        cudaFuncSetAttribute(tridiag_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kCl); cfg.blockDim = dim3(kClThreads); cfg.dynamicSmemBytes = (size_t)maxsm;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kCl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, tridiag_cluster_kernel, &cfg) == cudaSuccess && nclusters >= 1) g_cl_ok = 1;
+    }
+    cudaGetLastError();            // a device without 16-CTA clusters is not an error: the grid-wide path serves it
+    g_cl_init_dev = dev;
+    return 0;
+}
+
+// 1 when a block of size n is served by the cluster kernel on this device
+int tridiag_cluster_fits(int n) {
+    tridiag_cluster_init();
+    if (!g_cl_ok || n < kCl || n > kClMaxN) return 0;
+    int dev = 0, maxsm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&maxsm, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    return cl_smem_max(n) <= (size_t)maxsm;
+}
+
+// S1 + S2 + S3 in one launch.  w.W (ldw x kNB) hosts the raw-column ring.
+int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st) {
+    ClusterArgs a;
+    a.n = w.n; a.lda = w.lda; a.in = in; a.sub = sub; a.A = w.A; a.raw = w.W; a.d = w.d; a.e = w.e; a.tau = w.tau;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(kCl); cfg.blockDim = dim3(kClThreads); cfg.dynamicSmemBytes = cl_smem_max(w.n); cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kCl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    prof_begin(ST_PANEL, st);
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, tridiag_cluster_kernel, a);
+    prof_end(ST_PANEL, st);
+    g_launches++;
+    return e == cudaSuccess ? 0 : HPSD_ECUDA_;
+}
+
+}  // namespace hpsd
