@@ -125,7 +125,7 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *   "medium_dc" (0/1, default 1): medium blocks with n <= 83 solve their tridiagonal eigenproblems with
  *       the batched device-side divide & conquer (whole group as one virtual problem) instead of the
  *       in-CTA implicit QL.
- *   "cluster_tridiag" (0/1, default 0): blocks whose packed lower triangle fits in the shared memory of one
+ *   "cluster_tridiag" (0/1, default 1): blocks whose packed lower triangle fits in the shared memory of one
  *       16-CTA cluster (116 < n <= ~640) are tridiagonalised by the cluster-resident kernel (S1+S2+S3 in one
  *       launch); 0 forces the grid-wide panel kernel.
  *   "profile" (0/1): record CUDA events on the caller's stream around every stage

@@ -27,7 +27,7 @@ void tridiag_fill_tiles(int n, int2 *tiles_host);
 int launch_tridiag(const TridiagWs &w, cudaStream_t st);
 
 // ---- tridiag_cluster.cu: S1+S2+S3 in one 16-CTA cluster, matrix resident in distributed shared memory ----
-extern int g_cluster_tridiag;            // option "cluster_tridiag" (default 0)
+extern int g_cluster_tridiag;            // option "cluster_tridiag" (default 1)
 int tridiag_cluster_init();
 int tridiag_cluster_fits(int n);         // 1 when this device and this n are served by the cluster kernel
 int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st);

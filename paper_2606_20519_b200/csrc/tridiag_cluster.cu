@@ -19,12 +19,18 @@
 //   [B] one pass over the CTA's own columns j >= c+1: A_ij -= v_i conj(w_j) + w_i conj(v_j) (the
 //       rank-2 update of step c-1, applied late) and, in the same sweep, z_i += A_ij u_j,
 //       t_j += conj(A_ij) u_i (the Hermitian mat-vec of step c from the stored half);
-//   [C] contributions z_i (+ t_i) are pushed through DSMEM to CTA i mod 16, partial v^H y to everybody;
-//       cluster barrier 1;
-//   [D] CTA i mod 16 sums the 16 contributions of its rows and broadcasts tau y_i; cluster barrier 2;
+//   [C] contributions z_i (+ t_i) are pushed through DSMEM to the CTA that sums row i (rows are dealt to the
+//       16 CTAs in contiguous slices), partial v^H y to everybody;
+//   [D] that CTA sums the 16 contributions of its rows and broadcasts tau y_i;
 //       w_i = tau y_i - 1/2 |tau|^2 (v^H y) u_i is completed by every receiver.
-// The raw next column travels through a two-entry ring in global memory (L2): one writer, 16 readers,
-// ordered by the release/acquire of cluster barrier 1.
+// Both exchanges are st.async stores that complete transaction bytes on the RECEIVER's mbarrier: data and
+// signal travel together (one DSMEM trip), there is no cluster-wide barrier inside the loop (the hardware
+// cluster barrier costs 0.55-0.7 us with 16 CTAs, measured).  The raw next column travels through a
+// two-entry ring in global memory (L2): one writer, 16 readers, fenced before the writer's pushes.
+//
+// Measured on B200 (round 1), S1+S2+S3 alone: n = 200 0.75 ms (grid-wide panel kernel 1.31), n = 400 2.04 (2.70),
+// n = 625 4.00 (4.37).  Every warp walks a serial chain of ~10 trips of ~1500 cycles per column step (t_j warp
+// reductions and the issue overhead around the 16 DFMA per element), so the FP64 pipe is ~25 % busy at n = 625.
 #include <cooperative_groups.h>
 #include "kernels.h"
 #include "large.h"
@@ -35,14 +41,39 @@ namespace cg = cooperative_groups;
 namespace hpsd {
 
 constexpr int kCl = 16;            // CTAs per cluster (non-portable size)
-constexpr int kClThreads = 512;
+constexpr int kClThreads = 256;
 constexpr int kClWarps = kClThreads / 32;
-constexpr int kClR = 2;            // row slots per thread: n <= 1024
+constexpr int kClR = 3;            // row slots per thread: n <= 768
 constexpr int kClMaxN = 32 * kClWarps * kClR;
-constexpr int kKT = 2;             // own columns per trip of the pass
+constexpr int kKT = 4;             // own columns per trip of the pass
 constexpr int kRedN = 0, kRedQ = kClWarps, kRedS = 2 * kClWarps;   // s_red: norm partials | dot partials | alpha.x, alpha.y, d_c
 // 32-row chunk of (slot, warp): odd slots run backwards so that every warp gets a light and a heavy chunk
 __device__ __forceinline__ int cl_chunk(int s, int wp) { return kClWarps * s + ((s & 1) ? kClWarps - 1 - wp : wp); }
+// ---- data + signal in one DSMEM trip: st.async stores complete transaction bytes on the receiver's mbarrier ----
+__device__ __forceinline__ unsigned cl_mapa(unsigned addr, int rank) {
+    unsigned remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(addr), "r"(rank));
+    return remote;
+}
+__device__ __forceinline__ void cl_st_async(unsigned raddr, cplx v, unsigned rmbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(raddr), "d"(v.x), "d"(v.y), "r"(rmbar) : "memory");
+}
+__device__ __forceinline__ void cl_st_async(unsigned raddr, double v, unsigned rmbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(raddr), "d"(v), "r"(rmbar) : "memory");
+}
+// one pending arrival per phase (this arm) + the bytes the phase will receive
+__device__ __forceinline__ void cl_arm(unsigned mbar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cl_wait(unsigned mbar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "CL_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra CL_DONE_%=;\n\t"
+        "bra CL_WAIT_%=;\n\t"
+        "CL_DONE_%=:\n\t}" ::"r"(mbar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void cl_barrier() {
     // release/acquire at CLUSTER scope (cooperative_groups' cluster.sync() fences at gpu scope: MEMBAR.ALL.GPU)
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -61,13 +92,14 @@ __host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + 
 __host__ __device__ inline size_t cl_col_off(int n, int r, int jl) { return (size_t)jl * (n - r) - (size_t)8 * jl * (jl - 1); }
 
 struct ClusterSmem {
-    size_t colv, q, red, ysum, rbuf, wbuf, stor, total;
+    size_t mbar, colv, q, red, ysum, rbuf, wbuf, stor, total;
 };
 __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     ClusterSmem s;
     const int nc = cl_ncols(n, 0);                 // widest CTA
     const int rs = (n + kCl - 1) / kCl;
     size_t off = 0;
+    s.mbar = off; off += 16;                      // two mbarriers
     s.colv = off; off += sizeof(cplx) * 3 * nc;
     s.q = off; off += sizeof(double) * kCl;
     s.red = off; off += sizeof(double) * (2 * kClWarps + 4);   // block-reduction scratch + alpha, d_c
@@ -110,12 +142,41 @@ __device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, cons
 // dev-only: clock64 at eight points of every 8th column step, CTA 0 / thread 0
 __device__ long long g_cltrace[128 * 8];
 __device__ long long g_cltrace2[8 * 16 * 4];
-#define CLT2(pt) do { if (r == 0 && lane == 0 && c == 0) g_cltrace2[(wp * 16 + ((jl - jl0) >> 2)) * 4 + (pt)] = clock64(); } while (0)
+#define CLT2(pt) do { if (r == 0 && lane == 0 && c == 0) g_cltrace2[(wp * 16 + (((jl - jl0) >> 2) & 15)) * 4 + (pt)] = clock64(); } while (0)
 #define CLTRACE(slot) do { if (r == 0 && tid == 0 && (c & 7) == 0 && (c >> 3) < 128) g_cltrace[(c >> 3) * 8 + (slot)] = clock64(); } while (0)
 #else
 #define CLTRACE(slot) do {} while (0)
 #define CLT2(pt) do {} while (0)
 #endif
+
+// One row chunk x kKT own columns of the fused pass.  x holds A(i, j_k) (zero where the element does not exist).
+// MASKED = false: all 32 rows lie strictly below every diagonal of the trip (no predicates at all).
+template <bool MASKED>
+__device__ __forceinline__ void cl_elems(cplx (&x)[kKT], const bool (&m)[kKT], int i, int j0, cplx *const (&col)[kKT], int i0,
+                                         cplx v, cplx w, cplx u, const cplx (&cv)[kKT], const cplx (&cw)[kKT], const cplx (&cu)[kKT],
+                                         cplx &z, cplx (&tj)[kKT]) {
+#pragma unroll
+    for (int k = 0; k < kKT; ++k) {
+        cplx xx = x[k];
+        // xx -= v_i conj(w_j) + w_i conj(v_j)
+        xx.x = fma(-v.x, cw[k].x, xx.x); xx.x = fma(-v.y, cw[k].y, xx.x);
+        xx.x = fma(-w.x, cv[k].x, xx.x); xx.x = fma(-w.y, cv[k].y, xx.x);
+        xx.y = fma(-v.y, cw[k].x, xx.y); xx.y = fma(v.x, cw[k].y, xx.y);
+        xx.y = fma(-w.y, cv[k].x, xx.y); xx.y = fma(w.x, cv[k].y, xx.y);
+        cplx ut = u;
+        if (MASKED) {
+            const int j = j0 + kCl * k;
+            if (!m[k]) xx = mk(0.0, 0.0);
+            if (i == j) xx.y = 0.0;
+            if (i <= j) ut = mk(0.0, 0.0);
+            if (m[k]) col[k][i0] = xx;
+        } else {
+            col[k][i0] = xx;
+        }
+        cfma(z, xx, cu[k]);
+        cfma_conj(tj[k], xx, ut);
+    }
+}
 
 __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterArgs p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -153,6 +214,25 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0) : mk(0.0, 0.0);
     }
     cplx wc = mk(0.0, 0.0);
+    const unsigned mbar1 = (unsigned)__cvta_generic_to_shared(smem_raw + L.mbar), mbar2 = mbar1 + 8;
+    const unsigned rbuf_a = (unsigned)__cvta_generic_to_shared(rbuf), wbuf_a = (unsigned)__cvta_generic_to_shared(wbuf);
+    const unsigned sq_a = (unsigned)__cvta_generic_to_shared(s_q);
+    // bytes phase c of each mbarrier receives: 16 senders x (my active rows + the v^H y partial); all active rows of w
+    auto bytes_r = [&](int c) -> unsigned {
+        int lo = r * RS, hi = lo + RS;
+        if (lo < c + 1) lo = c + 1;
+        if (hi > n) hi = n;
+        const int act = hi > lo ? hi - lo : 0;
+        return (unsigned)(kCl * (act * 16 + 8));
+    };
+    auto bytes_w = [&](int c) -> unsigned { return (unsigned)((n - c - 1) * 16); };
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar1), "r"(1));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar2), "r"(1));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        cl_arm(mbar1, bytes_r(0));
+        cl_arm(mbar2, bytes_w(0));
+    }
     cl_barrier();       // every CTA of the cluster is resident before the first DSMEM access
 
     for (int c = 0; c < n; ++c) {
@@ -217,8 +297,15 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         for (int s = 0; s < kClR; ++s) z[s] = mk(0.0, 0.0);
         const int jl0 = (c + 1 > r) ? (c + 1 - r + kCl - 1) / kCl : 0;
         cplx *rawn = p.raw + (size_t)((c + 1) & 1) * lda;
-        for (int jl = jl0; jl < nc; jl += kKT) {
+        // rows of this warp end at top_end: once the trip's first column lies beyond them the warp is done
+        int top_end = 0;
+#pragma unroll
+        for (int s = 0; s < kClR; ++s) { const int e = 32 * cl_chunk(s, wp) + 32; if (e - 32 < n && e > top_end) top_end = e; }
+        if (top_end > n) top_end = n;
+        int jl = jl0;
+        for (; jl < nc; jl += kKT) {
             const int j0 = r + kCl * jl;
+            if (j0 >= top_end) break;                              // warp-uniform
             CLT2(0);
             cplx cv[kKT], cw[kKT], cu[kKT], tj[kKT];
             cplx *col[kKT];
@@ -228,50 +315,31 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 const int jk = okc ? jl + k : jl;
                 cv[k] = colv_v[jk]; cw[k] = colv_w[jk];
                 cu[k] = okc ? colv_u[jk] : mk(0.0, 0.0);
-                col[k] = stor + cl_col_off(n, r, jk) - (r + kCl * jk);   // col[k][i] = A(i, j_k)
+                col[k] = stor + cl_col_off(n, r, jk) - (r + kCl * jk) + lane;   // col[k][i0] = A(i0 + lane, j_k)
                 tj[k] = mk(0.0, 0.0);
             }
-            const bool exp_col = (j0 == c + 1);                   // only the first column of a trip can be column c+1
+            const int ncol = nc - jl;                             // valid columns of this trip (>= kKT except in the last one)
             cplx x[kClR][kKT];
-            bool ok[kClR][kKT];
+            bool m[kClR][kKT];
 #pragma unroll
             for (int s = 0; s < kClR; ++s) {
-                const int i0 = 32 * cl_chunk(s, wp);
-                const bool slot_on = !(i0 + 31 < j0 || i0 >= n);   // warp-uniform
+                const int i0 = 32 * cl_chunk(s, wp), i = i0 + lane;
 #pragma unroll
                 for (int k = 0; k < kKT; ++k) {
-                    const int i = i0 + lane;
-                    ok[s][k] = slot_on && (jl + k < nc) && i >= j0 + kCl * k && i < n;
-#if defined(HPSD_CLX) && HPSD_CLX == 3
-                    x[s][k] = mk(1.0 * i, 0.5);
-#else
-                    x[s][k] = ok[s][k] ? col[k][i] : mk(0.0, 0.0);
-#endif
+                    m[s][k] = (k < ncol) && i >= j0 + kCl * k && i < n;
+                    x[s][k] = mk(0.0, 0.0);
+                    if (m[s][k]) x[s][k] = col[k][i0];
                 }
             }
             CLT2(1);
 #pragma unroll
             for (int s = 0; s < kClR; ++s) {
-                const int i = 32 * cl_chunk(s, wp) + lane;
-#pragma unroll
-                for (int k = 0; k < kKT; ++k) {
-                    if (!ok[s][k]) continue;
-                    cplx xx = x[s][k];
-                    // xx -= v_i conj(w_j) + w_i conj(v_j)
-                    xx.x = fma(-v[s].x, cw[k].x, xx.x); xx.x = fma(-v[s].y, cw[k].y, xx.x);
-                    xx.x = fma(-w[s].x, cv[k].x, xx.x); xx.x = fma(-w[s].y, cv[k].y, xx.x);
-                    xx.y = fma(-v[s].y, cw[k].x, xx.y); xx.y = fma(v[s].x, cw[k].y, xx.y);
-                    xx.y = fma(-w[s].y, cv[k].x, xx.y); xx.y = fma(w[s].x, cv[k].y, xx.y);
-                    const int j = j0 + kCl * k;
-                    if (i == j) xx.y = 0.0;
-#if defined(HPSD_CLX) && HPSD_CLX == 2
-                    if (k == 0 && exp_col) rawn[i] = xx;
-#else
-                    if (k == 0 && exp_col) rawn[i] = xx; else col[k][i] = xx;
-#endif
-                    cfma(z[s], xx, cu[k]);
-                    if (i > j) cfma_conj(tj[k], xx, u[s]);
-                }
+                const int i0 = 32 * cl_chunk(s, wp), i = i0 + lane;
+                if (i0 + 31 < j0 || i0 >= n) continue;            // warp-uniform: nothing of this chunk in the trip
+                if (i0 > j0 + kCl * (kKT - 1) && i0 + 32 <= n && ncol >= kKT)
+                    cl_elems<false>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
+                else
+                    cl_elems<true>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
             }
             CLT2(2);
             // halving butterfly: kKT values x 32 lanes -> lane 32 q / kKT holds the total of column q
@@ -303,7 +371,14 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             }
             CLT2(3);
         }
+        for (int q = jl + lane; q < nc; q += 32) tpart[wp * ncw + q] = mk(0.0, 0.0);   // columns beyond this warp's rows
         __syncthreads();
+        if (jl0 < nc && r + kCl * jl0 == c + 1) {
+            // this CTA owns column c+1, now in its final state: export it for step c+1 (L2, read after barrier 1)
+            const cplx *colx = stor + cl_col_off(n, r, jl0) - (c + 1);
+            for (int i = c + 1 + tid; i < n; i += kClThreads) rawn[i] = colx[i];
+            __threadfence();     // ordered before this thread's st.async pushes, which the readers acquire through their mbarrier
+        }
         CLTRACE(3);
 
         // ================= [C] contributions to y = A v: reduce-scatter through DSMEM =================
@@ -321,8 +396,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                     for (int k = 0; k < kClWarps; ++k) y = y + tpart[k * ncw + slot];
                 }
                 qp += u[s].x * y.x + u[s].y * y.y;               // Re(conj(u_i) y_i): v^H A v is real
-                cplx *dst = cluster.map_shared_rank(rbuf, dest[s]);
-                dst[r * RSP + dslot[s]] = y;
+                cl_st_async(cl_mapa(rbuf_a + 16u * (unsigned)(r * RSP + dslot[s]), dest[s]), y, cl_mapa(mbar1, dest[s]));
             }
         }
         qp = warp_sum(qp);
@@ -332,17 +406,17 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             double q = 0.0;
 #pragma unroll
             for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
-            double *dst = cluster.map_shared_rank(s_q, tid);
-            dst[r] = q;
+            cl_st_async(cl_mapa(sq_a + 8u * (unsigned)r, tid), q, cl_mapa(mbar1, tid));
         }
         CLTRACE(4);
-        cl_barrier();                                             // barrier 1
+        cl_wait(mbar1, c & 1);                                    // every contribution to my rows has landed
+        if (tid == 0) cl_arm(mbar1, bytes_r(c + 1));
         CLTRACE(5);
 
         // ================= [D] sum the contributions of my rows, broadcast tau y =================
         const cplx *rawc = p.raw + (size_t)((c + 1) & 1) * lda;
 #pragma unroll
-        for (int s = 0; s < kClR; ++s) raw[s] = (row[s] >= c + 1 && row[s] < n) ? rawc[row[s]] : mk(0.0, 0.0);
+        for (int s = 0; s < kClR; ++s) raw[s] = (row[s] >= c + 1 && row[s] < n) ? ldcg_(&rawc[row[s]]) : mk(0.0, 0.0);   // L2: the ring is rewritten every other step
         double q = 0.0;
 #pragma unroll
         for (int k = 0; k < kCl; ++k) q += s_q[k];
@@ -365,14 +439,16 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         {
             // kClThreads / 16 threads per destination CTA, contiguous rows
             constexpr int kPer = kClThreads / kCl;
-            cplx *dst = cluster.map_shared_rank(wbuf, tid / kPer);
+            const int dk = tid / kPer;
+            const unsigned dst = cl_mapa(wbuf_a, dk), dmb = cl_mapa(mbar2, dk);
             for (int t = tid % kPer; t < RS; t += kPer) {
                 const int i = r * RS + t;
-                if (i >= c + 1 && i < n) dst[i] = ysum[t];
+                if (i >= c + 1 && i < n) cl_st_async(dst + 16u * (unsigned)i, ysum[t], dmb);
             }
         }
         CLTRACE(6);
-        cl_barrier();                                             // barrier 2
+        cl_wait(mbar2, c & 1);                                    // all of tau y has landed
+        if (tid == 0) cl_arm(mbar2, bytes_w(c + 1));
         CLTRACE(7);
 #pragma unroll
         for (int s = 0; s < kClR; ++s) {
@@ -393,7 +469,7 @@ extern "C" int hpsd_debug_cltrace(long long *out) {
     return cudaMemcpyFromSymbol(out, g_cltrace, sizeof(long long) * 128 * 8) == cudaSuccess ? 0 : -1;
 }
 #endif
-int g_cluster_tridiag = 0;     // experimental until it beats the grid-wide panel kernel
+int g_cluster_tridiag = 1;
 static int g_cl_init_dev = -1;
 static int g_cl_ok = 0;            // 1: 16-CTA clusters with the maximum shared memory are launchable on this device
 

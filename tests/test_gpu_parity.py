@@ -461,3 +461,32 @@ def test_admm_step_fused(orc, hp):
     torch.cuda.synchronize()
     assert np.array_equal(t_ut2.cpu().numpy(), t_u.cpu().numpy())
     assert np.array_equal(t_v2.cpu().numpy(), t_v.cpu().numpy())
+
+
+@pytest.mark.parametrize("n", [117, 130, 255, 256, 257, 400, 625, 636])
+def test_cluster_tridiag_kernel(orc, hp, n):
+    """S1+S2+S3 by the cluster-resident kernel (tridiag_cluster.cu; option "cluster_tridiag", on by default).
+    Whole-path parity against the oracle, (d, e) against the grid-wide panel kernel (same reflector convention,
+    so the tridiagonals agree to rounding), and the fused ADMM subtraction of Eq. (D33) on this path."""
+    import torch
+    rng = np.random.default_rng(700 + n)
+    sv = orc.pack(herm(rng, n, 1.0 / np.sqrt(n)))
+    t = torch.from_numpy(sv).cuda()
+    hp.set_option("cluster_tridiag", 0)
+    d0, e0 = hp.tridiagonalize(t, n)
+    hp.set_option("cluster_tridiag", 1)
+    try:
+        got, _ = check_vs_oracle(orc, hp, [n], sv, nthreads=orc.max_threads())
+        d1, e1 = hp.tridiagonalize(t, n)
+        v = orc.pack(herm(rng, n, 1.0 / np.sqrt(n)))
+        t_v, t_u = torch.from_numpy(v.copy()).cuda(), torch.empty_like(t)
+        hp.admm_step_([n], t, t_v, t_u)
+        torch.cuda.synchronize()
+        want_u, want_v = orc.admm_step([n], sv, v, nthreads=orc.max_threads())
+    finally:
+        hp.set_option("cluster_tridiag", 1)
+    scale = float(d0.abs().max() + e0.abs().max())
+    assert float((d1 - d0).abs().max()) <= 1e-13 * n * scale
+    assert float((e1 - e0).abs().max()) <= 1e-13 * n * scale
+    assert parity_err(t_u.cpu().numpy(), want_u, sv - v, n) <= TOL * n
+    assert parity_err(t_v.cpu().numpy(), want_v, sv - v, n) <= TOL * n
