@@ -44,12 +44,13 @@ def f_alg(n: int, kpos: int) -> float:
 
 
 # stage -> the part of f_alg that stage carries (flops), used for the dominant-kernel roofline
-def stage_flops(stage: str, sizes, kpos, jmax: int) -> float:
+def stage_flops(stage: str, sizes, kpos, jmax: int, cluster: bool = False) -> float:
     tot = 0.0
     for n, k in zip(sizes, kpos):
         large = n > jmax
         if stage == "S2S3_tridiag_panel" and large:
-            tot += (8.0 / 3.0) * n ** 3          # the mat-vec half of the reduction
+            # the mat-vec half of the reduction; the cluster-resident kernel (tridiag_cluster.cu) does both halves
+            tot += ((16.0 if cluster else 8.0) / 3.0) * n ** 3
         elif stage == "S2_her2k_trailing" and large:
             tot += (8.0 / 3.0) * n ** 3          # the rank-2k half
         elif stage == "S4_stedc" and large:
@@ -81,6 +82,7 @@ def measured_hbm_gbs():
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu
 # --set full captures (profiles/r1_tuned_ncu_full.md); None where no capture exists for that workload
 NCU_TRAFFIC = {
+    ("S1S2S3_tridiag_cluster", 3): {"bytes_per_launch": 3.18e6, "source": "profiles/r1_cluster_ncu_full.md (n=625, whole reduction in one launch)"},
     ("S2S3_tridiag_panel", 3): {"bytes_per_launch": 2.82e6, "source": "profiles/r1_tuned_ncu_full.md (first panel, n=625)"},
     ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.24e9, "source": "profiles/r1_tuned_ncu_full.md (first panels, n=4096)"},
     ("S10_householder_ql", 2): {"bytes_per_launch": 1.35e7, "source": "profiles/r1_tuned_ncu_full.md (256 x n=81)"},
@@ -329,12 +331,25 @@ def main():
     dom = max(stages, key=lambda k: stages[k]["ms_per_step"])
     dom_ms = stages[dom]["ms_per_step"]
     dom_spans = max(stages[dom]["launch_spans_per_step"], 1)
-    dom_flops = stage_flops(dom, sizes, kpos, jmax)
+    # the cluster-resident kernel (116 < n <= ~640) leaves no HER2K spans: S1+S2+S3 are one launch
+    cluster = dom == "S2S3_tridiag_panel" and "S2_her2k_trailing" not in stages and "S1_unpack" not in stages
+    dom_flops = stage_flops(dom, sizes, kpos, jmax, cluster)
     F = sum(f_alg(n, k) for n, k in zip(sizes, kpos))
     hbm_peak, hbm_src = measured_hbm_gbs()
     fp64_src = (f"measured in this run by hpsd_fp64_peak_probe: DFMA {peak_dfma:.1f}, DMMA {peak_dmma:.1f} TFLOP/s "
                 "(MEASURED_PEAKS.json has no FP64 figure)")
-    if dom in ("S2S3_tridiag_panel", "S1_unpack"):
+    if cluster:
+        # matrix resident in the shared memory of one 16-CTA cluster: HBM sees the svec once (8 n^2 bytes) and the
+        # reflectors once (~8 n^2 bytes); the bound is FP64 FMA issue (unblocked rank-2 update + mat-vec, DFMA)
+        achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+        roofline = {"kernel": "S1S2S3_tridiag_cluster", "bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s",
+                    "frac": achieved / peak_dfma if peak_dfma else None,
+                    "traffic": (NCU_TRAFFIC.get(("S1S2S3_tridiag_cluster", cfg)) or {}).get("bytes_per_launch"),
+                    "traffic_source": (NCU_TRAFFIC.get(("S1S2S3_tridiag_cluster", cfg)) or {}).get("source"),
+                    "peak_source": fp64_src + "; DFMA figure, whole chip", "algorithmic_flops_per_step": dom_flops,
+                    "algorithmic_bytes_per_step": sum(16.0 * n * n for n in sizes if n > jmax),
+                    "sms_used": 16, "frac_of_16_sm_dfma_peak": achieved / (peak_dfma * 16.0 / 148.0) if peak_dfma else None}
+    elif dom in ("S2S3_tridiag_panel", "S1_unpack"):
         # memory-bound stages: the one-stage reduction streams the stored lower triangle of the trailing
         # matrix through the SMs once per column; unpack reads 8n^2 and writes 8n^2 bytes
         if dom == "S1_unpack":
