@@ -20,16 +20,18 @@
 //       rank-2 update of step c-1, applied late) and, in the same sweep, z_i += A_ij u_j,
 //       t_j += conj(A_ij) u_i (the Hermitian mat-vec of step c from the stored half);
 //   [C] contributions z_i (+ t_i) are pushed through DSMEM to the CTA that sums row i (rows are dealt to the
-//       16 CTAs in contiguous slices), partial v^H y to everybody;
+//       16 CTAs in contiguous slices); the partial v^H y goes to everybody with phase 2 (needed only with w);
 //   [D] that CTA sums the 16 contributions of its rows and broadcasts tau y_i;
 //       w_i = tau y_i - 1/2 |tau|^2 (v^H y) u_i is completed by every receiver.
 // Both exchanges are st.async stores that complete transaction bytes on the RECEIVER's mbarrier: data and
 // signal travel together (one DSMEM trip), there is no cluster-wide barrier inside the loop (the hardware
 // cluster barrier costs 0.55-0.7 us with 16 CTAs, measured).  The raw next column travels through a
-// two-entry ring in global memory (L2): one writer, 16 readers, fenced before the writer's pushes.
+// two-entry ring in global memory (L2): the CTA that stores column c+1 brings it up to date and exports it BEFORE
+// its pass, fences after the pass and sends one 8-byte token per warp to every CTA on the phase-1 mbarrier, so
+// nobody reads the ring before the export is visible and the fence is off the critical path.
 //
-// Measured on B200 (round 1), S1+S2+S3 alone: n = 200 0.75 ms (grid-wide panel kernel 1.31), n = 400 2.04 (2.70),
-// n = 625 4.00 (4.37).  Every warp walks a serial chain of ~10 trips of ~1500 cycles per column step (t_j warp
+// Measured on B200 (round 1), S1+S2+S3 alone: n = 200 0.70 ms (grid-wide panel kernel 1.31), n = 400 1.97 (2.70),
+// n = 625 3.93 (4.37).  Every warp walks a serial chain of ~10 trips of ~1500 cycles per column step (t_j warp
 // reductions and the issue overhead around the 16 DFMA per element), so the FP64 pipe is ~25 % busy at n = 625.
 #include <cooperative_groups.h>
 #include "kernels.h"
@@ -92,7 +94,7 @@ __host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + 
 __host__ __device__ inline size_t cl_col_off(int n, int r, int jl) { return (size_t)jl * (n - r) - (size_t)8 * jl * (jl - 1); }
 
 struct ClusterSmem {
-    size_t mbar, colv, q, red, ysum, rbuf, wbuf, stor, total;
+    size_t mbar, tok, colv, q, red, rbuf, wbuf, stor, total;
 };
 __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     ClusterSmem s;
@@ -100,10 +102,10 @@ __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     const int rs = (n + kCl - 1) / kCl;
     size_t off = 0;
     s.mbar = off; off += 16;                      // two mbarriers
+    s.tok = off; off += 8 * kClWarps;             // landing slots of the export tokens
     s.colv = off; off += sizeof(cplx) * 3 * nc;
-    s.q = off; off += sizeof(double) * kCl;
+    s.q = off; off += sizeof(double) * 2 * kCl;    // v^H y partials, double-buffered by step parity
     s.red = off; off += sizeof(double) * (2 * kClWarps + 4);   // block-reduction scratch + alpha, d_c
-    s.ysum = off; off += sizeof(cplx) * rs;        // tau y of the rows this CTA reduces
     s.rbuf = off; off += sizeof(cplx) * kCl * (rs | 1);
     s.wbuf = off;
     const size_t wb = sizeof(cplx) * n, tp = sizeof(cplx) * kClWarps * nc;
@@ -190,7 +192,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
     cplx *colv_w = colv_v + ncw, *colv_u = colv_w + ncw;
     double *s_q = reinterpret_cast<double *>(smem_raw + L.q);
     double *s_red = reinterpret_cast<double *>(smem_raw + L.red);   // kRedN.. norm, kRedQ.. dot, kRedS.. alpha, d_c
-    cplx *ysum = reinterpret_cast<cplx *>(smem_raw + L.ysum);
     cplx *rbuf = reinterpret_cast<cplx *>(smem_raw + L.rbuf);                 // [sender][RSP]
     const int RS = (n + kCl - 1) / kCl, RSP = RS | 1;
     cplx *wbuf = reinterpret_cast<cplx *>(smem_raw + L.wbuf);
@@ -216,16 +217,16 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
     cplx wc = mk(0.0, 0.0);
     const unsigned mbar1 = (unsigned)__cvta_generic_to_shared(smem_raw + L.mbar), mbar2 = mbar1 + 8;
     const unsigned rbuf_a = (unsigned)__cvta_generic_to_shared(rbuf), wbuf_a = (unsigned)__cvta_generic_to_shared(wbuf);
-    const unsigned sq_a = (unsigned)__cvta_generic_to_shared(s_q);
+    const unsigned sq_a = (unsigned)__cvta_generic_to_shared(s_q), tok_a = (unsigned)__cvta_generic_to_shared(smem_raw + L.tok);
     // bytes phase c of each mbarrier receives: 16 senders x (my active rows + the v^H y partial); all active rows of w
     auto bytes_r = [&](int c) -> unsigned {
         int lo = r * RS, hi = lo + RS;
         if (lo < c + 1) lo = c + 1;
         if (hi > n) hi = n;
         const int act = hi > lo ? hi - lo : 0;
-        return (unsigned)(kCl * (act * 16 + 8));
+        return (unsigned)(kCl * act * 16 + kClWarps * 8);        // + the export tokens of the owner of column c+1
     };
-    auto bytes_w = [&](int c) -> unsigned { return (unsigned)((n - c - 1) * 16); };
+    auto bytes_w = [&](int c) -> unsigned { return (unsigned)((n - c - 1) * 16 + kCl * 8); };
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar1), "r"(1));
         asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar2), "r"(1));
@@ -297,6 +298,27 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         for (int s = 0; s < kClR; ++s) z[s] = mk(0.0, 0.0);
         const int jl0 = (c + 1 > r) ? (c + 1 - r + kCl - 1) / kCl : 0;
         cplx *rawn = p.raw + (size_t)((c + 1) & 1) * lda;
+        const bool owner = (jl0 < nc && r + kCl * jl0 == c + 1);  // this CTA stores column c+1
+        if (owner) {
+            // bring column c+1 to its final state first and export it for step c+1 (L2); every thread updates the
+            // rows it also handles in the pass, so no synchronisation is needed; the pass then skips its update
+            const cplx cvo = colv_v[jl0], cwo = colv_w[jl0];
+            cplx *colx = stor + cl_col_off(n, r, jl0) - (c + 1);
+#pragma unroll
+            for (int s = 0; s < kClR; ++s) {
+                const int i = row[s];
+                if (i >= c + 1 && i < n) {
+                    cplx x = colx[i];
+                    x.x = fma(-v[s].x, cwo.x, x.x); x.x = fma(-v[s].y, cwo.y, x.x);
+                    x.x = fma(-w[s].x, cvo.x, x.x); x.x = fma(-w[s].y, cvo.y, x.x);
+                    x.y = fma(-v[s].y, cwo.x, x.y); x.y = fma(v[s].x, cwo.y, x.y);
+                    x.y = fma(-w[s].y, cvo.x, x.y); x.y = fma(w[s].x, cvo.y, x.y);
+                    if (i == c + 1) x.y = 0.0;
+                    colx[i] = x;
+                    rawn[i] = x;
+                }
+            }
+        }
         // rows of this warp end at top_end: once the trip's first column lies beyond them the warp is done
         int top_end = 0;
 #pragma unroll
@@ -314,6 +336,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 const bool okc = jl + k < nc;
                 const int jk = okc ? jl + k : jl;
                 cv[k] = colv_v[jk]; cw[k] = colv_w[jk];
+                if (owner && jk == jl0) cv[k] = cw[k] = mk(0.0, 0.0);           // column c+1 is already up to date
                 cu[k] = okc ? colv_u[jk] : mk(0.0, 0.0);
                 col[k] = stor + cl_col_off(n, r, jk) - (r + kCl * jk) + lane;   // col[k][i0] = A(i0 + lane, j_k)
                 tj[k] = mk(0.0, 0.0);
@@ -372,13 +395,14 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             CLT2(3);
         }
         for (int q = jl + lane; q < nc; q += 32) tpart[wp * ncw + q] = mk(0.0, 0.0);   // columns beyond this warp's rows
-        __syncthreads();
-        if (jl0 < nc && r + kCl * jl0 == c + 1) {
-            // this CTA owns column c+1, now in its final state: export it for step c+1 (L2, read after barrier 1)
-            const cplx *colx = stor + cl_col_off(n, r, jl0) - (c + 1);
-            for (int i = c + 1 + tid; i < n; i += kClThreads) rawn[i] = colx[i];
-            __threadfence();     // ordered before this thread's st.async pushes, which the readers acquire through their mbarrier
+        if (owner) {
+            // the export stores were issued before the pass: the fence is cheap by now.  One token per warp and
+            // receiver on phase 1: nobody reads the ring before every exporting warp has fenced.
+            __threadfence();
+            __syncwarp();
+            if (lane < kCl) cl_st_async(cl_mapa(tok_a + 8u * (unsigned)wp, lane), 1.0, cl_mapa(mbar1, lane));
         }
+        __syncthreads();
         CLTRACE(3);
 
         // ================= [C] contributions to y = A v: reduce-scatter through DSMEM =================
@@ -406,7 +430,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             double q = 0.0;
 #pragma unroll
             for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
-            cl_st_async(cl_mapa(sq_a + 8u * (unsigned)r, tid), q, cl_mapa(mbar1, tid));
+            cl_st_async(cl_mapa(sq_a + 8u * (unsigned)((c & 1) * kCl + r), tid), q, cl_mapa(mbar2, tid));   // needed only with w: phase 2
         }
         CLTRACE(4);
         cl_wait(mbar1, c & 1);                                    // every contribution to my rows has landed
@@ -417,12 +441,9 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         const cplx *rawc = p.raw + (size_t)((c + 1) & 1) * lda;
 #pragma unroll
         for (int s = 0; s < kClR; ++s) raw[s] = (row[s] >= c + 1 && row[s] < n) ? ldcg_(&rawc[row[s]]) : mk(0.0, 0.0);   // L2: the ring is rewritten every other step
-        double q = 0.0;
-#pragma unroll
-        for (int k = 0; k < kCl; ++k) q += s_q[k];
-        const double alphap = -0.5 * abs2(tau) * q;
         {
-            // slot t = tid / 4 (row i = r RS + t); the four threads of a slot sum four contributions each
+            // slot t = tid / 4 (row i = r RS + t); the four threads of a slot sum four contributions each and
+            // send tau y_i to four of the 16 CTAs each
             const int t = tid >> 2, part = tid & 3;
             const int i = r * RS + t;
             const bool on = (t < RS && i >= c + 1 && i < n);      // uniform over the four threads of a slot
@@ -433,21 +454,18 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             }
             y.x += __shfl_xor_sync(0xffffffffu, y.x, 1); y.y += __shfl_xor_sync(0xffffffffu, y.y, 1);
             y.x += __shfl_xor_sync(0xffffffffu, y.x, 2); y.y += __shfl_xor_sync(0xffffffffu, y.y, 2);
-            if (on && part == 0) ysum[t] = tau * y;
-        }
-        __syncthreads();
-        {
-            // kClThreads / 16 threads per destination CTA, contiguous rows
-            constexpr int kPer = kClThreads / kCl;
-            const int dk = tid / kPer;
-            const unsigned dst = cl_mapa(wbuf_a, dk), dmb = cl_mapa(mbar2, dk);
-            for (int t = tid % kPer; t < RS; t += kPer) {
-                const int i = r * RS + t;
-                if (i >= c + 1 && i < n) cl_st_async(dst + 16u * (unsigned)i, ysum[t], dmb);
+            if (on) {
+                const cplx ty = tau * y;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) cl_st_async(cl_mapa(wbuf_a + 16u * (unsigned)i, 4 * part + k), ty, cl_mapa(mbar2, 4 * part + k));
             }
         }
         CLTRACE(6);
         cl_wait(mbar2, c & 1);                                    // all of tau y has landed
+        double q = 0.0;
+#pragma unroll
+        for (int k = 0; k < kCl; ++k) q += s_q[(c & 1) * kCl + k];
+        const double alphap = -0.5 * abs2(tau) * q;
         if (tid == 0) cl_arm(mbar2, bytes_w(c + 1));
         CLTRACE(7);
 #pragma unroll
