@@ -128,6 +128,9 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *   "cluster_tridiag" (0/1, default 1): blocks whose packed lower triangle fits in the shared memory of one
  *       16-CTA cluster (116 < n <= ~640) are tridiagonalised by the cluster-resident kernel (S1+S2+S3 in one
  *       launch); 0 forces the grid-wide panel kernel.
+ *   "overlap_factors" (0/1, default 1): the compact-WY factors of the back-transform (they depend on the
+ *       reflectors only) run on an internal side stream next to the divide & conquer; fork and join are events
+ *       on the caller's stream, so the call stays asynchronous and capturable.
  *   "profile" (0/1): record CUDA events on the caller's stream around every stage
  *       of the path (S1..S10) for hpsd_profile_read.  Off by default. */
 int hpsd_set_option(const char *name, int value);

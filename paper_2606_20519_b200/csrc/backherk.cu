@@ -206,7 +206,24 @@ int backherk_init() {
     return 0;
 }
 
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st) {
+// Compact-WY factors of all reflector blocks (Gram matrices, T_b, V_b T_b): they depend on the reflectors only,
+// so the large path runs them on a side stream next to the divide & conquer (S4).
+int launch_bt_factors(const BackWs &w, cudaStream_t st) {
+    const int n = w.n;
+    int rc = backherk_init();
+    if (rc) return rc;
+    const int nblocks = (n + kNBT - 1) / kNBT;
+    const int nt = (n + 63) / 64;
+    bt_gram_kernel<<<dim3(kSplitK, 1, nblocks), BG_THREADS, kSmemKK, st>>>(w);
+    HPSD_LAUNCH_CHECK();
+    bt_tfactor_kernel<<<nblocks, kNBT, sizeof(cplx) * kNBT * kNBT, st>>>(w);
+    HPSD_LAUNCH_CHECK();
+    bt_vt_kernel<<<dim3(nt, 1, nblocks), BG_THREADS, kSmemMK, st>>>(w);
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done) {
     const int n = w.n;
     int rc = backherk_init();
     if (rc) return rc;
@@ -218,13 +235,10 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     HPSD_LAUNCH_CHECK();
     scale_convert_kernel<<<dim3((n + 1023) / 1024, n), 256, 0, st>>>(n, lam, Zt, ldzt, w.Zc, w.ldz, w.cnt);
     HPSD_LAUNCH_CHECK();
-    // compact-WY factors of all blocks (off the dependent chain: batched over blocks)
-    bt_gram_kernel<<<dim3(kSplitK, 1, nblocks), BG_THREADS, kSmemKK, st>>>(w);
-    HPSD_LAUNCH_CHECK();
-    bt_tfactor_kernel<<<nblocks, kNBT, sizeof(cplx) * kNBT * kNBT, st>>>(w);
-    HPSD_LAUNCH_CHECK();
-    bt_vt_kernel<<<dim3(nt, 1, nblocks), BG_THREADS, kSmemMK, st>>>(w);
-    HPSD_LAUNCH_CHECK();
+    if (!factors_done) {
+        rc = launch_bt_factors(w, st);
+        if (rc) return rc;
+    }
     for (int b = nblocks - 1; b >= 0; --b) {
         const int m = n - b * kNBT - 1;
         if (m <= 0) continue;

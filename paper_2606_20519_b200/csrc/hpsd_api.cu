@@ -269,6 +269,10 @@ int hpsd_set_option(const char *name, int value) {
         g_opt.medium_dc = (value != 0);
         return HPSD_OK;
     }
+    if (std::strcmp(name, "overlap_factors") == 0) {
+        g_overlap_factors = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "cluster_tridiag") == 0) {
         g_cluster_tridiag = (value != 0);
         return HPSD_OK;

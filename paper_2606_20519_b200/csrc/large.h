@@ -27,6 +27,7 @@ void tridiag_fill_tiles(int n, int2 *tiles_host);
 int launch_tridiag(const TridiagWs &w, cudaStream_t st);
 
 // ---- tridiag_cluster.cu: S1+S2+S3 in one 16-CTA cluster, matrix resident in distributed shared memory ----
+extern int g_overlap_factors;            // option "overlap_factors" (default 1), largepath.cu
 extern int g_cluster_tridiag;            // option "cluster_tridiag" (default 1)
 int tridiag_cluster_init();
 int tridiag_cluster_fits(int n);         // 1 when this device and this n are served by the cluster kernel
@@ -79,6 +80,8 @@ struct BackWs {
 };
 int backherk_init();
 // lam ascending (n), Zt real eigenvectors of T (ldzt x n); writes the projection's svec (and the ADMM v update) through io.
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st);
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done = false);
+// the part of S5 that needs the reflectors only (Gram, T_b, V_b T_b); launch_back_herk(..., factors_done = true) then skips it
+int launch_bt_factors(const BackWs &w, cudaStream_t st);
 
 }  // namespace hpsd

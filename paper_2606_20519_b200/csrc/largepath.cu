@@ -10,6 +10,9 @@ namespace hpsd {
 namespace {
 
 int g_sms = 0;
+}  // namespace
+int g_overlap_factors = 1;    // option "overlap_factors"
+namespace {
 
 struct LargeWs {
     TridiagWs t;
@@ -72,6 +75,29 @@ LargeWs carve(int n, unsigned char *base) {
     return w;
 }
 
+// Side stream of the large path: the compact-WY factors of S5 run next to the divide & conquer (fork after S2/S3,
+// join before the back-transform; capturable in a CUDA graph like any fork/join of events).
+struct Side {
+    cudaStream_t st = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+    int dev = -1;
+};
+thread_local Side g_side;
+
+bool side_ready() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (g_side.st && g_side.dev == dev) return true;
+    if (g_side.st) { cudaStreamDestroy(g_side.st); cudaEventDestroy(g_side.fork); cudaEventDestroy(g_side.join); g_side = Side(); }
+    if (cudaStreamCreateWithFlags(&g_side.st, cudaStreamNonBlocking) != cudaSuccess) { g_side = Side(); cudaGetLastError(); return false; }
+    if (cudaEventCreateWithFlags(&g_side.fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g_side.join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaStreamDestroy(g_side.st); g_side = Side(); cudaGetLastError(); return false;
+    }
+    g_side.dev = dev;
+    return true;
+}
+
 int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, const double *sub, cudaStream_t st) {
     if (g_cluster_tridiag && tridiag_cluster_fits(n)) return launch_tridiag_cluster(w.t, in, sub, st);
     if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
@@ -124,12 +150,21 @@ int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int
     w.s.info = info;
     int rc = reduce_to_tridiagonal(w, n, io.in, io.sub, st);
     if (rc) return rc;
+    bool forked = false;
+    if (g_overlap_factors && side_ready() && cudaEventRecord(g_side.fork, st) == cudaSuccess &&
+        cudaStreamWaitEvent(g_side.st, g_side.fork, 0) == cudaSuccess) {
+        rc = launch_bt_factors(w.b, g_side.st);
+        forked = true;                                    // joined below even on error: a capture must not be left forked
+        if (cudaEventRecord(g_side.join, g_side.st) != cudaSuccess && !rc) rc = HPSD_ECUDA_;
+    }
     double *lam, *Z;
     prof_begin(ST_STEDC, st);
-    rc = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
+    int rc2 = launch_stedc(w.s, w.t.d, w.t.e, &lam, &Z, st);
     prof_end(ST_STEDC, st);
+    if (forked && cudaStreamWaitEvent(st, g_side.join, 0) != cudaSuccess && !rc) rc = HPSD_ECUDA_;
     if (rc) return rc;
-    return launch_back_herk(w.b, lam, Z, w.s.ldz, io, st);
+    if (rc2) return rc2;
+    return launch_back_herk(w.b, lam, Z, w.s.ldz, io, st, forked);
 }
 
 }  // namespace hpsd
