@@ -131,6 +131,10 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *   "overlap_factors" (0/1, default 1): the compact-WY factors of the back-transform (they depend on the
  *       reflectors only) run on an internal side stream next to the divide & conquer; fork and join are events
  *       on the caller's stream, so the call stays asynchronous and capturable.
+ *   "graph_replay" (0/1, default 1): the second call with the same size list AND the same buffers (an ADMM
+ *       loop) is captured into a CUDA graph on an internal stream; that call and the following ones are one
+ *       cudaGraphLaunch on the caller's stream (same kernels, same order).  Off while "profile" is on or when the
+ *       caller's stream is itself capturing.  Any hpsd_set_option call discards the cached graphs.
  *   "profile" (0/1): record CUDA events on the caller's stream around every stage
  *       of the path (S1..S10) for hpsd_profile_read.  Off by default. */
 int hpsd_set_option(const char *name, int value);

@@ -52,6 +52,7 @@ struct Options {
     int jacobi_max_n = 32;            // blocks with 2 <= n <= this use the one-CTA Jacobi kernel
     int medium_max_n = kMediumMaxN;   // blocks with jacobi_max_n < n <= this use the one-CTA Householder kernels
     int medium_dc = 1;                // medium blocks with n <= kMedDcMaxN: batched divide & conquer instead of in-CTA QL
+    int graph_replay = 1;             // replay repeated calls (same buffers) as a CUDA graph
 } g_opt;
 
 inline bool use_meddc(const Options &o, int n) { return o.medium_dc && n > o.jacobi_max_n && n <= o.medium_max_n && n <= kMedDcMaxN; }
@@ -68,7 +69,17 @@ struct JacobiGroup {
 
 struct LargeBlock { int n; long long off; int idx; };
 
+// A projection replayed as a CUDA graph: ADMM calls the library with the same buffers every iteration, and below
+// n ~ 1000 the 20-170 dependent launches of a call are launch-latency-bound.  Keyed by every pointer of the call.
+struct GraphEntry {
+    const void *in = nullptr, *sub = nullptr, *out = nullptr, *vout = nullptr, *ws = nullptr, *info = nullptr;
+    cudaGraphExec_t exec = nullptr;     // null until the second call with the same key
+    int launches = 0;
+    unsigned long long stamp = 0;
+};
+
 struct Plan {
+    std::vector<GraphEntry> graphs;
     std::vector<int> sizes;
     int jacobi_max_n, medium_max_n, medium_dc;
     std::vector<JacobiGroup> groups;
@@ -80,7 +91,12 @@ struct Plan {
     size_t n_ll = 0, n_int = 0;
     std::map<int, int2 *> tiles_dev;   // tridiagonalisation tile tables per distinct large n
     size_t ws_bytes = 0;               // scratch needed by the large path (max over large blocks) + info
+    void drop_graphs() {
+        for (GraphEntry &g : graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+        graphs.clear();
+    }
     ~Plan() {
+        drop_graphs();
         if (desc_dev) cudaFree(desc_dev);
         for (auto &kv : tiles_dev) cudaFree(kv.second);
     }
@@ -89,6 +105,8 @@ struct Plan {
 };
 
 struct DeviceState {
+    cudaStream_t cap_stream = nullptr;     // graphs are captured here (the caller's stream may be the legacy stream)
+    unsigned long long stamp = 0;
     std::vector<std::unique_ptr<Plan>> plans;
     void *ws = nullptr; size_t ws_bytes = 0;
     double *stage_in = nullptr, *stage_out = nullptr; size_t stage_elems = 0;
@@ -256,6 +274,12 @@ const char *hpsd_strerror(int code) {
 int hpsd_set_option(const char *name, int value) {
     if (!name) return HPSD_EINVAL;
     std::lock_guard<std::mutex> lk(g_mu);
+    for (auto &kv : g_dev)                      // a captured call froze the options it ran with
+        for (auto &pl : kv.second.plans) pl->drop_graphs();
+    if (std::strcmp(name, "graph_replay") == 0) {
+        g_opt.graph_replay = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "profile") == 0) {
         g_profile = (value != 0);
         return HPSD_OK;
@@ -343,7 +367,55 @@ static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void 
     Plan *pl;
     rc = get_plan(ds, n_blocks, sizes, &pl);
     if (rc) return rc;
-    return run_plan(*pl, io, ws, info_dev, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (!g_opt.graph_replay || g_profile || cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return run_plan(*pl, io, ws, info_dev, st);           // includes: the caller is capturing this call itself
+    }
+    GraphEntry *ge = nullptr;
+    for (GraphEntry &g : pl->graphs)
+        if (g.in == io.in && g.sub == io.sub && g.out == io.out && g.vout == io.vout && g.ws == ws && g.info == info_dev) { ge = &g; break; }
+    if (ge && ge->exec) {
+        ge->stamp = ++ds.stamp;
+        g_launches = ge->launches;
+        return cudaGraphLaunch(ge->exec, st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    }
+    if (!ge) {
+        // first call with these buffers: plain launches (also warms every lazy initialisation up)
+        if (pl->graphs.size() >= 8) {
+            size_t old = 0;
+            for (size_t i = 1; i < pl->graphs.size(); ++i) if (pl->graphs[i].stamp < pl->graphs[old].stamp) old = i;
+            if (pl->graphs[old].exec) cudaGraphExecDestroy(pl->graphs[old].exec);
+            pl->graphs.erase(pl->graphs.begin() + old);
+        }
+        GraphEntry g;
+        g.in = io.in; g.sub = io.sub; g.out = io.out; g.vout = io.vout; g.ws = ws; g.info = info_dev; g.stamp = ++ds.stamp;
+        pl->graphs.push_back(g);
+        return run_plan(*pl, io, ws, info_dev, st);
+    }
+    // second call with the same buffers: capture on the library's stream, replay on the caller's from now on
+    if (!ds.cap_stream && cudaStreamCreateWithFlags(&ds.cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError();
+        return run_plan(*pl, io, ws, info_dev, st);
+    }
+    if (cudaStreamBeginCapture(ds.cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return run_plan(*pl, io, ws, info_dev, st);
+    }
+    rc = run_plan(*pl, io, ws, info_dev, ds.cap_stream);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ec = cudaStreamEndCapture(ds.cap_stream, &graph);
+    if (rc || ec != cudaSuccess || !graph || cudaGraphInstantiate(&ge->exec, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        ge->exec = nullptr;
+        cudaGetLastError();
+        return rc ? rc : run_plan(*pl, io, ws, info_dev, st);
+    }
+    cudaGraphDestroy(graph);
+    ge->launches = g_launches;
+    ge->stamp = ++ds.stamp;
+    return cudaGraphLaunch(ge->exec, st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
 }
 
 // library-owned workspace of the current device, grown on demand
@@ -502,6 +574,7 @@ int hpsd_release(void) {
         cudaDeviceSynchronize();
         DeviceState &ds = it->second;
         ds.plans.clear();
+        if (ds.cap_stream) { cudaStreamDestroy(ds.cap_stream); ds.cap_stream = nullptr; }
         if (ds.ws) cudaFree(ds.ws);
         if (ds.stage_in) cudaFree(ds.stage_in);
         if (ds.stage_out) cudaFree(ds.stage_out);

@@ -490,3 +490,49 @@ def test_cluster_tridiag_kernel(orc, hp, n):
     assert float((e1 - e0).abs().max()) <= 1e-13 * n * scale
     assert parity_err(t_u.cpu().numpy(), want_u, sv - v, n) <= TOL * n
     assert parity_err(t_v.cpu().numpy(), want_v, sv - v, n) <= TOL * n
+
+
+def test_graph_replay_of_repeated_calls(orc, hp):
+    """Option "graph_replay" (default 1): the second and later calls with the same size list and the same buffers
+    (an ADMM loop) are replayed as a CUDA graph.  The replay must equal the plain launches bit for bit, must see new
+    CONTENTS of the same buffers, must work on a non-default stream, and the fused ADMM step must replay as well."""
+    import torch
+    rng = np.random.default_rng(77)
+    sizes = [150, 1, 24, 81, 36]
+    sv1 = pack_all(orc, [herm(rng, n) for n in sizes])
+    sv2 = pack_all(orc, [herm(rng, n) for n in sizes])
+    hp.set_option("graph_replay", 0)
+    plain1, plain2 = gpu_project(hp, sizes, sv1), gpu_project(hp, sizes, sv2)
+    hp.set_option("graph_replay", 1)
+    t_in, t_out = torch.from_numpy(sv1.copy()).cuda(), torch.empty(sv1.size, dtype=torch.float64, device="cuda")
+    for it in range(4):                                  # 1: plain launches, 2: capture + launch, 3-4: replay
+        t_out.zero_()
+        hp.project_(sizes, t_in, t_out)
+        torch.cuda.synchronize()
+        assert np.array_equal(t_out.cpu().numpy(), plain1), it
+    t_in.copy_(torch.from_numpy(sv2))                    # same buffers, new contents
+    hp.project_(sizes, t_in, t_out)
+    torch.cuda.synchronize()
+    assert np.array_equal(t_out.cpu().numpy(), plain2)
+    want = orc.project(sizes, sv2, nthreads=orc.max_threads())
+    off = 0
+    for n in sizes:
+        sl = slice(off, off + n * n)
+        assert parity_err(t_out.cpu().numpy()[sl], want[sl], sv2[sl], n) <= TOL * n
+        off += n * n
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        for _ in range(3):
+            hp.project_(sizes, t_in, t_out, stream=s)
+    s.synchronize()
+    assert np.array_equal(t_out.cpu().numpy(), plain2)
+    # fused ADMM step (Eqs. D33-D34), repeated with the same buffers: v changes every iteration
+    ut, v = torch.from_numpy(sv1.copy()).cuda(), torch.from_numpy(sv2.copy()).cuda()
+    u = torch.empty_like(ut)
+    v_ref, u_ref = sv2.copy(), None
+    for it in range(3):
+        hp.admm_step_(sizes, ut, v, u)
+        torch.cuda.synchronize()
+        u_ref, v_ref = orc.admm_step(sizes, sv1, v_ref, nthreads=orc.max_threads())
+        assert rel_err(u.cpu().numpy(), u_ref) <= TOL * max(sizes), it
+        assert rel_err(v.cpu().numpy(), v_ref) <= TOL * max(sizes), it
