@@ -120,12 +120,17 @@ __device__ __forceinline__ void cl_householder(cplx alpha, double xnorm2, double
     if (xnorm2 == 0.0 && alpha.y == 0.0) {
         beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
     } else {
-        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        // zlarfg scalars with one reciprocal square root and one reciprocal on the dependent chain (every CTA runs this
+        // redundantly once per column): 1/beta comes from rsqrt, refined by one Newton step to full accuracy
+        const double s = alpha.x * alpha.x + alpha.y * alpha.y + xnorm2;
+        double rinv = rsqrt(s);
+        rinv = fma(0.5 * rinv, fma(-s * rinv, rinv, 1.0), rinv);
+        const double nrm = s * rinv;
         beta = -copysign(nrm, alpha.x);
-        const double ib = 1.0 / beta;
+        const double ib = -copysign(rinv, alpha.x);
         tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
         const cplx den = mk(alpha.x - beta, alpha.y);
-        const double id2 = 1.0 / abs2(den);
+        const double id2 = __drcp_rn(abs2(den));
         scale = mk(den.x * id2, -den.y * id2);
     }
 }
