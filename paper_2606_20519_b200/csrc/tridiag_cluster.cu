@@ -102,7 +102,7 @@ __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     const int rs = (n + kCl - 1) / kCl;
     size_t off = 0;
     s.mbar = off; off += 16;                      // two mbarriers
-    s.tok = off; off += 8 * kClWarps;             // landing slots of the export tokens
+    s.tok = off; off += 8 * (kClWarps + kCl);     // landing slots of the export tokens and of the phase tokens
     s.colv = off; off += sizeof(cplx) * 3 * nc;
     s.q = off; off += sizeof(double) * 2 * kCl;    // v^H y partials, double-buffered by step parity
     s.red = off; off += sizeof(double) * (2 * kClWarps + 4);   // block-reduction scratch + alpha, d_c
@@ -229,7 +229,8 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         if (lo < c + 1) lo = c + 1;
         if (hi > n) hi = n;
         const int act = hi > lo ? hi - lo : 0;
-        return (unsigned)(kCl * act * 16 + kClWarps * 8);        // + the export tokens of the owner of column c+1
+        // + the export tokens of the owner of column c+1 + (from step 1 on) one phase token per CTA
+        return (unsigned)(kCl * act * 16 + kClWarps * 8 + (c > 0 ? kCl * 8 : 0));
     };
     auto bytes_w = [&](int c) -> unsigned { return (unsigned)((n - c - 1) * 16 + kCl * 8); };
     if (tid == 0) {
@@ -431,15 +432,18 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         qp = warp_sum(qp);
         if (lane == 0) s_red[kRedQ + wp] = qp;
         __syncthreads();
-        if (tid < kCl) {
-            double q = 0.0;
-#pragma unroll
-            for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
-            cl_st_async(cl_mapa(sq_a + 8u * (unsigned)((c & 1) * kCl + r), tid), q, cl_mapa(mbar2, tid));   // needed only with w: phase 2
-        }
         CLTRACE(4);
         cl_wait(mbar1, c & 1);                                    // every contribution to my rows has landed
         if (tid == 0) cl_arm(mbar1, bytes_r(c + 1));
+        if (tid < kCl) {
+            // the partial v^H y is needed only with w, so it rides on phase 2; it is sent AFTER this CTA completed
+            // phase 1, which makes "a peer completed phase 2 of step c" imply "I completed phase 1 of step c":
+            // nothing of step c+1 can reach an mbarrier that is still in step c (see also the tokens below)
+            double q = 0.0;
+#pragma unroll
+            for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
+            cl_st_async(cl_mapa(sq_a + 8u * (unsigned)((c & 1) * kCl + r), tid), q, cl_mapa(mbar2, tid));
+        }
         CLTRACE(5);
 
         // ================= [D] sum the contributions of my rows, broadcast tau y =================
@@ -467,6 +471,9 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         }
         CLTRACE(6);
         cl_wait(mbar2, c & 1);                                    // all of tau y has landed
+        // one 8-byte token to every CTA on phase 1 of the NEXT step: a peer completes that phase only after I have
+        // completed phase 2 of this step, so its phase-2 traffic of step c+1 cannot arrive here early
+        if (tid < kCl && c + 1 < n - 1) cl_st_async(cl_mapa(tok_a + 8u * (unsigned)(kClWarps + r), tid), 1.0, cl_mapa(mbar1, tid));
         double q = 0.0;
 #pragma unroll
         for (int k = 0; k < kCl; ++k) q += s_q[(c & 1) * kCl + k];
