@@ -245,17 +245,22 @@ def test_medium_kernel_on_small_sizes(orc, hp, n):
         hp.set_option("jacobi_max_n", 32)
 
 
+@pytest.mark.parametrize("cluster", [1, 0])
 @pytest.mark.parametrize("n", [2, 3, 31, 32, 33, 63, 64, 65, 85, 96, 127, 128, 129, 200, 257, 320])
-def test_large_path_sizes(orc, hp, n):
-    """Force every block through S1..S8 of the Householder/D&C path (ragged tiles, several panels)."""
+def test_large_path_sizes(orc, hp, n, cluster):
+    """Force every block through S1..S8 of the Householder/D&C path (ragged tiles, several panels): with the
+    cluster-resident reduction (default for 16 <= n <= 638) and with the grid-wide panel kernel (cluster = 0), which
+    otherwise only serves n > 638."""
     rng = np.random.default_rng(300 + n)
     sv = orc.pack(herm(rng, n))
     force_large(hp, True)
+    hp.set_option("cluster_tridiag", cluster)
     try:
         got, _ = check_vs_oracle(orc, hp, [n], sv, nthreads=orc.max_threads() if n > 150 else 1)
         check_invariants(hp, [n], sv, got)
     finally:
         force_large(hp, False)
+        hp.set_option("cluster_tridiag", 1)
 
 
 # ------------------------------------------------------------------ degenerate inputs
