@@ -365,10 +365,9 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             for (int s = 0; s < kClR; ++s) {
                 const int i0 = 32 * cl_chunk(s, wp), i = i0 + lane;
                 if (i0 + 31 < j0 || i0 >= n) continue;            // warp-uniform: nothing of this chunk in the trip
-                if (i0 > j0 + kCl * (kKT - 1) && i0 + 32 <= n && ncol >= kKT)
-                    cl_elems<false>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
-                else
-                    cl_elems<true>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
+                // (a predicate-free variant for chunks entirely below the diagonals was measured and dropped: the extra
+                // warp-uniform branch costs more than the ~11 select/compare instructions per element it saves)
+                cl_elems<true>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
             }
             CLT2(2);
             // halving butterfly: kKT values x 32 lanes -> lane 32 q / kKT holds the total of column q
