@@ -122,8 +122,13 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
                     double s = 1.0, c = 1.0, p = 0.0;
                     int i;
                     bool under = false;
+                    // the operands of step i are loaded one step ahead: the compiler cannot hoist the loads over the
+                    // stores of the previous step (possible alias), and their latency would sit in the dependent chain
+                    double e_i = ee[mm - 1], d_i = dd[mm - 1], d_i1 = dd[mm];
                     for (i = mm - 1; i >= l; --i) {
-                        const double f = s * ee[i], b = c * ee[i];
+                        const double e_cur = e_i, d_cur = d_i, d_up = d_i1;
+                        if (i > l) { e_i = ee[i - 1]; d_i = dd[i - 1]; }
+                        const double f = s * e_cur, b = c * e_cur;
                         const double h2 = fma(f, f, g * g);
                         double ir;
                         if (h2 > 1e-280) {                      // T is scaled to unit max-norm: no overflow
@@ -137,10 +142,11 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
                         ee[i + 1] = r;
                         if (r == 0.0) { dd[i + 1] -= p; ee[mm] = 0.0; under = true; break; }
                         s = f * ir; c = g * ir;
-                        g = dd[i + 1] - p;
-                        r = (dd[i] - g) * s + 2.0 * c * b;
+                        g = d_up - p;
+                        r = (d_cur - g) * s + 2.0 * c * b;
                         p = s * r;
                         dd[i + 1] = g + p;
+                        d_i1 = d_cur;                            // dd[i] is untouched until the next step rewrites it
                         g = c * r - b;
                         cs[i] = c; sn[i] = s;
                     }
@@ -153,12 +159,15 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
             const int mm = ctrl[0], ilo = ctrl[1];
             if (mm == l) break;
             if (++iter > 80) { fail = true; break; }
-            if (lane < m) {
+            if (lane < m && mm - 1 >= ilo) {
+                // column ii of one rotation is column (ii-1)+1 of the next: carried in a register, not through shared memory
+                double f = Zs[mm * (kLeaf + 1) + lane];
                 for (int ii = mm - 1; ii >= ilo; --ii) {
-                    const double f = Zs[(ii + 1) * (kLeaf + 1) + lane], q = Zs[ii * (kLeaf + 1) + lane];
+                    const double q = Zs[ii * (kLeaf + 1) + lane];
                     Zs[(ii + 1) * (kLeaf + 1) + lane] = sn[ii] * q + cs[ii] * f;
-                    Zs[ii * (kLeaf + 1) + lane] = cs[ii] * q - sn[ii] * f;
+                    f = cs[ii] * q - sn[ii] * f;
                 }
+                Zs[ilo * (kLeaf + 1) + lane] = f;
             }
             __syncwarp();
         }
