@@ -133,17 +133,23 @@ __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
         const double alphap = -0.5 * abs2(tau) * q.x;       // v^H A v is real
         for (int r = c + 1 + tid; r < n; r += kMedThreads) sm.y[r] = tau * sm.y[r] + alphap * sm.x[r];
         __syncthreads();
-        // A22 -= v w^H + w v^H on the full trailing block
-        for (int e = tid; e < m * m; e += kMedThreads) {
-            const int rr = e % m, jj = e / m;
-            const int r = c + 1 + rr, j = c + 1 + jj;
-            cplx a = A[(size_t)j * ld + r];
-            const cplx vr = sm.x[r], wr = sm.y[r], vj = sm.x[j], wj = sm.y[j];
-            // v_r conj(w_j) + w_r conj(v_j)
-            a.x -= vr.x * wj.x + vr.y * wj.y + wr.x * vj.x + wr.y * vj.y;
-            a.y -= vr.y * wj.x - vr.x * wj.y + wr.y * vj.x - wr.x * vj.y;
-            if (r == j) a.y = 0.0;
-            A[(size_t)j * ld + r] = a;
+        // A22 -= v w^H + w v^H on the full trailing block: lane = row (its v_r, w_r stay in registers), warp = column
+        // class; no integer divisions, the column's v_j, w_j are broadcast loads
+        for (int rb = 0; rb < m; rb += 32) {
+            const int r = c + 1 + rb + lane;
+            const bool rok = r < n;
+            const cplx vr = rok ? sm.x[r] : mk(0.0, 0.0), wr = rok ? sm.y[r] : mk(0.0, 0.0);
+            for (int j = c + 1 + warp; j < n; j += kMedThreads / 32) {
+                const cplx vj = sm.x[j], wj = sm.y[j];
+                if (rok) {
+                    cplx a = A[(size_t)j * ld + r];
+                    // v_r conj(w_j) + w_r conj(v_j)
+                    a.x -= vr.x * wj.x + vr.y * wj.y + wr.x * vj.x + wr.y * vj.y;
+                    a.y -= vr.y * wj.x - vr.x * wj.y + wr.y * vj.x - wr.x * vj.y;
+                    if (r == j) a.y = 0.0;
+                    A[(size_t)j * ld + r] = a;
+                }
+            }
         }
         __syncthreads();
     }
