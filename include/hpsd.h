@@ -126,11 +126,17 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *       the batched device-side divide & conquer (whole group as one virtual problem) instead of the
  *       in-CTA implicit QL.
  *   "cluster_tridiag" (0/1, default 1): blocks whose packed lower triangle fits in the shared memory of one
- *       16-CTA cluster (116 < n <= ~640) are tridiagonalised by the cluster-resident kernel (S1+S2+S3 in one
+ *       16-CTA cluster (116 < n <= ~631) are tridiagonalised by the cluster-resident kernel (S1+S2+S3 in one
  *       launch); 0 forces the grid-wide panel kernel.
  *   "overlap_factors" (0/1, default 1): the compact-WY factors of the back-transform (they depend on the
  *       reflectors only) run on an internal side stream next to the divide & conquer; fork and join are events
  *       on the caller's stream, so the call stays asynchronous and capturable.
+ *   "large_lanes" (0/1, default 1): two or more blocks of one call whose reduction runs on a single 16-CTA cluster
+ *       (sizes up to ~631) are processed next to each other on up to 8 internal lane streams, each with its own part of
+ *       the workspace (hpsd_workspace_size accounts for it); fork and join are events on the caller's stream.
+ *   "medium_reroute" (0/1, default 1): a group of at most 5 blocks of one size in 84..116 (the in-CTA QL range), or a
+ *       single block of size 64..83, goes through the large path (cluster-resident reduction) instead of the one-CTA
+ *       medium kernels, which pay their latency once per group, not per block.
  *   "graph_replay" (0/1, default 1): the second call with the same size list AND the same buffers (an ADMM
  *       loop) is captured into a CUDA graph on an internal stream; that call and the following ones are one
  *       cudaGraphLaunch on the caller's stream (same kernels, same order).  Off while "profile" is on or when the

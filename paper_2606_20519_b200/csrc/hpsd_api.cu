@@ -53,6 +53,8 @@ struct Options {
     int medium_max_n = kMediumMaxN;   // blocks with jacobi_max_n < n <= this use the one-CTA Householder kernels
     int medium_dc = 1;                // medium blocks with n <= kMedDcMaxN: batched divide & conquer instead of in-CTA QL
     int graph_replay = 1;             // replay repeated calls (same buffers) as a CUDA graph
+    int medium_reroute = 1;           // few medium blocks of one size go through the cluster-resident large path
+    int large_lanes = 1;              // several cluster-sized blocks of one call run on parallel lane streams
 } g_opt;
 
 inline bool use_meddc(const Options &o, int n) { return o.medium_dc && n > o.jacobi_max_n && n <= o.medium_max_n && n <= kMedDcMaxN; }
@@ -67,7 +69,7 @@ struct JacobiGroup {
     size_t idx_index;   // index (in int units) of this group's info indices
 };
 
-struct LargeBlock { int n; long long off; int idx; };
+struct LargeBlock { int n; long long off; int idx; int lane = -1; };   // lane >= 0: runs on that lane stream, next to other blocks
 
 // A projection replayed as a CUDA graph: ADMM calls the library with the same buffers every iteration, and below
 // n ~ 1000 the 20-170 dependent launches of a call are launch-latency-bound.  Keyed by every pointer of the call.
@@ -81,7 +83,7 @@ struct GraphEntry {
 struct Plan {
     std::vector<GraphEntry> graphs;
     std::vector<int> sizes;
-    int jacobi_max_n, medium_max_n, medium_dc;
+    int jacobi_max_n, medium_max_n, medium_dc, medium_reroute, large_lanes;
     std::vector<JacobiGroup> groups;
     std::vector<LargeBlock> large;
     int n_scalar = 0;
@@ -91,6 +93,8 @@ struct Plan {
     size_t n_ll = 0, n_int = 0;
     std::map<int, int2 *> tiles_dev;   // tridiagonalisation tile tables per distinct large n
     size_t ws_bytes = 0;               // scratch needed by the large path (max over large blocks) + info
+    int n_lanes = 0;                   // blocks served by the cluster-resident reduction run on this many lane streams
+    size_t base_ws = 0, lane_ws = 0;   // scratch of the sequential part | of ONE lane (lanes follow the sequential part)
     void drop_graphs() {
         for (GraphEntry &g : graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
         graphs.clear();
@@ -105,6 +109,8 @@ struct Plan {
 };
 
 struct DeviceState {
+    cudaStream_t lane_stream[kLargeLanes] = {};   // several cluster-sized blocks of one call run next to each other
+    cudaEvent_t lane_fork = nullptr, lane_join[kLargeLanes] = {};
     cudaStream_t cap_stream = nullptr;     // graphs are captured here (the caller's stream may be the legacy stream)
     unsigned long long stamp = 0;
     std::vector<std::unique_ptr<Plan>> plans;
@@ -130,14 +136,19 @@ int init_device(DeviceState &ds) {
     return 0;
 }
 
-int build_plan(int n_blocks, const int *sizes, Plan &pl) {
+// Host-only part of the plan: routes every block (scalar / one-CTA group / large path, sequential or on a lane) and
+// sizes the workspace.  `fits(n)`: the cluster-resident reduction serves size n.  hpsd_workspace_size runs it with the
+// device-independent size test and with "never" and takes the larger result, so its answer bounds every device's plan.
+int cluster_never(int) { return 0; }
+
+void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*fits)(int), std::vector<long long> &ll, std::vector<int> &ints) {
     pl.sizes.assign(sizes, sizes + n_blocks);
     pl.jacobi_max_n = g_opt.jacobi_max_n;
     pl.medium_max_n = g_opt.medium_max_n;
     pl.medium_dc = g_opt.medium_dc;
+    pl.medium_reroute = g_opt.medium_reroute;
+    pl.large_lanes = g_opt.large_lanes;
     const int lim = small_limit(g_opt);
-    std::vector<long long> ll;
-    std::vector<int> ints;
     std::map<int, std::vector<std::pair<long long, int>>> by_n;
     std::vector<long long> scalars;
     long long off = 0;
@@ -152,6 +163,15 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     pl.scalar_off_index = ll.size();
     for (long long o : scalars) ll.push_back(o);
     for (auto &kv : by_n) {
+        // Few blocks of one medium size are faster one after the other through the large path, whose reduction runs on
+        // a 16-CTA cluster (measured on B200: n = 84..116, in-CTA QL 2.6-5.0 ms per GROUP up to 64 blocks against
+        // 0.50-0.73 ms per BLOCK; n = 64..83, one block: 0.63-0.65 against 0.49-0.56 ms)
+        const int gn = kv.first, gc = (int)kv.second.size();
+        if (g_opt.medium_reroute && gn > g_opt.jacobi_max_n && fits(gn) &&
+            ((gn > kMedDcMaxN || !g_opt.medium_dc) ? gc <= 5 : (gn >= 64 && gc == 1))) {
+            for (auto &pr : kv.second) pl.large.push_back({gn, pr.first, pr.second});
+            continue;
+        }
         JacobiGroup g;
         g.n = kv.first; g.count = (int)kv.second.size();
         g.medium = g.n > pl.jacobi_max_n;
@@ -160,6 +180,32 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
         for (auto &pr : kv.second) { ll.push_back(pr.first); ints.push_back(pr.second); }
         pl.groups.push_back(g);
     }
+    // blocks whose reduction occupies one 16-CTA cluster leave 132 SMs idle: two or more of them in one call run on
+    // lane streams with a scratch area each (up to kLargeLanes at a time, round robin)
+    int n_fast = 0;
+    if (g_opt.large_lanes)
+        for (auto &lb : pl.large) if (fits(lb.n)) ++n_fast;
+    pl.n_lanes = n_fast >= 2 ? std::min(n_fast, kLargeLanes) : 0;
+    if (pl.n_lanes) {
+        int k = 0;
+        for (auto &lb : pl.large) if (fits(lb.n)) lb.lane = (k++) % pl.n_lanes;
+    }
+    size_t ws = 0, lane_ws = 0;
+    for (const JacobiGroup &g : pl.groups)
+        if (g.dc) ws = std::max(ws, meddc_ws_bytes(g.n, g.count));
+    for (auto &lb : pl.large) {
+        const size_t w = align_up(largepath_ws_bytes(lb.n), 256);
+        if (lb.lane >= 0) { if (w > lane_ws) lane_ws = w; }
+        else if (w > ws) ws = w;
+    }
+    pl.base_ws = align_up(ws, 256); pl.lane_ws = lane_ws;
+    pl.ws_bytes = pl.base_ws + pl.n_lanes * pl.lane_ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
+}
+
+int build_plan(int n_blocks, const int *sizes, Plan &pl) {
+    std::vector<long long> ll;
+    std::vector<int> ints;
+    route_plan(n_blocks, sizes, pl, tridiag_cluster_fits, ll, ints);
     pl.n_ll = ll.size(); pl.n_int = ints.size();
     const size_t bytes = ll.size() * sizeof(long long) + ints.size() * sizeof(int);
     if (bytes) {
@@ -169,9 +215,6 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
         std::memcpy(host.data() + ll.size() * sizeof(long long), ints.data(), ints.size() * sizeof(int));
         if (cudaMemcpy(pl.desc_dev, host.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) return HPSD_ECUDA;
     }
-    size_t ws = 0;
-    for (const JacobiGroup &g : pl.groups)
-        if (g.dc) ws = std::max(ws, meddc_ws_bytes(g.n, g.count));
     for (auto &lb : pl.large) {
         if (!pl.tiles_dev.count(lb.n)) {
             const size_t nt = tridiag_tile_count(lb.n);
@@ -182,10 +225,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
             if (cudaMemcpy(dptr, t.data(), nt * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(dptr); return HPSD_ECUDA; }
             pl.tiles_dev[lb.n] = dptr;
         }
-        const size_t w = largepath_ws_bytes(lb.n);
-        if (w > ws) ws = w;
     }
-    pl.ws_bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
     return 0;
 }
 
@@ -193,7 +233,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
 // synchronises (cudaMalloc/cudaMemcpy); later calls with the same list are launch-only.
 int get_plan(DeviceState &ds, int n_blocks, const int *sizes, Plan **out) {
     for (auto &p : ds.plans) {
-        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n && p->medium_dc == g_opt.medium_dc &&
+        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n && p->medium_dc == g_opt.medium_dc && p->medium_reroute == g_opt.medium_reroute && p->large_lanes == g_opt.large_lanes &&
             (n_blocks == 0 || std::memcmp(p->sizes.data(), sizes, sizeof(int) * n_blocks) == 0)) {
             *out = p.get();
             return 0;
@@ -221,7 +261,16 @@ int check_args(int n_blocks, const int *sizes, const void *in, const void *out, 
     return 0;
 }
 
-int run_plan(const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStream_t st) {
+bool lanes_ready(DeviceState &ds, int n) {
+    if (!ds.lane_fork && cudaEventCreateWithFlags(&ds.lane_fork, cudaEventDisableTiming) != cudaSuccess) { ds.lane_fork = nullptr; cudaGetLastError(); return false; }
+    for (int l = 0; l < n; ++l) {
+        if (!ds.lane_stream[l] && cudaStreamCreateWithFlags(&ds.lane_stream[l], cudaStreamNonBlocking) != cudaSuccess) { ds.lane_stream[l] = nullptr; cudaGetLastError(); return false; }
+        if (!ds.lane_join[l] && cudaEventCreateWithFlags(&ds.lane_join[l], cudaEventDisableTiming) != cudaSuccess) { ds.lane_join[l] = nullptr; cudaGetLastError(); return false; }
+    }
+    return true;
+}
+
+int run_plan(DeviceState &ds, const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStream_t st) {
     // info lives at the start of the workspace when the caller gave none
     int *info = info_dev ? info_dev : reinterpret_cast<int *>(ws);
     unsigned char *scratch = reinterpret_cast<unsigned char *>(ws) + align_up(pl.sizes.size() * sizeof(int) + 4, 256);
@@ -244,11 +293,30 @@ int run_plan(const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStre
         prof_end(g.medium ? ST_MEDIUM : ST_JACOBI, st);
         if (rc) return rc;
     }
-    for (const LargeBlock &lb : pl.large) {
-        rc = largepath_project(lb.n, io_offset(io, lb.off), scratch, pl.tiles_dev.at(lb.n), info + lb.idx, st);
-        if (rc) return rc;
+    // lanes: fork from the caller's stream, one stream and one scratch area per lane, join at the end.  Not under
+    // "profile" (the stage timers want one stream).  The sequential blocks (cooperative panel kernel) go in between.
+    const bool lanes = pl.n_lanes > 0 && !g_profile && lanes_ready(ds, pl.n_lanes) && cudaEventRecord(ds.lane_fork, st) == cudaSuccess;
+    int rc_lane = 0;
+    if (lanes) {
+        for (int l = 0; l < pl.n_lanes; ++l)
+            if (cudaStreamWaitEvent(ds.lane_stream[l], ds.lane_fork, 0) != cudaSuccess) rc_lane = HPSD_ECUDA;
+        for (const LargeBlock &lb : pl.large) {
+            if (lb.lane < 0 || rc_lane) continue;
+            rc_lane = largepath_project(lb.n, io_offset(io, lb.off), scratch + pl.base_ws + (size_t)lb.lane * pl.lane_ws, pl.tiles_dev.at(lb.n),
+                                        info + lb.idx, ds.lane_stream[lb.lane], lb.lane);
+        }
     }
-    return 0;
+    for (const LargeBlock &lb : pl.large) {
+        if (lanes && lb.lane >= 0) continue;
+        // without lanes every block takes the sequential scratch (a lane block fits: base_ws or lane 0's area)
+        unsigned char *sc = (lb.lane >= 0 && pl.lane_ws > pl.base_ws) ? scratch + pl.base_ws : scratch;
+        rc = largepath_project(lb.n, io_offset(io, lb.off), sc, pl.tiles_dev.at(lb.n), info + lb.idx, st);
+        if (rc) break;
+    }
+    if (lanes)                                           // always join: a capture must not be left forked
+        for (int l = 0; l < pl.n_lanes; ++l)
+            if (cudaEventRecord(ds.lane_join[l], ds.lane_stream[l]) != cudaSuccess || cudaStreamWaitEvent(st, ds.lane_join[l], 0) != cudaSuccess) rc_lane = HPSD_ECUDA;
+    return rc ? rc : rc_lane;
 }
 
 }  // namespace
@@ -276,6 +344,14 @@ int hpsd_set_option(const char *name, int value) {
     std::lock_guard<std::mutex> lk(g_mu);
     for (auto &kv : g_dev)                      // a captured call froze the options it ran with
         for (auto &pl : kv.second.plans) pl->drop_graphs();
+    if (std::strcmp(name, "large_lanes") == 0) {
+        g_opt.large_lanes = (value != 0);
+        return HPSD_OK;
+    }
+    if (std::strcmp(name, "medium_reroute") == 0) {
+        g_opt.medium_reroute = (value != 0);
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "graph_replay") == 0) {
         g_opt.graph_replay = (value != 0);
         return HPSD_OK;
@@ -339,14 +415,16 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     int rc = check_args(n_blocks, sizes, (void *)1, (void *)1, &total);
     if (rc) return rc;
     size_t ws = 0;
-    std::map<int, int> dc_count;
-    for (int b = 0; b < n_blocks; ++b) {
-        if (sizes[b] > small_limit(g_opt)) {
-            const size_t w = largepath_ws_bytes(sizes[b]);
-            if (w > ws) ws = w;
-        } else if (use_meddc(g_opt, sizes[b])) dc_count[sizes[b]]++;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);       // the options are read under the lock
+        for (int pass = 0; pass < 2; ++pass) {
+            Plan tmp;
+            std::vector<long long> ll;
+            std::vector<int> ints;
+            route_plan(n_blocks, sizes, tmp, pass == 0 ? tridiag_cluster_size_ok : cluster_never, ll, ints);
+            ws = std::max(ws, tmp.ws_bytes);
+        }
     }
-    for (auto &kv : dc_count) ws = std::max(ws, meddc_ws_bytes(kv.first, kv.second));
     *bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int) + 4, 256) + 256;
     return HPSD_OK;
 }
@@ -371,7 +449,7 @@ static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void 
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (!g_opt.graph_replay || g_profile || cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
         cudaGetLastError();
-        return run_plan(*pl, io, ws, info_dev, st);           // includes: the caller is capturing this call itself
+        return run_plan(ds, *pl, io, ws, info_dev, st);           // includes: the caller is capturing this call itself
     }
     GraphEntry *ge = nullptr;
     for (GraphEntry &g : pl->graphs)
@@ -392,25 +470,25 @@ static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void 
         GraphEntry g;
         g.in = io.in; g.sub = io.sub; g.out = io.out; g.vout = io.vout; g.ws = ws; g.info = info_dev; g.stamp = ++ds.stamp;
         pl->graphs.push_back(g);
-        return run_plan(*pl, io, ws, info_dev, st);
+        return run_plan(ds, *pl, io, ws, info_dev, st);
     }
     // second call with the same buffers: capture on the library's stream, replay on the caller's from now on
     if (!ds.cap_stream && cudaStreamCreateWithFlags(&ds.cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
         cudaGetLastError();
-        return run_plan(*pl, io, ws, info_dev, st);
+        return run_plan(ds, *pl, io, ws, info_dev, st);
     }
     if (cudaStreamBeginCapture(ds.cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
-        return run_plan(*pl, io, ws, info_dev, st);
+        return run_plan(ds, *pl, io, ws, info_dev, st);
     }
-    rc = run_plan(*pl, io, ws, info_dev, ds.cap_stream);
+    rc = run_plan(ds, *pl, io, ws, info_dev, ds.cap_stream);
     cudaGraph_t graph = nullptr;
     const cudaError_t ec = cudaStreamEndCapture(ds.cap_stream, &graph);
     if (rc || ec != cudaSuccess || !graph || cudaGraphInstantiate(&ge->exec, graph, 0) != cudaSuccess) {
         if (graph) cudaGraphDestroy(graph);
         ge->exec = nullptr;
         cudaGetLastError();
-        return rc ? rc : run_plan(*pl, io, ws, info_dev, st);
+        return rc ? rc : run_plan(ds, *pl, io, ws, info_dev, st);
     }
     cudaGraphDestroy(graph);
     ge->launches = g_launches;
@@ -575,6 +653,11 @@ int hpsd_release(void) {
         DeviceState &ds = it->second;
         ds.plans.clear();
         if (ds.cap_stream) { cudaStreamDestroy(ds.cap_stream); ds.cap_stream = nullptr; }
+        for (int l = 0; l < kLargeLanes; ++l) {
+            if (ds.lane_stream[l]) { cudaStreamDestroy(ds.lane_stream[l]); ds.lane_stream[l] = nullptr; }
+            if (ds.lane_join[l]) { cudaEventDestroy(ds.lane_join[l]); ds.lane_join[l] = nullptr; }
+        }
+        if (ds.lane_fork) { cudaEventDestroy(ds.lane_fork); ds.lane_fork = nullptr; }
         if (ds.ws) cudaFree(ds.ws);
         if (ds.stage_in) cudaFree(ds.stage_in);
         if (ds.stage_out) cudaFree(ds.stage_out);

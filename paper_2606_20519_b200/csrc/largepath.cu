@@ -82,9 +82,11 @@ struct Side {
     cudaEvent_t fork = nullptr, join = nullptr;
     int dev = -1;
 };
-thread_local Side g_side;
+constexpr int kSides = 1 + kLargeLanes;      // slot 0: the caller's stream, slots 1..: the lanes of concurrent blocks
+thread_local Side g_sides[kSides];
 
-bool side_ready() {
+bool side_ready(int slot) {
+    Side &g_side = g_sides[slot];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return false;
     if (g_side.st && g_side.dev == dev) return true;
@@ -144,14 +146,16 @@ int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *sc
     return 0;
 }
 
-int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st) {
+int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st, int lane) {
+    const int slot = (lane >= 0 && lane < kLargeLanes) ? lane + 1 : 0;
+    Side &g_side = g_sides[slot];
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
     w.s.info = info;
     int rc = reduce_to_tridiagonal(w, n, io.in, io.sub, st);
     if (rc) return rc;
     bool forked = false;
-    if (g_overlap_factors && side_ready() && cudaEventRecord(g_side.fork, st) == cudaSuccess &&
+    if (g_overlap_factors && side_ready(slot) && cudaEventRecord(g_side.fork, st) == cudaSuccess &&
         cudaStreamWaitEvent(g_side.st, g_side.fork, 0) == cudaSuccess) {
         rc = launch_bt_factors(w.b, g_side.st);
         forked = true;                                    // joined below even on error: a capture must not be left forked

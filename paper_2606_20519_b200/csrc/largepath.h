@@ -6,7 +6,10 @@ namespace hpsd {
 int largepath_init();
 size_t largepath_ws_bytes(int n);
 // One block: svec in -> svec out.  scratch >= largepath_ws_bytes(n), 256-byte aligned.
-int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st);
+// lane: -1 on the caller's stream; 0 .. kLargeLanes-1 when several blocks run next to each other on the library's lane
+// streams (each lane has its own side stream for the compact-WY factors and needs its own scratch)
+constexpr int kLargeLanes = 8;
+int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st, int lane = -1);
 // S1+S2+S3 only (diagnostic / eigenvalue-only entry points).
 int largepath_tridiag_only(int n, const double *in, double *d, double *e, unsigned char *scratch, const int2 *tiles, cudaStream_t st);
 // S1..S4: ascending eigenvalues only.

@@ -1,5 +1,5 @@
 // tridiag_cluster.cu -- S1 + S2 + S3 of SURVEY.md §8(a) for blocks whose lower triangle fits in the
-// shared memory of ONE 16-CTA thread-block cluster (n <= ~640: the paper's d = 5, n = 625 block).
+// shared memory of ONE 16-CTA thread-block cluster (n <= ~631: the paper's d = 5, n = 625 block).
 // svec -> REAL symmetric tridiagonal (d, e) + reflectors V, tau, same conventions as tridiag.cu:
 // A = Q T Q^H, Q = H_0 ... H_{n-2}, H_c = I - tau_c v_c v_c^H (zlarfg: complex tau, real beta).
 // "Eigendecomposition" of PAPER.md:1536 starts here; the design is ours (the paper calls a library).
@@ -94,7 +94,7 @@ __host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + 
 __host__ __device__ inline size_t cl_col_off(int n, int r, int jl) { return (size_t)jl * (n - r) - (size_t)8 * jl * (jl - 1); }
 
 struct ClusterSmem {
-    size_t mbar, tok, colv, q, red, rbuf, wbuf, stor, total;
+    size_t mbar, tok, colv, q, red, rbuf, wbuf, tpart, stor, total;
 };
 __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     ClusterSmem s;
@@ -107,9 +107,10 @@ __host__ __device__ inline ClusterSmem cl_smem(int n, int r) {
     s.q = off; off += sizeof(double) * 2 * kCl;    // v^H y partials, double-buffered by step parity
     s.red = off; off += sizeof(double) * (2 * kClWarps + 4);   // block-reduction scratch + alpha, d_c
     s.rbuf = off; off += sizeof(cplx) * kCl * (rs | 1);
-    s.wbuf = off;
-    const size_t wb = sizeof(cplx) * n, tp = sizeof(cplx) * kClWarps * nc;
-    off += wb > tp ? wb : tp;                      // wbuf is dead during the pass: aliased with the t_j partials
+    s.wbuf = off; off += sizeof(cplx) * n;
+    // the t_j partials must NOT share memory with wbuf: a reducer may broadcast tau y (into wbuf) as soon as IT has the
+    // contributions of its own rows, while another thread of this CTA is still reading t_j partials for a different row
+    s.tpart = off; off += sizeof(cplx) * kClWarps * nc;
     s.stor = off;
     off += sizeof(cplx) * cl_col_off(n, r, cl_ncols(n, r));
     s.total = off;
@@ -200,7 +201,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
     cplx *rbuf = reinterpret_cast<cplx *>(smem_raw + L.rbuf);                 // [sender][RSP]
     const int RS = (n + kCl - 1) / kCl, RSP = RS | 1;
     cplx *wbuf = reinterpret_cast<cplx *>(smem_raw + L.wbuf);
-    cplx *tpart = wbuf;                                               // [warp][ncw], alive only inside a step
+    cplx *tpart = reinterpret_cast<cplx *>(smem_raw + L.tpart);       // [warp][ncw]
     cplx *stor = reinterpret_cast<cplx *>(smem_raw + L.stor);
     const int nc = cl_ncols(n, r);
 
@@ -530,6 +531,9 @@ int tridiag_cluster_init() {
     g_cl_init_dev = dev;
     return 0;
 }
+
+// device-independent: the packed lower triangle of an n x n block fits in 16 x 227 KB (hpsd_workspace_size's bound)
+int tridiag_cluster_size_ok(int n) { return n >= kCl && n <= kClMaxN && cl_smem_max(n) <= (size_t)232448; }
 
 // 1 when a block of size n is served by the cluster kernel on this device
 int tridiag_cluster_fits(int n) {

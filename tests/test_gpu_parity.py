@@ -212,8 +212,14 @@ def test_medium_path_sizes(orc, hp, n):
     rng = np.random.default_rng(250 + n)
     sizes = [n] * 3
     sv = pack_all(orc, [herm(rng, n) for _ in sizes])
-    got, _ = check_vs_oracle(orc, hp, sizes, sv)
-    check_invariants(hp, sizes, sv, got)
+    hp.set_option("medium_reroute", 0)          # keep the one-CTA kernels on the path (3 blocks of 84..116 would be rerouted)
+    try:
+        got, _ = check_vs_oracle(orc, hp, sizes, sv)
+        check_invariants(hp, sizes, sv, got)
+    finally:
+        hp.set_option("medium_reroute", 1)
+    rerouted, _ = check_vs_oracle(orc, hp, sizes, sv)  # default dispatch (large path for few blocks of 84..116)
+    assert rel_err(rerouted, got) <= TOL * n
 
 
 @pytest.mark.parametrize("n,count", [(33, 1), (36, 5), (64, 2), (81, 7), (83, 1)])
@@ -223,12 +229,14 @@ def test_medium_path_in_cta_ql(orc, hp, n, count):
     rng = np.random.default_rng(260 + n)
     sizes = [n] * count
     sv = pack_all(orc, [herm(rng, n) for _ in sizes])
-    got_dc, _ = check_vs_oracle(orc, hp, sizes, sv)
-    hp.set_option("medium_dc", 0)
+    hp.set_option("medium_reroute", 0)
     try:
+        got_dc, _ = check_vs_oracle(orc, hp, sizes, sv)
+        hp.set_option("medium_dc", 0)
         got_ql, _ = check_vs_oracle(orc, hp, sizes, sv)
     finally:
         hp.set_option("medium_dc", 1)
+        hp.set_option("medium_reroute", 1)
     assert rel_err(got_ql, got_dc) <= TOL * n
 
 
@@ -249,8 +257,8 @@ def test_medium_kernel_on_small_sizes(orc, hp, n):
 @pytest.mark.parametrize("n", [2, 3, 31, 32, 33, 63, 64, 65, 85, 96, 127, 128, 129, 200, 257, 320])
 def test_large_path_sizes(orc, hp, n, cluster):
     """Force every block through S1..S8 of the Householder/D&C path (ragged tiles, several panels): with the
-    cluster-resident reduction (default for 16 <= n <= 638) and with the grid-wide panel kernel (cluster = 0), which
-    otherwise only serves n > 638."""
+    cluster-resident reduction (default for 16 <= n <= 631) and with the grid-wide panel kernel (cluster = 0), which
+    otherwise only serves n > 631."""
     rng = np.random.default_rng(300 + n)
     sv = orc.pack(herm(rng, n))
     force_large(hp, True)
@@ -468,7 +476,7 @@ def test_admm_step_fused(orc, hp):
     assert np.array_equal(t_v2.cpu().numpy(), t_v.cpu().numpy())
 
 
-@pytest.mark.parametrize("n", [117, 130, 255, 256, 257, 400, 625, 636])
+@pytest.mark.parametrize("n", [117, 130, 255, 256, 257, 400, 625, 631])
 def test_cluster_tridiag_kernel(orc, hp, n):
     """S1+S2+S3 by the cluster-resident kernel (tridiag_cluster.cu; option "cluster_tridiag", on by default).
     Whole-path parity against the oracle, (d, e) against the grid-wide panel kernel (same reflector convention,
@@ -541,3 +549,32 @@ def test_graph_replay_of_repeated_calls(orc, hp):
         u_ref, v_ref = orc.admm_step(sizes, sv1, v_ref, nthreads=orc.max_threads())
         assert rel_err(u.cpu().numpy(), u_ref) <= TOL * max(sizes), it
         assert rel_err(v.cpu().numpy(), v_ref) <= TOL * max(sizes), it
+
+
+def test_concurrent_lanes_of_cluster_sized_blocks(orc, hp):
+    """Option "large_lanes" (default 1): several blocks whose reduction runs on one 16-CTA cluster are processed next to
+    each other on internal lane streams.  Must equal the sequential result BIT FOR BIT on every repetition (eight
+    clusters of n = 625 at once once exposed a shared-memory aliasing race in the cluster kernel), through plain
+    launches and graph replay, and match the oracle; plus a mixed list with sequential (n > 631) and small blocks."""
+    import torch
+    rng = np.random.default_rng(88)
+    for n, count, reps in ((625, 8, 30), (116, 7, 10), (300, 3, 6)):
+        sizes = [n] * count
+        sv = pack_all(orc, [herm(rng, n, 1.0 / np.sqrt(n)) for _ in sizes])
+        hp.set_option("large_lanes", 0)
+        base = gpu_project(hp, sizes, sv)
+        hp.set_option("large_lanes", 1)
+        t_in = torch.from_numpy(sv).cuda()
+        t_out = torch.empty_like(t_in)
+        for it in range(reps):
+            t_out.zero_()
+            hp.project_(sizes, t_in, t_out)
+            if it % 3 == 0:
+                torch.cuda.synchronize()
+            assert np.array_equal(t_out.cpu().numpy(), base), (n, it)
+        if n != 625:
+            want = orc.project(sizes, sv, nthreads=orc.max_threads())
+            assert rel_err(base, want) <= TOL * n
+    sizes = [200, 700, 36, 150, 1, 36, 420]
+    sv = pack_all(orc, [herm(rng, n, 1.0 / np.sqrt(max(n, 1))) for n in sizes])
+    check_vs_oracle(orc, hp, sizes, sv, nthreads=orc.max_threads())
