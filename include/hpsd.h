@@ -134,9 +134,9 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *   "large_lanes" (0/1, default 1): two or more blocks of one call whose reduction runs on a single 16-CTA cluster
  *       (sizes up to ~631) are processed next to each other on up to 8 internal lane streams, each with its own part of
  *       the workspace (hpsd_workspace_size accounts for it); fork and join are events on the caller's stream.
- *   "medium_reroute" (0/1, default 1): a group of at most 5 blocks of one size in 84..116 (the in-CTA QL range), or a
- *       single block of size 64..83, goes through the large path (cluster-resident reduction) instead of the one-CTA
- *       medium kernels, which pay their latency once per group, not per block.
+ *   "medium_reroute" (0/1, default 1): a group of at most 32 blocks of one size in 84..116 (the in-CTA QL range), or of
+ *       at most 4 blocks of one size in 64..83, goes through the large path (cluster-resident reduction, lanes) instead
+ *       of the one-CTA medium kernels (5 and 1 blocks when "large_lanes" is off).
  *   "graph_replay" (0/1, default 1): the second call with the same size list AND the same buffers (an ADMM
  *       loop) is captured into a CUDA graph on an internal stream; that call and the following ones are one
  *       cudaGraphLaunch on the caller's stream (same kernels, same order).  Off while "profile" is on or when the

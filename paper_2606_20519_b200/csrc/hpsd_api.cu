@@ -163,12 +163,14 @@ void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*fits)(int), std:
     pl.scalar_off_index = ll.size();
     for (long long o : scalars) ll.push_back(o);
     for (auto &kv : by_n) {
-        // Few blocks of one medium size are faster one after the other through the large path, whose reduction runs on
-        // a 16-CTA cluster (measured on B200: n = 84..116, in-CTA QL 2.6-5.0 ms per GROUP up to 64 blocks against
-        // 0.50-0.73 ms per BLOCK; n = 64..83, one block: 0.63-0.65 against 0.49-0.56 ms)
+        // Few blocks of one medium size are faster through the large path, whose reduction runs on a 16-CTA cluster and
+        // whose blocks run on up to 8 lanes (measured on B200: n = 84..116, in-CTA QL 2.6-5.0 ms per GROUP of up to 64
+        // blocks against 0.5-0.75 ms per ROUND of 8 blocks; n = 64..83, batched D&C 0.65-0.68 ms per group against
+        // 0.52-0.58 ms for up to 4 blocks)
         const int gn = kv.first, gc = (int)kv.second.size();
-        if (g_opt.medium_reroute && gn > g_opt.jacobi_max_n && fits(gn) &&
-            ((gn > kMedDcMaxN || !g_opt.medium_dc) ? gc <= 5 : (gn >= 64 && gc == 1))) {
+        const bool in_cta_ql = gn > kMedDcMaxN || !g_opt.medium_dc;
+        const int max_count = in_cta_ql ? (g_opt.large_lanes ? 32 : 5) : (gn >= 64 ? (g_opt.large_lanes ? 4 : 1) : 0);
+        if (g_opt.medium_reroute && gn > g_opt.jacobi_max_n && fits(gn) && gc <= max_count) {
             for (auto &pr : kv.second) pl.large.push_back({gn, pr.first, pr.second});
             continue;
         }

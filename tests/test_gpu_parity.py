@@ -306,6 +306,8 @@ def test_degenerate_inputs(orc, hp, n, large):
     cases = _special_cases(rng, n)
     if large:
         force_large(hp, True)
+    else:
+        hp.set_option("medium_reroute", 0)      # keep the one-CTA kernels on the path (a single n = 81 block would be re-routed)
     try:
         for name, X in cases.items():
             X = 0.5 * (X + X.conj().T)
@@ -320,6 +322,7 @@ def test_degenerate_inputs(orc, hp, n, large):
                 np.testing.assert_allclose(got, np.maximum(sv, 0), rtol=8 * EPS, atol=0, err_msg=name)
     finally:
         force_large(hp, False)
+        hp.set_option("medium_reroute", 1)
 
 
 def test_n0_n1_and_empty_list(orc, hp):
@@ -561,17 +564,22 @@ def test_concurrent_lanes_of_cluster_sized_blocks(orc, hp):
     for n, count, reps in ((625, 8, 30), (116, 7, 10), (300, 3, 6)):
         sizes = [n] * count
         sv = pack_all(orc, [herm(rng, n, 1.0 / np.sqrt(n)) for _ in sizes])
-        hp.set_option("large_lanes", 0)
-        base = gpu_project(hp, sizes, sv)
-        hp.set_option("large_lanes", 1)
-        t_in = torch.from_numpy(sv).cuda()
-        t_out = torch.empty_like(t_in)
-        for it in range(reps):
-            t_out.zero_()
-            hp.project_(sizes, t_in, t_out)
-            if it % 3 == 0:
-                torch.cuda.synchronize()
-            assert np.array_equal(t_out.cpu().numpy(), base), (n, it)
+        force_large(hp, True)                     # the same route with and without lanes (the re-routing rule depends on them)
+        try:
+            hp.set_option("large_lanes", 0)
+            base = gpu_project(hp, sizes, sv)
+            hp.set_option("large_lanes", 1)
+            t_in = torch.from_numpy(sv).cuda()
+            t_out = torch.empty_like(t_in)
+            for it in range(reps):
+                t_out.zero_()
+                hp.project_(sizes, t_in, t_out)
+                if it % 3 == 0:
+                    torch.cuda.synchronize()
+                assert np.array_equal(t_out.cpu().numpy(), base), (n, it)
+        finally:
+            force_large(hp, False)
+            hp.set_option("large_lanes", 1)
         if n != 625:
             want = orc.project(sizes, sv, nthreads=orc.max_threads())
             assert rel_err(base, want) <= TOL * n
