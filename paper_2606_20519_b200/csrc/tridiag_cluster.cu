@@ -5,12 +5,12 @@
 // "Eigendecomposition" of PAPER.md:1536 starts here; the design is ours (the paper calls a library).
 //
 // Why: at n = 625 the grid-wide panel kernel is bound by two grid barriers per column (1.1-1.5 us
-// each on B200).  A cluster barrier costs ~0.2 us, and 16 x 227 KB of distributed
+// each on B200).  Exchanges inside a cluster are cheaper, and 16 x 227 KB of distributed
 // shared memory hold the whole packed lower triangle (3.1 MB at n = 625), so the matrix is read from
 // HBM exactly once (straight from the svec: S1 is fused) and every column step runs out of shared memory.
 //
 // Layout: column j belongs to CTA j mod 16 and is stored packed (rows j..n-1, contiguous).
-// Rows are owned by threads: row i = 32 (8 s + warp) + lane for register slot s < 3; each thread
+// Rows are owned by threads: three 32-row chunks per warp (cl_chunk: a light, a middle and a heavy one); each thread
 // keeps v_i, w_i, u_i of its rows in registers.
 //
 // Step c (unblocked, LAPACK zhetd2 arithmetic, one fused pass per column):
@@ -29,6 +29,9 @@
 // two-entry ring in global memory (L2): the CTA that stores column c+1 brings it up to date and exports it BEFORE
 // its pass, fences after the pass and sends one 8-byte token per warp to every CTA on the phase-1 mbarrier, so
 // nobody reads the ring before the export is visible and the fence is off the critical path.
+// Buffer and mbarrier-phase reuse is safe by construction, not by timing: phase tokens and the late
+// push of v^H y order the steps between CTAs, every thread reads before it sends, and nothing a peer may write early
+// shares memory with anything read late (the t_j partials once did: a race that eight concurrent clusters exposed).
 //
 // Measured on B200 (round 1), S1+S2+S3 alone: n = 200 0.70 ms (grid-wide panel kernel 1.31), n = 400 1.97 (2.70),
 // n = 625 3.93 (4.37).  Every warp walks a serial chain of ~10 trips of ~1500 cycles per column step (t_j warp
@@ -157,9 +160,8 @@ __device__ long long g_cltrace2[8 * 16 * 4];
 #define CLT2(pt) do {} while (0)
 #endif
 
-// One row chunk x kKT own columns of the fused pass.  x holds A(i, j_k) (zero where the element does not exist).
-// MASKED = false: all 32 rows lie strictly below every diagonal of the trip (no predicates at all).
-template <bool MASKED>
+// One row chunk x kKT own columns of the fused pass.  x holds A(i, j_k) (zero where the element does not exist), m says
+// where it exists.  Branch-free: masks are selects (a predicate-free variant behind a warp-uniform branch was slower).
 __device__ __forceinline__ void cl_elems(cplx (&x)[kKT], const bool (&m)[kKT], int i, int j0, cplx *const (&col)[kKT], int i0,
                                          cplx v, cplx w, cplx u, const cplx (&cv)[kKT], const cplx (&cw)[kKT], const cplx (&cu)[kKT],
                                          cplx &z, cplx (&tj)[kKT]) {
@@ -172,15 +174,11 @@ __device__ __forceinline__ void cl_elems(cplx (&x)[kKT], const bool (&m)[kKT], i
         xx.y = fma(-v.y, cw[k].x, xx.y); xx.y = fma(v.x, cw[k].y, xx.y);
         xx.y = fma(-w.y, cv[k].x, xx.y); xx.y = fma(w.x, cv[k].y, xx.y);
         cplx ut = u;
-        if (MASKED) {
-            const int j = j0 + kCl * k;
-            if (!m[k]) xx = mk(0.0, 0.0);
-            if (i == j) xx.y = 0.0;
-            if (i <= j) ut = mk(0.0, 0.0);
-            if (m[k]) col[k][i0] = xx;
-        } else {
-            col[k][i0] = xx;
-        }
+        const int j = j0 + kCl * k;
+        if (!m[k]) xx = mk(0.0, 0.0);
+        if (i == j) xx.y = 0.0;                                   // the diagonal stays real
+        if (i <= j) ut = mk(0.0, 0.0);                            // t_j sums the rows strictly below the diagonal
+        if (m[k]) col[k][i0] = xx;
         cfma(z, xx, cu[k]);
         cfma_conj(tj[k], xx, ut);
     }
@@ -368,7 +366,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 if (i0 + 31 < j0 || i0 >= n) continue;            // warp-uniform: nothing of this chunk in the trip
                 // (a predicate-free variant for chunks entirely below the diagonals was measured and dropped: the extra
                 // warp-uniform branch costs more than the ~11 select/compare instructions per element it saves)
-                cl_elems<true>(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
+                cl_elems(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
             }
             CLT2(2);
             // halving butterfly: kKT values x 32 lanes -> lane 32 q / kKT holds the total of column q
