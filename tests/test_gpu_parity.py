@@ -586,3 +586,60 @@ def test_concurrent_lanes_of_cluster_sized_blocks(orc, hp):
     sizes = [200, 700, 36, 150, 1, 36, 420]
     sv = pack_all(orc, [herm(rng, n, 1.0 / np.sqrt(max(n, 1))) for n in sizes])
     check_vs_oracle(orc, hp, sizes, sv, nthreads=orc.max_threads())
+
+
+def test_random_cone_lists(orc, hp):
+    """Seeded random cone lists across every route (scalars, Jacobi, one-CTA medium kernels, re-routed medium blocks,
+    cluster-sized blocks on lanes, panel-kernel blocks) and several matrix structures (dense, low-rank + noise, exact
+    repeated eigenvalues, diagonal, scaled by 1e-8 .. 1e8): per-block parity with the oracle on the first call, on the
+    captured call and on the graph replay."""
+    import torch
+    rng = np.random.default_rng(4242)
+
+    def rand_size():
+        k = rng.integers(0, 10)
+        if k == 0:
+            return 1
+        if k <= 2:
+            return int(rng.integers(2, 33))
+        if k <= 4:
+            return int(rng.integers(33, 117))
+        if k <= 7:
+            return int(rng.integers(117, 632))
+        if k == 8:
+            return int(rng.integers(632, 700))
+        return int(rng.choice([16, 36, 81]))
+
+    def rand_mat(n):
+        kind = rng.integers(0, 5)
+        h = herm(rng, n, 1.0 / np.sqrt(max(n, 1)))
+        if kind == 0 or n < 3:
+            return h
+        if kind == 1:
+            r = max(1, n // 20)
+            b = rng.standard_normal((n, r)) + 1j * rng.standard_normal((n, r))
+            return b @ b.conj().T / n + 1e-3 * h
+        if kind == 2:
+            q = workloads.haar_unitary(rng, n)
+            lam = np.repeat(rng.standard_normal(n // 8 + 1), 8)[:n]
+            x = (q * lam) @ q.conj().T
+            return 0.5 * (x + x.conj().T)
+        if kind == 3:
+            return np.diag(rng.standard_normal(n)).astype(complex)
+        return h * 10.0 ** int(rng.integers(-8, 9))
+
+    for _ in range(12):
+        sizes = [rand_size() for _ in range(int(rng.integers(1, 9)))]
+        sv = pack_all(orc, [rand_mat(n) for n in sizes])
+        want = orc.project(sizes, sv, nthreads=orc.max_threads())
+        t_in = torch.from_numpy(sv).cuda()
+        t_out = torch.empty_like(t_in)
+        for rep in range(3):
+            t_out.zero_()
+            hp.project_(sizes, t_in, t_out)
+            torch.cuda.synchronize()
+            got, off = t_out.cpu().numpy(), 0
+            for n in sizes:
+                sl = slice(off, off + n * n)
+                assert parity_err(got[sl], want[sl], sv[sl], n) <= TOL * max(n, 1), (sizes, n, rep)
+                off += n * n
