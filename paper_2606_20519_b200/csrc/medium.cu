@@ -100,14 +100,21 @@ __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int c = 0; c < n - 1; ++c) {
         const int m = n - c - 1;
+        // norm of the sub-column, alpha and the diagonal entry travel through ONE block barrier (red[0..7] partial
+        // norms, red[16..18] alpha and d_c; the next writes to these slots are several barriers away)
         double S = 0.0;
         for (int r = c + 2 + tid; r < n; r += kMedThreads) S += abs2(A[(size_t)c * ld + r]);
-        S = block_sum(S, sm.red);
-        const cplx alpha = A[(size_t)c * ld + c + 1];
+        S = warp_sum(S);
+        if (lane == 0) sm.red[warp] = S;
+        if (tid == 32) { const cplx al = A[(size_t)c * ld + c + 1]; sm.red[16] = al.x; sm.red[17] = al.y; sm.red[18] = A[(size_t)c * ld + c].x; }
+        __syncthreads();
+        S = 0.0;
+#pragma unroll
+        for (int k = 0; k < kMedThreads / 32; ++k) S += sm.red[k];
+        const cplx alpha = mk(sm.red[16], sm.red[17]);
         double beta; cplx tau, scale;
         med_householder(alpha, S, beta, tau, scale);
-        if (tid == 0) { sm.d[c] = A[(size_t)c * ld + c].x; sm.e[c] = beta; sm.tau[c] = tau; }
-        __syncthreads();                                   // alpha read by everyone before it is overwritten
+        if (tid == 0) { sm.d[c] = sm.red[18]; sm.e[c] = beta; sm.tau[c] = tau; }
         for (int r = c + 1 + tid; r < n; r += kMedThreads) {
             const cplx v = (r == c + 1) ? mk(1.0, 0.0) : scale * A[(size_t)c * ld + r];
             sm.x[r] = v;
@@ -129,8 +136,16 @@ __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
                 cfma_conj(q, sm.x[r], acc);                 // conj(v_r) y_r
             }
         }
-        q = block_sum(q, sm.red);
-        const double alphap = -0.5 * abs2(tau) * q.x;       // v^H A v is real
+        // v^H y (real): partials in red[8..15], one barrier, which also publishes y
+        {
+            const double qs = warp_sum(q.x);
+            if (lane == 0) sm.red[8 + warp] = qs;
+        }
+        __syncthreads();
+        double qsum = 0.0;
+#pragma unroll
+        for (int k = 0; k < kMedThreads / 32; ++k) qsum += sm.red[8 + k];
+        const double alphap = -0.5 * abs2(tau) * qsum;      // v^H A v is real
         for (int r = c + 1 + tid; r < n; r += kMedThreads) sm.y[r] = tau * sm.y[r] + alphap * sm.x[r];
         __syncthreads();
         // A22 -= v w^H + w v^H on the full trailing block: lane = row (its v_r, w_r stay in registers), warp = column
