@@ -91,3 +91,31 @@ def test_product_never_imports_oracle():
     otxt = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "hpsd_oracle.c")).read()
     assert not re.search(r"^\s*(import|from)\s+paper_2606_20519_b200\b", otxt, flags=re.M)
     assert '#include "' not in otxt
+
+
+def test_workspace_size_bounds_every_routing(lib):
+    """hpsd_workspace_size is host-only and must bound every plan a device can make (include/hpsd.h, options
+    "large_lanes", "medium_reroute"): lanes add one scratch area per concurrently processed cluster-sized block (up to 8),
+    re-routed medium blocks need the large path's scratch, and switching the options off never needs more."""
+    def ws(sizes):
+        arr = (ctypes.c_int * len(sizes))(*sizes)
+        sz = ctypes.c_size_t(0)
+        assert lib.hpsd_workspace_size(len(sizes), arr, ctypes.byref(sz)) == 0
+        return sz.value
+
+    one = ws([625])
+    assert ws([625, 625]) >= 2 * one - 4096                   # two lanes, two scratch areas
+    assert ws([625] * 8) >= 8 * one - 8 * 4096
+    assert ws([625] * 20) <= ws([625] * 8) + 4096             # at most 8 lanes
+    assert ws([700, 700]) < 2 * ws([700])                     # above the cluster limit: one after the other, one area
+    assert ws([100]) > 16 * 100 * 100                         # a single n = 100 block is re-routed to the large path
+    assert lib.hpsd_set_option(b"large_lanes", 0) == 0
+    try:
+        assert ws([625] * 8) <= ws([625]) + 4096
+    finally:
+        assert lib.hpsd_set_option(b"large_lanes", 1) == 0
+    assert lib.hpsd_set_option(b"medium_reroute", 0) == 0
+    try:
+        assert ws([100]) < 4096                               # the one-CTA kernel needs no scratch
+    finally:
+        assert lib.hpsd_set_option(b"medium_reroute", 1) == 0
