@@ -41,8 +41,10 @@ struct StoreEpi {      // C[i + j*ld] = acc
 };
 struct SubEpi {        // C[i + j*ld] -= acc
     cplx *C; int ld;
-    __device__ __forceinline__ void operator()(int i, int j, double re, double im) const {
-        cplx *c = C + (size_t)j * ld + i; cplx v = *c; v.x -= re; v.y -= im; *c = v;
+    static constexpr bool kRmw = true;
+    __device__ __forceinline__ cplx load(int i, int j) const { return C[(size_t)j * ld + i]; }
+    __device__ __forceinline__ void store(int i, int j, cplx v, double re, double im) const {
+        v.x -= re; v.y -= im; C[(size_t)j * ld + i] = v;
     }
 };
 

@@ -99,7 +99,12 @@ struct Acc {
     double im[CPLX ? MI : 1][CPLX ? NI : 1][2];
 };
 
-// Epilogue interface:  epi(row, col, re, im) called for every in-range element of the tile.
+// Epilogue interface:  epi(row, col, re, im) called for every in-range element of the tile; an epilogue that
+// declares `static constexpr bool kRmw = true` instead provides load(row, col) and store(row, col, old, re, im),
+// and the tile body issues the loads of a row of blocks together.
+template <class E, class = void> struct epi_is_rmw { static constexpr bool value = false; };
+template <class E> struct epi_is_rmw<E, decltype((void)E::kRmw)> { static constexpr bool value = true; };
+
 // LOWER: only tiles with (tile row block) >= (tile col block) are computed; the epilogue masks i<j.
 template <typename TA, typename TB, int LA, int LB, bool CONJA, bool CONJB, int MI, int NI, int WM, int WN, bool LOWER, int STAGES = kGemmStages, class Epi>
 __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int tile_m, int tile_n, unsigned char *smem_raw, Epi &epi) {
@@ -179,19 +184,47 @@ __device__ __forceinline__ void gemm_tile_body(const GemmProblem<TA, TB> &p, int
     cp_async_wait<0>();
 
     // epilogue: lane holds D[fr][2*fk + {0,1}] of each 8x8 block
+    if constexpr (epi_is_rmw<Epi>::value) {
+        // read-modify-write epilogues (C -= acc): a plain load/subtract/store per element is one dependent chain of
+        // 2 MI NI global round trips per thread (a store may alias the next load, so the compiler keeps the order).
+        // Here the 2 NI loads of one row of blocks are issued together, then their stores: MI round trips.
 #pragma unroll
-    for (int i = 0; i < MI; ++i)
+        for (int i = 0; i < MI; ++i) {
+            const int row = m0 + wm * MI * 8 + i * 8 + fr;
+            decltype(epi.load(0, 0)) old[NI][2];
 #pragma unroll
-        for (int j = 0; j < NI; ++j)
+            for (int j = 0; j < NI; ++j)
 #pragma unroll
-            for (int c = 0; c < 2; ++c) {
-                const int row = m0 + wm * MI * 8 + i * 8 + fr;
-                const int col = n0 + wn * NI * 8 + j * 8 + 2 * fk + c;
-                if (row < p.M && col < p.N && (!LOWER || row >= col)) {
-                    if constexpr (CC) epi(row, col, acc.re[i][j][c], acc.im[i][j][c]);
-                    else epi(row, col, acc.re[i][j][c], 0.0);
+                for (int c = 0; c < 2; ++c) {
+                    const int col = n0 + wn * NI * 8 + j * 8 + 2 * fk + c;
+                    if (row < p.M && col < p.N && (!LOWER || row >= col)) old[j][c] = epi.load(row, col);
                 }
-            }
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const int col = n0 + wn * NI * 8 + j * 8 + 2 * fk + c;
+                    if (row < p.M && col < p.N && (!LOWER || row >= col)) {
+                        if constexpr (CC) epi.store(row, col, old[j][c], acc.re[i][j][c], acc.im[i][j][c]);
+                        else epi.store(row, col, old[j][c], acc.re[i][j][c], 0.0);
+                    }
+                }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < MI; ++i)
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const int row = m0 + wm * MI * 8 + i * 8 + fr;
+                    const int col = n0 + wn * NI * 8 + j * 8 + 2 * fk + c;
+                    if (row < p.M && col < p.N && (!LOWER || row >= col)) {
+                        if constexpr (CC) epi(row, col, acc.re[i][j][c], acc.im[i][j][c]);
+                        else epi(row, col, acc.re[i][j][c], 0.0);
+                    }
+                }
+    }
 }
 
 template <typename TA, typename TB, int LA, int LB, int MI, int NI, int WM, int WN, int STAGES = kGemmStages>

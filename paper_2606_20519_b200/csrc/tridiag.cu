@@ -557,12 +557,12 @@ static size_t panel_smem_bytes() {
 // ---------------------------------------------------------------- HER2K (DMMA)
 struct Her2kEpi {
     cplx *C; int ldc;
-    __device__ __forceinline__ void operator()(int i, int j, double re, double im) const {
-        cplx *c = C + (size_t)j * ldc + i;
-        cplx v = *c;
+    static constexpr bool kRmw = true;
+    __device__ __forceinline__ cplx load(int i, int j) const { return C[(size_t)j * ldc + i]; }
+    __device__ __forceinline__ void store(int i, int j, cplx v, double re, double im) const {
         v.x -= re; v.y -= im;
         if (i == j) v.y = 0.0;
-        *c = v;
+        C[(size_t)j * ldc + i] = v;
     }
 };
 
