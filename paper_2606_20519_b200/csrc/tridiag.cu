@@ -51,7 +51,7 @@ struct PanelArgs {
 };
 
 #ifdef HPSD_PANEL_TRACE
-// dev-only: per-column phase timestamps of CTA 0 and CTA G/2 (clock64), first traced launch only
+// dev-only: per-column phase timestamps of CTA 0 and CTA G/2 (clock64) of panel number (armed - 1)
 __device__ long long g_trace[2 * 32 * 16];
 __device__ int g_trace_armed = 0;
 #define TRACE(slot)                                                                                   \
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     const int n = p.n, lda = p.lda, ldw = p.ldw, ldp = p.ldp;
     cplx *A = p.A, *W = p.W;
 #ifdef HPSD_PANEL_TRACE
-    const bool trace_on = (tid == 0 && g_trace_armed == 1 && p.j0 == 0 && (g == 0 || g == G / 2));
+    const bool trace_on = (tid == 0 && g_trace_armed >= 1 && p.j0 == (g_trace_armed - 1) * kNB && (g == 0 || g == G / 2));
 #endif
     constexpr int PSTRIDE = 2 * kNB + 1;
     const int T = p.T, q = p.q;
@@ -438,19 +438,20 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     if (lane + 96 < nq) qv3 = ldx_(&p.qpart[lane + 96]);
                     for (int k = lane + 128; k < nq; k += 32) qv4 += ldx_(&p.qpart[k]);
                 }
+                // cV, cW are the same 2 x 32 values for every warp of every CTA: one warp fetches them with two coalesced
+                // loads and hands them over in shared memory (a load per warp and value made these 8 lines the hottest
+                // in L2: ~1000 requests per line per column at n = 4096, queued for microseconds)
+                cplx totV = mk(0.0, 0.0), totW = mk(0.0, 0.0);
+                if (warp == 2 && lane < i) { totV = ldx_(&p.tot[lane]); totW = ldx_(&p.tot[kNB + lane]); }
                 TRACE(8);
-                cplx Vr[kNB / 8], Wr[kNB / 8], cv[kNB / 8], cw[kNB / 8];
+                cplx Vr[kNB / 8], Wr[kNB / 8];
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
                     const int t = warp + 8 * k;
-                    Vr[k] = mk(0.0, 0.0); Wr[k] = mk(0.0, 0.0); cv[k] = mk(0.0, 0.0); cw[k] = mk(0.0, 0.0);
-                    if (t < i) {
-                        if (ok) {
-                            Vr[k] = ldx_(&A[(size_t)(p.j0 + t) * lda + r]);
-                            Wr[k] = ldx_(&W[(size_t)t * ldw + r]);
-                        }
-                        cv[k] = ldx_(&p.tot[t]);
-                        cw[k] = ldx_(&p.tot[kNB + t]);
+                    Vr[k] = mk(0.0, 0.0); Wr[k] = mk(0.0, 0.0);
+                    if (t < i && ok) {
+                        Vr[k] = ldx_(&A[(size_t)(p.j0 + t) * lda + r]);
+                        Wr[k] = ldx_(&W[(size_t)t * ldw + r]);
                     }
                 }
                 cplx p1 = mk(0.0, 0.0);
@@ -474,23 +475,25 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 TRACE_USE(p1.x);
                 TRACE(11);
                 if (warp == 1) qv = warp_sum((qv0 + qv1) + (qv2 + qv3) + qv4);
+                if (warp == 2) { s_cV[lane] = totV; s_cW[lane] = totW; }
+                __syncthreads();                                  // cV, cW visible; previous pass / previous column readers done
                 // ---- partial sums of this warp: y - V cW - W cV,  V conj(W[c+1,:]) + W conj(V[c+1,:]),  Re(cV^H cW)
                 cplx p2 = mk(0.0, 0.0);
                 double re = 0.0;
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
                     if (warp + 8 * k >= i) continue;             // warp-uniform
+                    const cplx cvk = s_cV[warp + 8 * k], cwk = s_cW[warp + 8 * k];
                     // rows c+1 of V and W sit in the helper lane
                     const cplx v1 = mk(__shfl_sync(0xffffffffu, Vr[k].x, 31), __shfl_sync(0xffffffffu, Vr[k].y, 31));
                     const cplx w1 = mk(__shfl_sync(0xffffffffu, Wr[k].x, 31), __shfl_sync(0xffffffffu, Wr[k].y, 31));
                     cplx corr = mk(0.0, 0.0);
-                    cfma(corr, Vr[k], cw[k]); cfma(corr, Wr[k], cv[k]);
+                    cfma(corr, Vr[k], cwk); cfma(corr, Wr[k], cvk);
                     p1 = p1 - corr;
                     cfma(p2, Vr[k], conj_(w1)); cfma(p2, Wr[k], conj_(v1));
-                    re += cv[k].x * cw[k].x + cv[k].y * cw[k].y;
+                    re += cvk.x * cwk.x + cvk.y * cwk.y;
                 }
                 TRACE(4);
-                __syncthreads();                                  // previous pass / previous column readers done
                 s_p1[warp * 32 + lane] = p1;
                 s_p2[warp * 32 + lane] = p2;
                 if (lane == 0) s_re[warp] = re;
