@@ -116,8 +116,9 @@ __global__ void __launch_bounds__(BG_THREADS) bt_vt_kernel(BackWs w) {
 }
 
 // X_part[s] = V_b^H Z over the s-th chunk of rows (blockIdx.x = column tile, blockIdx.y = s, blockIdx.z = row tile)
-template <int MI, int NI>
-__global__ void __launch_bounds__(BG_THREADS) bt_vhz_kernel(BackWs w, int b) {
+// ST = 2: two CTAs (eight warps) per SM; three stages of the 64 x 64 instance need 122 KB of shared memory, one CTA per SM
+template <int MI, int NI, int ST = kGemmStages>
+__global__ void __launch_bounds__(BG_THREADS, (ST == 2 ? 2 : 1)) bt_vhz_kernel(BackWs w, int b) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
@@ -131,7 +132,7 @@ __global__ void __launch_bounds__(BG_THREADS) bt_vhz_kernel(BackWs w, int b) {
     p.B = w.Zc + cb + 1 + k0; p.ldb = w.ldz;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = kpos; p.K = klen > 0 ? klen : 0; p.K2 = 0;
     StoreEpi epi{w.Xp + (size_t)blockIdx.y * kNBT * w.n, kNBT};
-    gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, MI, NI, BG_WM, BG_WN, false>(p, blockIdx.z, blockIdx.x, smem_raw, epi);
+    gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, MI, NI, BG_WM, BG_WN, false, ST>(p, blockIdx.z, blockIdx.x, smem_raw, epi);
 }
 
 __global__ void __launch_bounds__(256) bt_reduce_kernel(BackWs w) {
@@ -184,6 +185,7 @@ __global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, SvecIo 
 // ---- host driver -------------------------------------------------------------------------------
 static int g_bh_init_dev = -1;
 constexpr size_t kSmemKK = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
+constexpr size_t kSmemKK2 = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN, 2>();
 constexpr size_t kSmemMK = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN>();
 constexpr size_t kSmemMK2 = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, BG_MI, BG_NI, BG_WM, BG_WN, 2>();
 constexpr size_t kSmemKKs = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, 2, 2, BG_WM, BG_WN>();
@@ -198,6 +200,7 @@ int backherk_init() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_tfactor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(cplx) * kNBT * kNBT));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<4, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKK2);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vhz_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemKKs);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_update_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMKs);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bt_vt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMK);
@@ -245,6 +248,7 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
         const int m = n - b * kNBT - 1;
         if (m <= 0) continue;
         if (small) bt_vhz_kernel<2, 2><<<dim3((n + 31) / 32, kSplitK, 2), BG_THREADS, kSmemKKs, st>>>(w, b);
+        else if (n >= 3072) bt_vhz_kernel<4, 4, 2><<<dim3(nt, kSplitK, 1), BG_THREADS, kSmemKK2, st>>>(w, b);   // > 148 live CTAs: two per SM
         else bt_vhz_kernel<4, 4><<<dim3(nt, kSplitK, 1), BG_THREADS, kSmemKK, st>>>(w, b);
         HPSD_LAUNCH_CHECK();
         bt_reduce_kernel<<<(kNBT * n + 255) / 256 < 1184 ? (kNBT * n + 255) / 256 : 1184, 256, 0, st>>>(w);
