@@ -104,19 +104,56 @@ __device__ __forceinline__ int producers(int rows, int G) {
     return l == 31 ? (rows + 30) / 31 : (rows + l - 1) / l;
 }
 
-// One warp copies tile (I, J) of A into a shared-memory slot (zero fill outside the matrix).
-__device__ __forceinline__ void warp_load_tile(cplx *slot, const cplx *__restrict__ A, int lda, int n, int2 ij, int lane) {
-    const int r = ij.x * kTS + lane, c0 = ij.y * kTS;
+// ---- mbarrier / bulk-copy helpers (each tile slot has an mbarrier that one load completes one phase of)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned mbar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned mbar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(mbar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+
+// One warp copies tile (I, J) of A into a shared-memory slot and completes one phase of the slot's mbarrier.
+// Full tiles: one 512-byte bulk copy (TMA engine) per column, issued by lane = column; the LSU path (cp.async, 16 bytes
+// per thread) caps the bytes an SM keeps in flight, which is what bounded the streaming regime.  Edge tiles (zero fill
+// outside the matrix): cp.async, waited for here.
+__device__ __forceinline__ void warp_load_tile(cplx *slot, unsigned mbar, const cplx *__restrict__ A, int lda, int n, int2 ij, int lane) {
+    const int r0 = ij.x * kTS, c0 = ij.y * kTS;
+    if (r0 + kTS <= n && c0 + kTS <= n) {                  // warp-uniform
+        if (lane == 0) mbar_arrive_expect_tx(mbar, kTS * kTS * (unsigned)sizeof(cplx));
+        __syncwarp();
+        bulk_g2s(smem_u32(slot + lane * kTP), A + (size_t)(c0 + lane) * lda + r0, kTS * (unsigned)sizeof(cplx), mbar);
+        return;
+    }
+    const int r = r0 + lane;
     const bool rok = r < n;
 #pragma unroll 8
     for (int cc = 0; cc < kTS; ++cc) {
         const bool ok = rok && (c0 + cc < n);
         cp_async_16(slot + cc * kTP + lane, ok ? A + (size_t)(c0 + cc) * lda + r : A, ok);
     }
-}
-
-__device__ __forceinline__ void cp_async_wait_dyn(int pending) {
-    if (pending <= 0) cp_async_wait<0>(); else cp_async_wait<1>();
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(mbar);
 }
 
 __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelArgs p) {
@@ -133,6 +170,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     cplx *s_sc = s_gW + 8 * kNB;                               // [0]=tau [1]=scale [2]=w_{c+1}
     double *s_S = reinterpret_cast<double *>(s_sc + 4);        // 8
     double *s_q = s_S + 8;                                     // 8 (+1: total)
+    const unsigned mbar0 = smem_u32(s_q + 12);                 // kSlots mbarriers (8 bytes each), one per tile slot
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = blockIdx.x, G = p.G;
@@ -149,16 +187,15 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     // ---------------- tile slots: this warp owns slots `warp` and (for warps 0..3) `warp + 8` ---------
     // tile k of this CTA is tiles[g + k G]; it lives in slot k % kSlots, served by warp (k % kSlots) % 8.
     const int nsl = (warp + 8 < kSlots) ? 2 : 1;
-    int issued = 0;
-    int ready_seq[2] = {0, 0};
+    if (threadIdx.x < kSlots) mbar_init(mbar0 + 8u * threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async;" ::: "memory");
+    __syncthreads();
+    unsigned ph[2] = {0u, 0u};           // parity of the latest load into this warp's slot h (waiting on it again is free)
     for (int h = 0; h < nsl; ++h) {
         const int k = warp + 8 * h;
         const int idx = g + k * G;
-        if (k < q && idx < T) {
-            warp_load_tile(s_slots + (size_t)k * kSlotElems, A, lda, n, p.tiles[idx], lane);
-            cp_async_commit();
-            ready_seq[h] = ++issued;
-        }
+        if (k < q && idx < T) warp_load_tile(s_slots + (size_t)k * kSlotElems, mbar0 + 8u * k, A, lda, n, p.tiles[idx], lane);
     }
 
     // this warp's tiles in sequence order j = 0..cnt-1: k(j) = (j / nsl) kSlots + warp + 8 (j % nsl), ascending in j
@@ -196,7 +233,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             p.part[(size_t)g * PSTRIDE] = mk(t, 0.0);
         }
     }
-    if (wide) cp_async_wait<0>();      // the slots are read by other warps in wide mode
+    // wide mode: the slots are read by other warps; every reader waits for its slot's (only) load itself
+    if (wide && (warp >> 2) < q && g + (warp >> 2) * G < T) mbar_wait(mbar0 + 8u * (warp >> 2), 0u);
     grid.sync();
 
     for (int i = 0; i < p.nbp; ++i) {
@@ -339,7 +377,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         __syncwarp();
                         vI[lane] = a; vJ[lane] = b;
                     }
-                    cp_async_wait_dyn(issued - ready_seq[h]);
+                    mbar_wait(mbar0 + 8u * (k % kSlots), ph[h]);
                     __syncwarp();
                     const cplx *sl = s_slots + (size_t)(k % kSlots) * kSlotElems;
                     // two independent accumulator sets (even / odd columns) halve the dependent DFMA chains
@@ -384,9 +422,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         if (jn >= 0 && jn < cnt) {
                             const int kn = (jn / nsl) * kSlots + warp + 8 * h;
                             __syncwarp();
-                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, A, lda, n, p.tiles[g + kn * G], lane);
-                            cp_async_commit();
-                            ready_seq[h] = ++issued;
+                            ph[h] ^= 1u;
+                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, mbar0 + 8u * (k % kSlots), A, lda, n, p.tiles[g + kn * G], lane);
                         }
                     }
                 }
@@ -550,11 +587,15 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         if (i + 1 < p.nbp) grid.sync();
         TRACE(7);
     }
-    cp_async_wait<0>();
+    // no bulk copy may be in flight when the CTA exits (a one-column last panel never reads its tiles)
+    for (int h = 0; h < nsl; ++h) {
+        const int k = warp + 8 * h;
+        if (k < q && g + k * G < T) mbar_wait(mbar0 + 8u * k, ph[h]);
+    }
 }
 
 static size_t panel_smem_bytes() {
-    return sizeof(cplx) * (size_t)(kSlots * kSlotElems + 8 * 2 * kTS + 4 * kNB + 16 * kNB + 4) + sizeof(double) * 20;
+    return sizeof(cplx) * (size_t)(kSlots * kSlotElems + 8 * 2 * kTS + 4 * kNB + 16 * kNB + 4) + sizeof(double) * (20 + kSlots);
 }
 
 // ---------------------------------------------------------------- HER2K (DMMA)
