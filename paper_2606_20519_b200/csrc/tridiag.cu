@@ -249,7 +249,14 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         // wide mode (at most two tiles per CTA): four warps share a tile, eight columns each
         const int wtile = warp >> 2, wq = warp & 3;
         const bool wvalid = wide && wtile < q && g + wtile * G < T;
+        // coordinates of this warp's tile number jj of the pass (pass order: forwards or backwards through its sequence)
+        auto tile_of = [&](int jj) -> int2 {
+            const int j = fwd ? jj : cnt - 1 - jj;
+            const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
+            return (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
+        };
         cplx rawI[2], rawJ[2];
+        int2 ijq[3] = {make_int2(0, 0), make_int2(0, 0), make_int2(0, 0)};     // coordinates of tiles jj, jj + 1, jj + 2
 #pragma unroll
         for (int jj = 0; jj < 2; ++jj) {
             rawI[jj] = mk(0.0, 0.0); rawJ[jj] = mk(0.0, 0.0);
@@ -261,14 +268,14 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[0] = ldx_(&A[(size_t)c * lda + rJ]);
                 }
             } else if (jj < cnt) {
-                const int j = fwd ? jj : cnt - 1 - jj;
-                const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
-                const int2 ij = (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
+                const int2 ij = tile_of(jj);
+                ijq[jj] = ij;
                 const int rI = ij.x * kTS + lane, rJ = ij.y * kTS + lane;
                 if (rI < n && rI > c + 1) rawI[jj] = ldx_(&A[(size_t)c * lda + rI]);
                 if (ij.x != ij.y && rJ < n && rJ > c + 1) rawJ[jj] = ldx_(&A[(size_t)c * lda + rJ]);
             }
         }
+        if (!wide && cnt > 2) ijq[2] = tile_of(2);
         const int nprod = producers(n - c, G);          // CTAs that left partials for this column
         // warp 0: Householder scalars from the partial norms
         if (warp == 0) {
@@ -354,24 +361,30 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         } else {
             cplx *vI = s_v + warp * 2 * kTS, *vJ = vI + kTS;
             {
+                // the tile coordinates run three tiles and the pieces of column c two tiles ahead of the tile in work: a
+                // tile used to start with two dependent L2 round trips (coordinates, then the column pieces)
                 for (int jj = 0; jj < cnt; ++jj) {
                     const int j = fwd ? jj : cnt - 1 - jj;
                     const int h = j % nsl;
                     const int k = (j / nsl) * kSlots + warp + 8 * h;
-                    const int2 ij = (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
+                    const int2 ij = ijq[0];
                     const int r0 = ij.x * kTS, c0 = ij.y * kTS;
                     const bool diag = (ij.x == ij.y);
+                    int2 ij3 = make_int2(0, 0);
+                    if (jj + 3 < cnt) ij3 = tile_of(jj + 3);
+                    cplx nxtI = mk(0.0, 0.0), nxtJ = mk(0.0, 0.0);
+                    if (jj + 2 < cnt) {
+                        const int rI = ijq[2].x * kTS + lane, rJ = ijq[2].y * kTS + lane;
+                        if (rI < n && rI > c + 1) nxtI = ldx_(&A[(size_t)c * lda + rI]);
+                        if (ijq[2].x != ijq[2].y && rJ < n && rJ > c + 1) nxtJ = ldx_(&A[(size_t)c * lda + rJ]);
+                    }
+                    const int2 ijrefill = (nsl == 2) ? ijq[2] : ijq[1];      // the tile nsl further on in this pass
                     // v pieces (formed on the fly; zero outside the trailing matrix)
                     {
                         const int rI = r0 + lane, rJ = c0 + lane;
-                        cplx a, b;
-                        if (jj == 0) { a = rawI[0]; b = rawJ[0]; }
-                        else if (jj == 1) { a = rawI[1]; b = rawJ[1]; }
-                        else {
-                            a = mk(0.0, 0.0); b = mk(0.0, 0.0);
-                            if (rI < n && rI > c + 1) a = ldx_(&A[(size_t)c * lda + rI]);
-                            if (!diag && rJ < n && rJ > c + 1) b = ldx_(&A[(size_t)c * lda + rJ]);
-                        }
+                        cplx a = rawI[0], b = rawJ[0];
+                        rawI[0] = rawI[1]; rawJ[0] = rawJ[1]; rawI[1] = nxtI; rawJ[1] = nxtJ;
+                        ijq[0] = ijq[1]; ijq[1] = ijq[2]; ijq[2] = ij3;
                         a = (rI == c + 1) ? mk(1.0, 0.0) : scale * a;
                         b = diag ? a : ((rJ == c + 1) ? mk(1.0, 0.0) : scale * b);
                         __syncwarp();
@@ -423,7 +436,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                             const int kn = (jn / nsl) * kSlots + warp + 8 * h;
                             __syncwarp();
                             ph[h] ^= 1u;
-                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, mbar0 + 8u * (k % kSlots), A, lda, n, p.tiles[g + kn * G], lane);
+                            (void)kn;
+                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, mbar0 + 8u * (k % kSlots), A, lda, n, ijrefill, lane);
                         }
                     }
                 }
