@@ -427,7 +427,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         p.PC[(size_t)ij.x * ldp + c0 + lane] = accC;
                         qterm = 2.0 * (vI[lane].x * accR.x + vI[lane].y * accR.y);
                     }
-                    qacc += warp_sum(qterm);
+                    qacc += qterm;                    // per lane; one warp reduction after the pass
                     if (streaming) {
                         // refill this slot with the tile that uses it next in this pass; at the end of a pass
                         // the slot keeps its tile, which is the first one the reversed next pass needs
@@ -443,6 +443,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 }
             }
         }
+        if (!wide) qacc = warp_sum(qacc);
         if (lane == 0) s_q[warp] = qacc;
         TRACE(2);
         __syncthreads();
