@@ -80,11 +80,11 @@ def measured_hbm_gbs():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu
-# --set full captures (profiles/r1_tuned_ncu_full.md); None where no capture exists for that workload
+# --set full captures (profiles/r1_*_ncu_full.md); None where no capture exists for that workload
 NCU_TRAFFIC = {
     ("S1S2S3_tridiag_cluster", 3): {"bytes_per_launch": 3.17e6, "source": "profiles/r1_cluster_ncu_full.md (n=625, whole reduction in one launch)"},
     ("S2S3_tridiag_panel", 3): {"bytes_per_launch": 2.82e6, "source": "profiles/r1_tuned_ncu_full.md (first panel, n=625)"},
-    ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.24e9, "source": "profiles/r1_tuned_ncu_full.md (first panels, n=4096)"},
+    ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.23e9, "source": "profiles/r1_final_ncu_full.md (first panels, n=4096)"},
     ("S10_householder_ql", 2): {"bytes_per_launch": 1.35e7, "source": "profiles/r1_tuned_ncu_full.md (256 x n=81)"},
 }
 
