@@ -7,8 +7,9 @@
 //   * panel of NB = 32 columns in ONE persistent cooperative kernel, two grid barriers per column.
 //     The trailing matrix is NOT modified inside a panel, so its 32 x 32 tiles are distributed over
 //     the shared memory of all SMs ONCE per panel (12 slots of 16.5 KB per CTA: 28 MB over 148 SMs,
-//     i.e. trailing sizes up to ~1880 stay resident; larger ones stream through the same slots
-//     with per-warp cp.async rings that prefetch across the grid barrier).
+//     i.e. trailing sizes up to ~1880 stay resident; larger ones stream through the same slots:
+//     each pair of warps runs a ring of three slots filled by 512-byte bulk copies (TMA engine, one
+//     mbarrier per slot) that keeps its last tiles across the grid barrier).
 //     Phase A (per column): every warp multiplies its own tiles by the Householder vector
 //       (y = A22 v, row parts and column parts of the stored lower triangle), no block-level sync.
 //     Phase B: rows are spread over the CTAs; y is assembled from the tile partials, w is formed,
@@ -184,32 +185,42 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     const bool streaming = q > kSlots;
     const bool wide = q <= 2;                       // block-uniform
 
-    // ---------------- tile slots: this warp owns slots `warp` and (for warps 0..3) `warp + 8` ---------
-    // tile k of this CTA is tiles[g + k G]; it lives in slot k % kSlots, served by warp (k % kSlots) % 8.
-    const int nsl = (warp + 8 < kSlots) ? 2 : 1;
-    if (threadIdx.x < kSlots) mbar_init(mbar0 + 8u * threadIdx.x, 1);
+    // ---------------- tile slots: warps p and p + 4 (a pair) share the slots p, p + 4, p + 8 as a ring of three ---------
+    // tile k of this CTA is tiles[g + k G]; the pair's tiles are t = 0, 1, 2, ... with k(t) = (t / 3) kSlots + p + 4 (t % 3),
+    // tile t lives in slot p + 4 (t % 3).  In pass order (forwards on even, backwards on odd columns) the two warps take
+    // alternate positions P = 2 jj + m; whoever finishes position P refills its slot with the tile of position P + 3,
+    // which the OTHER warp consumes.  So all eight warps carry the same number of tiles and every load has a whole tile
+    // time to arrive (before: warps 0..3 owned two slots and did two thirds of the tiles, warps 4..7 one slot, no prefetch).
+    const int pr_p = warp & 3, pr_m = warp >> 2;
+    auto kpair = [&](int t) { return (t / 3) * kSlots + pr_p + 4 * (t % 3); };
+    volatile int *s_iss = reinterpret_cast<volatile int *>(s_q + 12 + kSlots);     // loads issued so far into each slot
+    if (threadIdx.x < kSlots) { mbar_init(mbar0 + 8u * threadIdx.x, 1); s_iss[threadIdx.x] = 1; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
     __syncthreads();
-    unsigned ph[2] = {0u, 0u};           // parity of the latest load into this warp's slot h (waiting on it again is free)
-    for (int h = 0; h < nsl; ++h) {
-        const int k = warp + 8 * h;
-        const int idx = g + k * G;
-        if (k < q && idx < T) warp_load_tile(s_slots + (size_t)k * kSlotElems, mbar0 + 8u * k, A, lda, n, p.tiles[idx], lane);
-    }
-
-    // this warp's tiles in sequence order j = 0..cnt-1: k(j) = (j / nsl) kSlots + warp + 8 (j % nsl), ascending in j
-    int cnt = 0;
-    for (int j = 0;; ++j) {
-        const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
+    int pcnt = 0;                           // tiles of this pair
+    for (int t = 0;; ++t) {
+        const int k = kpair(t);
         if (k >= q || g + k * G >= T) break;
-        cnt = j + 1;
+        pcnt = t + 1;
     }
-
-    // tile coordinates of this warp's first two tiles (all of them in the resident regimes), read once
-    int2 ijc[2] = {make_int2(0, 0), make_int2(0, 0)};
+    const int cnt = (pcnt + 1 - pr_m) / 2;  // positions of this warp in a pass
+    // coordinates of the pair's first three tiles (all of them in the resident regimes), read once
+    int2 ijc[3] = {make_int2(0, 0), make_int2(0, 0), make_int2(0, 0)};
     if (wide) { if ((warp >> 2) < q && g + (warp >> 2) * G < T) ijc[0] = p.tiles[g + (warp >> 2) * G]; }
-    else { for (int j = 0; j < 2 && j < cnt; ++j) ijc[j] = p.tiles[g + ((j / nsl) * kSlots + warp + 8 * (j % nsl)) * G]; }
+    else {
+#pragma unroll
+        for (int t = 0; t < 3; ++t) if (t < pcnt) ijc[t] = p.tiles[g + kpair(t) * G];
+    }
+    if (wide) {           // slots 0 and 1 (tiles 0 and 1), loaded by warps 0 and 1, read by four warps each
+        if (warp < 2 && warp < q && g + warp * G < T) warp_load_tile(s_slots + (size_t)warp * kSlotElems, mbar0 + 8u * warp, A, lda, n, p.tiles[g + warp * G], lane);
+    } else {
+#pragma unroll
+        for (int t = 0; t < 3; ++t)
+            if (t < pcnt && (t & 1) == pr_m)
+                warp_load_tile(s_slots + (size_t)(pr_p + 4 * t) * kSlotElems, mbar0 + 8u * (pr_p + 4 * t), A, lda, n, ijc[t], lane);
+    }
+    unsigned base0 = 1u, base1 = 1u, base2 = 1u;     // loads issued into the pair's three slots before the current pass
 
     // ---------------- panel start: d[j0] and the partial norm of column j0 (already fully updated) -----
     {
@@ -250,11 +261,11 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         const int wtile = warp >> 2, wq = warp & 3;
         const bool wvalid = wide && wtile < q && g + wtile * G < T;
         // coordinates of this warp's tile number jj of the pass (pass order: forwards or backwards through its sequence)
-        auto tile_of = [&](int jj) -> int2 {
-            const int j = fwd ? jj : cnt - 1 - jj;
-            const int k = (j / nsl) * kSlots + warp + 8 * (j % nsl);
-            return (j == 0) ? ijc[0] : (j == 1) ? ijc[1] : p.tiles[g + k * G];
+        auto pos_tile = [&](int P) -> int2 {          // tile of the pair at position P of this pass
+            const int t = fwd ? P : pcnt - 1 - P;
+            return (t == 0) ? ijc[0] : (t == 1) ? ijc[1] : (t == 2) ? ijc[2] : p.tiles[g + kpair(t) * G];
         };
+        auto tile_of = [&](int jj) -> int2 { return pos_tile(2 * jj + pr_m); };
         cplx rawI[2], rawJ[2];
         int2 ijq[3] = {make_int2(0, 0), make_int2(0, 0), make_int2(0, 0)};     // coordinates of tiles jj, jj + 1, jj + 2
 #pragma unroll
@@ -276,6 +287,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
             }
         }
         if (!wide && cnt > 2) ijq[2] = tile_of(2);
+        int2 ijr = make_int2(0, 0);                 // coordinates of the tile this warp loads after its next tile
+        if (streaming && pr_m + 3 < pcnt) ijr = pos_tile(pr_m + 3);
         const int nprod = producers(n - c, G);          // CTAs that left partials for this column
         // warp 0: Householder scalars from the partial norms
         if (warp == 0) {
@@ -364,9 +377,10 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 // the tile coordinates run three tiles and the pieces of column c two tiles ahead of the tile in work: a
                 // tile used to start with two dependent L2 round trips (coordinates, then the column pieces)
                 for (int jj = 0; jj < cnt; ++jj) {
-                    const int j = fwd ? jj : cnt - 1 - jj;
-                    const int h = j % nsl;
-                    const int k = (j / nsl) * kSlots + warp + 8 * h;
+                    const int P = 2 * jj + pr_m;
+                    const int s3 = (fwd ? P : pcnt - 1 - P) % 3;
+                    const int slot = pr_p + 4 * s3;
+                    const unsigned expected = ((s3 == 0) ? base0 : (s3 == 1) ? base1 : base2) + (unsigned)(P / 3);
                     const int2 ij = ijq[0];
                     const int r0 = ij.x * kTS, c0 = ij.y * kTS;
                     const bool diag = (ij.x == ij.y);
@@ -378,7 +392,8 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         if (rI < n && rI > c + 1) nxtI = ldx_(&A[(size_t)c * lda + rI]);
                         if (ijq[2].x != ijq[2].y && rJ < n && rJ > c + 1) nxtJ = ldx_(&A[(size_t)c * lda + rJ]);
                     }
-                    const int2 ijrefill = (nsl == 2) ? ijq[2] : ijq[1];      // the tile nsl further on in this pass
+                    int2 ijr_n = make_int2(0, 0);
+                    if (streaming && P + 5 < pcnt) ijr_n = pos_tile(P + 5);
                     // v pieces (formed on the fly; zero outside the trailing matrix)
                     {
                         const int rI = r0 + lane, rJ = c0 + lane;
@@ -390,9 +405,13 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         __syncwarp();
                         vI[lane] = a; vJ[lane] = b;
                     }
-                    mbar_wait(mbar0 + 8u * (k % kSlots), ph[h]);
+                    // the load of this tile is the `expected`-th into its slot; it may not have been issued yet (the other warp
+                    // of the pair issues it after its own tile): wait for the issue count first, a parity alone could be a
+                    // whole phase behind
+                    if (streaming) { while ((unsigned)s_iss[slot] < expected) {} }
+                    mbar_wait(mbar0 + 8u * slot, (expected - 1u) & 1u);
                     __syncwarp();
-                    const cplx *sl = s_slots + (size_t)(k % kSlots) * kSlotElems;
+                    const cplx *sl = s_slots + (size_t)slot * kSlotElems;
                     // two independent accumulator sets (even / odd columns) halve the dependent DFMA chains
                     cplx accR = mk(0.0, 0.0), accC = mk(0.0, 0.0), accR1 = mk(0.0, 0.0), accC1 = mk(0.0, 0.0);
                     if (!diag) {
@@ -429,15 +448,24 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     }
                     qacc += qterm;                    // per lane; one warp reduction after the pass
                     if (streaming) {
-                        // refill this slot with the tile that uses it next in this pass; at the end of a pass
-                        // the slot keeps its tile, which is the first one the reversed next pass needs
-                        const int jn = fwd ? j + nsl : j - nsl;
-                        if (jn >= 0 && jn < cnt) {
-                            const int kn = (jn / nsl) * kSlots + warp + 8 * h;
+                        // refill this slot with the tile that uses it next in this pass (position P + 3, the other warp's);
+                        // at the end of a pass the slots keep their tiles, the first ones the reversed next pass needs
+                        if (P + 3 < pcnt) {
                             __syncwarp();
-                            ph[h] ^= 1u;
-                            (void)kn;
-                            warp_load_tile(s_slots + (size_t)(k % kSlots) * kSlotElems, mbar0 + 8u * (k % kSlots), A, lda, n, ijrefill, lane);
+                            warp_load_tile(s_slots + (size_t)slot * kSlotElems, mbar0 + 8u * slot, A, lda, n, ijr, lane);
+                            if (lane == 0) { __threadfence_block(); s_iss[slot] = (int)(expected + 1u); }
+                        }
+                        ijr = ijr_n;
+                    }
+                }
+                if (streaming) {
+                    // loads of this pass per slot: positions 3 <= P' < pcnt; positions of one residue mod 3 share a slot
+#pragma unroll
+                    for (int r = 0; r < 3; ++r) {
+                        if (pcnt - 1 >= r) {
+                            const int s3r = (fwd ? r : pcnt - 1 - r) % 3;
+                            const unsigned add = (unsigned)((pcnt - 1 - r) / 3);
+                            if (s3r == 0) base0 += add; else if (s3r == 1) base1 += add; else base2 += add;
                         }
                     }
                 }
@@ -603,14 +631,16 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         TRACE(7);
     }
     // no bulk copy may be in flight when the CTA exits (a one-column last panel never reads its tiles)
-    for (int h = 0; h < nsl; ++h) {
-        const int k = warp + 8 * h;
-        if (k < q && g + k * G < T) mbar_wait(mbar0 + 8u * k, ph[h]);
+    if (wide) { if (warp < 2 && warp < q && g + warp * G < T) mbar_wait(mbar0 + 8u * warp, 0u); }
+    else {
+        if (0 < pcnt) mbar_wait(mbar0 + 8u * (pr_p + 0), (base0 - 1u) & 1u);
+        if (1 < pcnt) mbar_wait(mbar0 + 8u * (pr_p + 4), (base1 - 1u) & 1u);
+        if (2 < pcnt) mbar_wait(mbar0 + 8u * (pr_p + 8), (base2 - 1u) & 1u);
     }
 }
 
 static size_t panel_smem_bytes() {
-    return sizeof(cplx) * (size_t)(kSlots * kSlotElems + 8 * 2 * kTS + 4 * kNB + 16 * kNB + 4) + sizeof(double) * (20 + kSlots);
+    return sizeof(cplx) * (size_t)(kSlots * kSlotElems + 8 * 2 * kTS + 4 * kNB + 16 * kNB + 4) + sizeof(double) * (20 + kSlots + (kSlots + 1) / 2);
 }
 
 // ---------------------------------------------------------------- HER2K (DMMA)
