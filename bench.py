@@ -84,7 +84,7 @@ def measured_hbm_gbs():
 NCU_TRAFFIC = {
     ("S1S2S3_tridiag_cluster", 3): {"bytes_per_launch": 3.17e6, "source": "profiles/r1_cluster_ncu_full.md (n=625, whole reduction in one launch)"},
     ("S2S3_tridiag_panel", 3): {"bytes_per_launch": 2.82e6, "source": "profiles/r1_tuned_ncu_full.md (first panel, n=625)"},
-    ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.23e9, "source": "profiles/r1_final_ncu_full.md (first panels, n=4096)"},
+    ("S2S3_tridiag_panel", 5): {"bytes_per_launch": 2.01e9, "source": "profiles/r1_final_ncu_full.md (first panels, n=4096)"},
     ("S10_householder_ql", 2): {"bytes_per_launch": 1.35e7, "source": "profiles/r1_tuned_ncu_full.md (256 x n=81)"},
 }
 
@@ -101,7 +101,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.index)],
+                                          "-lms", "20", "-i", str(self.index)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()

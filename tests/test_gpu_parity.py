@@ -190,6 +190,21 @@ def test_config5_n4096_closed_form_and_invariants(orc, hp):
         assert rel_err(got, want) <= TOL * 4096
 
 
+@pytest.mark.parametrize("n", [1891, 1930])
+def test_panel_kernel_first_streamed_sizes_closed_form(orc, hp, n):
+    """Sizes just above the resident limit of the panel kernel (12 tile slots x 148 SMs = 1776 tiles: n <= 1888):
+    the first panels stream through the three-slot rings of the warp pairs with only one refill per ring, the last
+    tile row is ragged (n is not a multiple of 32), later panels are resident.  Pinned against the closed form from
+    the generator's own Q and lambda (no eigensolver) and the projection invariants."""
+    rng = np.random.default_rng(workloads.BASE_SEED + 100 + n)
+    b = workloads.from_spectrum(rng, workloads.spectrum_admm_lowrank(rng, n, n_big=8, sd=1e-1))
+    sv = orc.pack(b.X)
+    got = gpu_project(hp, [n], sv)
+    closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
+    assert rel_err(got, closed) <= TOL * n
+    check_invariants(hp, [n], sv, got)
+
+
 # ------------------------------------------------------------------ sizes across both paths
 
 @pytest.mark.parametrize("n", [2, 3, 4, 15, 31, 32, 33, 63, 64, 65, 83, 84])
