@@ -292,9 +292,13 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         const int nprod = producers(n - c, G);          // CTAs that left partials for this column
         // warp 0: Householder scalars from the partial norms
         if (warp == 0) {
-            double S = 0.0;
-            for (int k = lane; k < nprod; k += 32) S += ldx_(&p.part[(size_t)k * PSTRIDE].x);
+            // five independent loads in flight (a load -> add -> load loop costs one L2 round trip per 32 producers)
+            double Sp[5];
+#pragma unroll
+            for (int u = 0; u < 5; ++u) { const int k = lane + 32 * u; Sp[u] = (k < nprod) ? ldx_(&p.part[(size_t)k * PSTRIDE].x) : 0.0; }
             const cplx alpha = ldx_(&A[(size_t)c * lda + c + 1]);
+            double S = ((Sp[0] + Sp[1]) + (Sp[2] + Sp[3])) + Sp[4];
+            for (int k = lane + 160; k < nprod; k += 32) S += ldx_(&p.part[(size_t)k * PSTRIDE].x);
             S = warp_sum(S);
             double beta; cplx tau0, scale0;
             householder_scalars(alpha, S, beta, tau0, scale0);
@@ -308,8 +312,12 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         const bool reducer = (warp == 7 && i > 0 && g < 2 * kNB && (g % kNB) < i);
         if (reducer) {
             const int t = g % kNB, which = g / kNB;
-            for (int k = lane; k < nprod; k += 32) red_s = red_s + ldx_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
+            cplx rp[5];
+#pragma unroll
+            for (int u = 0; u < 5; ++u) { const int k = lane + 32 * u; rp[u] = (k < nprod) ? ldx_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]) : mk(0.0, 0.0); }
             red_top = which == 0 ? ldx_(&A[(size_t)(p.j0 + t) * lda + c + 1]) : ldx_(&W[(size_t)t * ldw + c + 1]);
+            red_s = ((rp[0] + rp[1]) + (rp[2] + rp[3])) + rp[4];
+            for (int k = lane + 160; k < nprod; k += 32) red_s = red_s + ldx_(&p.part[(size_t)k * PSTRIDE + 1 + which * kNB + t]);
             red_s = warp_sum(red_s);
         }
         __syncthreads();
