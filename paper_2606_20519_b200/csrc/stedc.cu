@@ -333,11 +333,16 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
             list[pos] = idx;
             ++ndefl;
         };
+        // the candidate's pole and weight are carried in registers and those of row r + 1 are loaded one step ahead
+        // (rotations only touch rows <= r): the serial chain per row loses three shared-memory latencies
+        double zn = zs[0], dn = ds[0], zpj = 0.0, dpj = 0.0;
         for (int r = 0; r < N; ++r) {
-            if (rho * fabs(zs[r]) <= tol) { push_defl(r); continue; }
-            if (pj < 0) { pj = r; continue; }
-            double s = zs[pj], c = zs[r];
-            const double t = ds[r] - ds[pj];
+            const double zr = zn, dr = dn;
+            if (r + 1 < N) { zn = zs[r + 1]; dn = ds[r + 1]; }
+            if (rho * fabs(zr) <= tol) { push_defl(r); continue; }
+            if (pj < 0) { pj = r; zpj = zr; dpj = dr; continue; }
+            double s = zpj, c = zr;
+            const double t = dr - dpj;
             // |t c s| <= tol with c = z_r/tau, s = -z_pj/tau, tau^2 = z_r^2 + z_pj^2, tested without sqrt or division
             if (fabs(t) * fabs(c * s) <= tol * (c * c + s * s)) {
                 const double tau = sqrt(c * c + s * s);      // weights are <= 1 in magnitude and > tol/rho: no over/underflow
@@ -347,14 +352,15 @@ __global__ void __launch_bounds__(256) stedc_merge_setup_kernel(MergeArgs a) {
                 a.rp[lo + nrot] = src[pj] & 0x0fffffff; a.rq[lo + nrot] = src[r] & 0x0fffffff;
                 a.rc[lo + nrot] = c; a.rs[lo + nrot] = s; ++nrot;
                 if ((src[pj] >> 28) != (src[r] >> 28)) src[r] = (src[r] & 0x0fffffff) | (2 << 28);
-                const double tt = ds[pj] * c * c + ds[r] * s * s;
-                ds[r] = ds[pj] * s * s + ds[r] * c * c;
+                const double tt = dpj * c * c + dr * s * s;
+                const double dnew = dpj * s * s + dr * c * c;
+                ds[r] = dnew;
                 ds[pj] = tt;
                 push_defl(pj);
-                pj = r;
+                pj = r; zpj = tau; dpj = dnew;
             } else {
                 list[K++] = pj;
-                pj = r;
+                pj = r; zpj = zr; dpj = dr;
             }
         }
         if (pj >= 0) list[K++] = pj;
