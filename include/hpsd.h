@@ -32,7 +32,10 @@
  *   - Return value: HPSD_OK (0) or a negative HPSD_E* code; never throws.
  *     Numerical trouble (an iteration that did not converge) cannot be
  *     returned synchronously: it sets info_dev[b] != 0 on the device.
- *   - NaN/Inf in the input propagate to the output; no check is made.
+ *   - NaN/Inf in the input (the paper is silent): a block that holds a non-finite
+ *     value gets an all-NaN output block (with hpsd_admm_step also an all-NaN v
+ *     block) and info[b] = 2; the other blocks of the call are unaffected.  Finite
+ *     entries whose squares overflow are outside the supported range.
  *   - n_b = 0 blocks are skipped; n_b = 1 gives out = max(in, 0).
  *   - There is no CPU fallback: without a CUDA device every compute call
  *     returns HPSD_ECUDA.
@@ -109,6 +112,16 @@ int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream);
  * n doubles) and sub-diagonal e (DEVICE, n-1 doubles).  First half of the
  * "eigendecomposition" of PAPER.md:1536; lets tests check the reduction alone. */
 int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream);
+
+/* S2 of SURVEY.md §8(a) alone (two-stage reduction, option "two_stage"): reduce one
+ * Hermitian block (svec, DEVICE, n >= 2) to a Hermitian BAND matrix of width
+ * b = hpsd_band_width() unitarily similar to it.  band (DEVICE) receives 2b x n
+ * complex FP64 elements, column-major with leading dimension 2b: element (i, j),
+ * j <= i <= j + b, of the band matrix at band[(i - j) + j * 2b] (rows b+1 .. 2b-1 of
+ * every column are zero: room for the bulge of S3).  HPSD_ECUDA when the device
+ * cannot launch the 16-CTA cluster the panel factorisation needs. */
+int hpsd_reduce_to_band(int n, const double *in_svec, double *band, void *stream);
+int hpsd_band_width(void);
 
 /* Eigenvalues of one Hermitian block given as svec (DEVICE), ascending, into
  * lambda (DEVICE, n doubles).  Diagnostic/NEXT-2 entry:

@@ -9,6 +9,8 @@ from .binding import (  # noqa: F401
     HpsdError,
     admm_step_,
     eigvalsh,
+    reduce_to_band,
+    band_width,
     fp64_peak_probe,
     last_launch_count,
     lib_path,

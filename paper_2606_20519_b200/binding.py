@@ -17,6 +17,7 @@ EXPORTS = [
     "hpsd_project_host", "hpsd_pack", "hpsd_unpack", "hpsd_tridiagonalize", "hpsd_eigvalsh",
     "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
+    "hpsd_reduce_to_band", "hpsd_band_width",
 ]
 
 
@@ -50,6 +51,7 @@ def load_library():
         lib.hpsd_unpack.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
         lib.hpsd_tridiagonalize.argtypes = [c_int, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_eigvalsh.argtypes = [c_int, c_vp, c_vp, c_vp]
+        lib.hpsd_reduce_to_band.argtypes = [c_int, c_vp, c_vp, c_vp]
         lib.hpsd_set_option.argtypes = [ctypes.c_char_p, c_int]
         lib.hpsd_last_launch_count.restype = c_int
         lib.hpsd_release.restype = c_int
@@ -206,6 +208,21 @@ def tridiagonalize(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Strea
     with torch.cuda.device(svec.device):
         _check(load_library().hpsd_tridiagonalize(n, svec.data_ptr(), d.data_ptr(), e.data_ptr(), _stream(stream)), "hpsd_tridiagonalize")
     return d, e
+
+
+def band_width() -> int:
+    return int(load_library().hpsd_band_width())
+
+
+def reduce_to_band(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_reduce_to_band: S2 alone.  Returns the band as an (n, 2b) complex tensor: row j holds column j of the
+    band storage (element (i, j) of the band matrix at [j, i - j])."""
+    _need_cuda_f64(svec, "svec")
+    b = band_width()
+    band = torch.empty((n, 2 * b), dtype=torch.complex128, device=svec.device)
+    with torch.cuda.device(svec.device):
+        _check(load_library().hpsd_reduce_to_band(n, svec.data_ptr(), band.data_ptr(), _stream(stream)), "hpsd_reduce_to_band")
+    return band
 
 
 def eigvalsh(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:

@@ -10,6 +10,7 @@
 #include "kernels.h"
 #include "gemm.cuh"
 #include "large.h"
+#include "twostage.h"
 #include "prof.h"
 
 namespace hpsd {
@@ -53,13 +54,13 @@ struct SubEpi {        // C[i + j*ld] -= acc
 __global__ void __launch_bounds__(BG_THREADS) bt_gram_kernel(BackWs w) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int b = blockIdx.z, cb = b * kNBT;
-    const int nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
+    const int nbw = min(kNBT, w.n - cb), m = w.n - cb - w.voff;
     if (m <= 0) return;
     const int chunk = (((m + kSplitK - 1) / kSplitK) + 15) & ~15;
     const int k0 = blockIdx.x * chunk;
     const int klen = min(chunk, m - k0);
     GemmProblem<cplx, cplx> p;
-    p.A = w.A + (size_t)cb * w.lda + cb + 1 + k0; p.lda = w.lda; p.B = p.A; p.ldb = w.lda;
+    p.A = w.A + (size_t)cb * w.lda + cb + w.voff + k0; p.lda = w.lda; p.B = p.A; p.ldb = w.lda;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = nbw; p.K = klen > 0 ? klen : 0; p.K2 = 0;
     StoreEpi epi{w.Xp + ((size_t)b * kSplitK + blockIdx.x) * kNBT * kNBT, kNBT};
     gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, 0, 0, smem_raw, epi);
@@ -105,13 +106,13 @@ __global__ void __launch_bounds__(kNBT) bt_tfactor_kernel(BackWs w) {
 __global__ void __launch_bounds__(BG_THREADS) bt_vt_kernel(BackWs w) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int b = blockIdx.z, cb = b * kNBT;
-    const int nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
+    const int nbw = min(kNBT, w.n - cb), m = w.n - cb - w.voff;
     if (m <= 0 || (int)blockIdx.x * 64 >= m) return;
     GemmProblem<cplx, cplx> p;
-    p.A = w.A + (size_t)cb * w.lda + cb + 1; p.lda = w.lda;
+    p.A = w.A + (size_t)cb * w.lda + cb + w.voff; p.lda = w.lda;
     p.B = w.Tm + (size_t)b * kNBT * kNBT; p.ldb = kNBT;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = m; p.N = nbw; p.K = nbw; p.K2 = 0;
-    StoreEpi epi{w.VT + (size_t)cb * w.lda + cb + 1, w.lda};
+    StoreEpi epi{w.VT + (size_t)cb * w.lda + cb + w.voff, w.lda};
     gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, BG_MI, BG_NI, BG_WM, BG_WN, false>(p, blockIdx.x, 0, smem_raw, epi);
 }
 
@@ -123,13 +124,13 @@ __global__ void __launch_bounds__(BG_THREADS, (ST == 2 ? 2 : 1)) bt_vhz_kernel(B
     constexpr int BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
     if ((int)blockIdx.x * BN >= kpos) return;
-    const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
+    const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - w.voff;
     const int chunk = (((m + kSplitK - 1) / kSplitK) + 15) & ~15;
     const int k0 = blockIdx.y * chunk;
     const int klen = min(chunk, m - k0);
     GemmProblem<cplx, cplx> p;
-    p.A = w.A + (size_t)cb * w.lda + cb + 1 + k0; p.lda = w.lda;
-    p.B = w.Zc + cb + 1 + k0; p.ldb = w.ldz;
+    p.A = w.A + (size_t)cb * w.lda + cb + w.voff + k0; p.lda = w.lda;
+    p.B = w.Zc + cb + w.voff + k0; p.ldb = w.ldz;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = nbw; p.N = kpos; p.K = klen > 0 ? klen : 0; p.K2 = 0;
     StoreEpi epi{w.Xp + (size_t)blockIdx.y * kNBT * w.n, kNBT};
     gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, MI, NI, BG_WM, BG_WN, false, ST>(p, blockIdx.z, blockIdx.x, smem_raw, epi);
@@ -152,20 +153,22 @@ __global__ void __launch_bounds__(BG_THREADS, 3) bt_update_kernel(BackWs w, int 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int BM = BG_WM * MI * 8, BN = BG_WN * NI * 8;
     const int kpos = w.cnt[1];
-    const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - 1;
+    const int cb = b * kNBT, nbw = min(kNBT, w.n - cb), m = w.n - cb - w.voff;
     if ((int)blockIdx.y * BN >= kpos || (int)blockIdx.x * BM >= m) return;
     GemmProblem<cplx, cplx> p;
-    p.A = w.VT + (size_t)cb * w.lda + cb + 1; p.lda = w.lda;
+    p.A = w.VT + (size_t)cb * w.lda + cb + w.voff; p.lda = w.lda;
     p.B = w.X; p.ldb = kNBT;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = m; p.N = kpos; p.K = nbw; p.K2 = 0;
-    SubEpi epi{w.Zc + cb + 1, w.ldz};
+    SubEpi epi{w.Zc + cb + w.voff, w.ldz};
     gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, MI, NI, BG_WM, BG_WN, false, 2>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
 // ---- S7 + S8: lower triangle of W W^H packed as vec_R (Eq. D10) --------------------------------
 struct PackEpi {
     SvecIo io; int n;
+    bool bad;          // non-finite input (flag of S1): the block's output is NaN
     __device__ __forceinline__ void operator()(int i, int j, double re, double im) const {
+        if (bad) { re = nan_(); im = nan_(); }
         const size_t c = svec_col_off(n, j);
         if (i == j) io_store(io, c, re);
         else { const int k = i - j - 1; io_store(io, c + 1 + 2 * k, kSqrt2 * re); io_store(io, c + 2 + 2 * k, kSqrt2 * im); }
@@ -178,7 +181,9 @@ __global__ void __launch_bounds__(BG_THREADS) herk_pack_kernel(BackWs w, SvecIo 
     GemmProblem<cplx, cplx> p;
     p.A = w.Zc; p.lda = w.ldz; p.B = w.Zc; p.ldb = w.ldz;
     p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = w.n; p.N = w.n; p.K = w.cnt[1]; p.K2 = 0;
-    PackEpi epi{io, w.n};
+    const bool bad = w.cnt[2] != 0;
+    if (bad && w.info != nullptr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) *w.info = kInfoNonFinite;
+    PackEpi epi{io, w.n, bad};
     gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, BG_MI, BG_NI, BG_WM, BG_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
 }
 
@@ -228,7 +233,8 @@ int launch_bt_factors(const BackWs &w, cudaStream_t st) {
     return 0;
 }
 
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done) {
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done,
+                     const TwoStageWs *ts) {
     const int n = w.n;
     int rc = backherk_init();
     if (rc) return rc;
@@ -241,11 +247,18 @@ int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int l
     scale_convert_kernel<<<dim3((n + 1023) / 1024, n), 256, 0, st>>>(n, lam, Zt, ldzt, w.Zc, w.ldz, w.cnt);
     HPSD_LAUNCH_CHECK();
     if (!factors_done) {
+        if (ts) { rc = launch_q2_factors(*ts, st); if (rc) return rc; }
         rc = launch_bt_factors(w, st);
         if (rc) return rc;
     }
+    if (ts) {
+        prof_end(ST_BACK, st);
+        rc = launch_q2_apply(*ts, w.Zc, w.ldz, w.cnt, st);
+        if (rc) return rc;
+        prof_begin(ST_BACK, st);
+    }
     for (int b = nblocks - 1; b >= 0; --b) {
-        const int m = n - b * kNBT - 1;
+        const int m = n - b * kNBT - w.voff;
         if (m <= 0) continue;
         if (small) bt_vhz_kernel<2, 2><<<dim3((n + 31) / 32, kSplitK, 2), BG_THREADS, kSmemKKs, st>>>(w, b);
         else if (n >= 3072) bt_vhz_kernel<4, 4, 2><<<dim3(nt, kSplitK, 1), BG_THREADS, kSmemKK2, st>>>(w, b);   // > 148 live CTAs: two per SM

@@ -34,6 +34,13 @@ __device__ __forceinline__ void cfma_conj(cplx &acc, cplx a, cplx b) {
 __device__ __forceinline__ double ldcg_(const double *p) { return __ldcg(p); }
 __device__ __forceinline__ cplx ldcg_(const cplx *p) { const double2 v = __ldcg(reinterpret_cast<const double2 *>(p)); return mk(v.x, v.y); }
 
+// NaN / Inf contract (include/hpsd.h): a block whose input holds a non-finite value gets an all-NaN output block
+// and info[b] = kInfoNonFinite; the arithmetic in between runs on a sanitised copy (zeros), so nothing downstream
+// (sorts, searches, iteration counts) ever sees a NaN.
+constexpr int kInfoNonFinite = 2;
+__device__ __forceinline__ bool nonfinite(double x) { return !(fabs(x) <= 1.79769313486231570e308); }
+__device__ __forceinline__ double nan_() { return __longlong_as_double(0x7ff8000000000000LL); }
+
 constexpr double kSqrt2 = 1.4142135623730951;      // nearest double to sqrt(2)
 constexpr double kEps = 2.220446049250313e-16;     // 2^-52
 
@@ -57,6 +64,10 @@ __device__ __forceinline__ double io_load(const SvecIo &io, size_t i) {
 __device__ __forceinline__ void io_store(const SvecIo &io, size_t i, double u) {
     if (io.sub) io.vout[i] = (io.sub[i] - io.in[i]) + u;
     io.out[i] = u;
+}
+// all n^2 svec entries of one block <- NaN (and the ADMM v update with it), by nthreads threads
+__device__ __forceinline__ void io_fill_nan(const SvecIo &io, size_t base, int n, int tid, int nthreads) {
+    for (size_t t = tid; t < (size_t)n * n; t += nthreads) io_store(io, base + t, nan_());
 }
 inline SvecIo io_offset(const SvecIo &io, long long off) {
     SvecIo r = io;

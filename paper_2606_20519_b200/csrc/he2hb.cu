@@ -1,0 +1,521 @@
+// he2hb.cu -- S2 of SURVEY.md §8(a): dense Hermitian -> Hermitian band of width b = kBW, A = Q1 B Q1^H.
+// First half of the "eigendecomposition" of PAPER.md:1536 in its two-stage form (BASELINE.json north star (c)).
+//
+// Per panel k (columns j0 = k b .. j0 + b - 1, trailing size m = n - j0 - b):
+//   [QR]   Householder QR of the m x b panel A[j0+b:, j0:j0+b] inside ONE 16-CTA cluster (he2hb_panel_kernel):
+//          rows are dealt to the CTAs and live in shared memory, every column step needs ONE all-to-all exchange
+//          (st.async + mbarrier, cluster.cuh): the CTAs exchange the b inner products of the raw column with all
+//          panel columns; norm, v^H P and the column V^H v of the T recurrence all follow from them.
+//          R goes to the band, V (explicit unit diagonal) to V1, T to Tk.
+//   [HEMM] Zp[s] = A22[:, K_s] V[K_s, :]           split-K complex DMMA GEMM over all SMs (A22 is stored in full)
+//   [SLAB] Z = sum_s Zp[s]; G = V^H Z (last CTA done: S = -1/2 T^H G T)
+//   [X]    X = Z T + V S                            (= A22 V T - 1/2 V T^H V^H A22 V T)
+//   [HER2K] A22 -= X V^H + V X^H                    lower tiles on DMMA, each element mirrored into the upper triangle
+// so that all (16/3) n^3 flops of the reduction are BLAS-3 and the dependent chain is n cluster exchanges instead of
+// 2 n grid-wide barriers.
+#include "kernels.h"
+#include "gemm.cuh"
+#include "cluster.cuh"
+#include "large.h"
+#include "twostage.h"
+#include "prof.h"
+
+namespace hpsd {
+
+constexpr int kQrCl = 16;                 // CTAs per cluster (non-portable size)
+constexpr int kQrWarps = 10;              // warp 0: top b x b block (kept by every CTA), warps 1..8: 32 rows each, warp 9: T
+constexpr int kQrThreads = kQrWarps * 32;
+constexpr int kQrRows = 256;              // ordinary rows per CTA
+constexpr int kQrP = kBW + 1;             // shared-memory pitch (elements): row-wise and column-wise accesses conflict free
+static_assert(kBW == 32, "the panel kernel maps lane = panel column");
+
+struct QrArgs {
+    int n, lda, ldv, ldab, j0;
+    const cplx *A;
+    cplx *V1, *tau1, *Tk, *AB;
+};
+
+struct QrSmem {
+    static constexpr size_t mbar = 0;                                            // two mbarriers
+    static constexpr size_t land = 16;                                           // [2][kQrCl][kBW]
+    static constexpr size_t part = land + sizeof(cplx) * 2 * kQrCl * kBW;        // [2][kQrWarps][kBW]
+    static constexpr size_t row = part + sizeof(cplx) * 2 * kQrWarps * kBW;      // [2][kBW]
+    static constexpr size_t qw = row + sizeof(cplx) * 2 * kBW;                   // [kBW]
+    static constexpr size_t tau = qw + sizeof(cplx) * kBW;                       // [kBW]
+    static constexpr size_t scl = tau + sizeof(cplx) * kBW;                      // [kBW]
+    static constexpr size_t top = scl + sizeof(cplx) * kBW;                      // [kBW][kQrP]
+    static constexpr size_t tf = top + sizeof(cplx) * kBW * kQrP;                // [kBW][kQrP]
+    static constexpr size_t rows = tf + sizeof(cplx) * kBW * kQrP;               // [kQrRows][kQrP]
+    static constexpr size_t total = rows + sizeof(cplx) * kQrRows * kQrP;
+};
+
+// zlarfg scalars: H = I - tau v v^H with v = [1; x scale] maps [alpha; x] to [beta; 0], beta real
+__device__ __forceinline__ void qr_householder(cplx alpha, double xnorm2, double &beta, cplx &tau, cplx &scale) {
+    if (xnorm2 == 0.0 && alpha.y == 0.0) {
+        beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
+    } else {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        beta = -copysign(nrm, alpha.x);
+        const double ib = 1.0 / beta;
+        tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
+        const cplx den = mk(alpha.x - beta, alpha.y);
+        const double id2 = 1.0 / abs2(den);
+        scale = mk(den.x * id2, -den.y * id2);
+    }
+}
+
+// acc_lane += sum over rows r0 <= r < r1 of conj(P[r][j]) P[r][lane]
+__device__ __forceinline__ cplx qr_dots(const cplx *P, int r0, int r1, int j, int lane) {
+    cplx a0 = mk(0.0, 0.0), a1 = a0, a2 = a0, a3 = a0;
+    int r = r0;
+    for (; r + 3 < r1; r += 4) {
+        const cplx x0 = P[(r + 0) * kQrP + j], p0 = P[(r + 0) * kQrP + lane];
+        const cplx x1 = P[(r + 1) * kQrP + j], p1 = P[(r + 1) * kQrP + lane];
+        const cplx x2 = P[(r + 2) * kQrP + j], p2 = P[(r + 2) * kQrP + lane];
+        const cplx x3 = P[(r + 3) * kQrP + j], p3 = P[(r + 3) * kQrP + lane];
+        cfma_conj(a0, x0, p0); cfma_conj(a1, x1, p1); cfma_conj(a2, x2, p2); cfma_conj(a3, x3, p3);
+    }
+    for (; r < r1; ++r) cfma_conj(a0, P[r * kQrP + j], P[r * kQrP + lane]);
+    return (a0 + a1) + (a2 + a3);
+}
+
+// rows r0 <= r < r1:  P[r][lane] -= f (P[r][j] scale)   for lane > j   (f = 0 on the other lanes)
+__device__ __forceinline__ void qr_update(cplx *P, int r0, int r1, int j, int lane, cplx f, cplx scale) {
+    const cplx nf = mk(-f.x, -f.y);
+    if (lane <= j) return;
+#pragma unroll 4
+    for (int r = r0; r < r1; ++r) {
+        const cplx v = P[r * kQrP + j] * scale;
+        cplx p = P[r * kQrP + lane];
+        cfma(p, nf, v);
+        P[r * kQrP + lane] = p;
+    }
+}
+
+__global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
+    extern __shared__ __align__(16) unsigned char sm[];
+    cplx *s_land = reinterpret_cast<cplx *>(sm + QrSmem::land);
+    cplx *s_part = reinterpret_cast<cplx *>(sm + QrSmem::part);
+    cplx *s_row = reinterpret_cast<cplx *>(sm + QrSmem::row);
+    cplx *s_qw = reinterpret_cast<cplx *>(sm + QrSmem::qw);
+    cplx *s_tau = reinterpret_cast<cplx *>(sm + QrSmem::tau);
+    cplx *s_scl = reinterpret_cast<cplx *>(sm + QrSmem::scl);
+    cplx *s_top = reinterpret_cast<cplx *>(sm + QrSmem::top);
+    cplx *s_T = reinterpret_cast<cplx *>(sm + QrSmem::tf);
+    cplx *s_P = reinterpret_cast<cplx *>(sm + QrSmem::rows);
+    const unsigned mbar0 = cx_smem_u32(sm + QrSmem::mbar);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int rank = (int)cx_rank();
+    const int n = a.n, j0 = a.j0, lda = a.lda;
+    const int g0 = j0 + kBW;                     // global row of panel row 0
+    const int m = n - g0;                        // panel rows (> 0)
+    const int mo = m > kBW ? m - kBW : 0;        // ordinary rows (below the top block)
+    const int rpc = (mo + kQrCl - 1) / kQrCl;    // per CTA (<= kQrRows)
+    const int lo = rank * rpc;
+    const int cnt = mo - lo < 0 ? 0 : (mo - lo < rpc ? mo - lo : rpc);
+    const int nsteps = m < kBW ? m : kBW;
+
+    if (tid == 0) {
+        cx_mbar_init(mbar0, 1);
+        cx_mbar_init(mbar0 + 8, 1);
+        cx_fence_mbar_init();
+        cx_arm(mbar0, kQrCl * kBW * (unsigned)sizeof(cplx));
+        cx_arm(mbar0 + 8, kQrCl * kBW * (unsigned)sizeof(cplx));
+    }
+    // top block (every CTA keeps and updates its own copy, bit-identically)
+    for (int e = tid; e < kBW * kBW; e += kQrThreads) {
+        const int l = e % kBW, k = e / kBW;
+        s_top[l * kQrP + k] = (l < m) ? a.A[(size_t)(j0 + k) * lda + g0 + l] : mk(0.0, 0.0);
+        s_T[l * kQrP + k] = mk(0.0, 0.0);
+    }
+    if (tid < kBW) { s_tau[tid] = mk(0.0, 0.0); s_scl[tid] = mk(0.0, 0.0); }
+    // ordinary rows of this CTA: lane = row (coalesced 512-byte segments), one panel column per iteration
+    if (warp >= 1 && warp <= 8) {
+        const int r = (warp - 1) * 32 + lane;
+        if (r < cnt) {
+            const cplx *src = a.A + (size_t)j0 * lda + g0 + kBW + lo + r;
+#pragma unroll 8
+            for (int k = 0; k < kBW; ++k) s_P[r * kQrP + k] = src[(size_t)k * lda];
+        }
+    }
+    // diagonal block of this panel -> band (final: no later update touches it)
+    if (rank == kQrCl - 1) {
+        for (int e = tid; e < kBW * kBW; e += kQrThreads) {
+            const int r = e % kBW, c = e / kBW;
+            if (r >= c) a.AB[(size_t)(j0 + c) * a.ldab + (r - c)] = a.A[(size_t)(j0 + c) * lda + j0 + r];
+        }
+    }
+    __syncthreads();
+    cx_barrier();                                // every mbarrier of the cluster is initialised and armed
+
+    const int r0 = (warp - 1) * 32;
+    const int r1 = (warp >= 1 && warp <= 8) ? (cnt < r0 + 32 ? cnt : r0 + 32) : 0;
+
+    for (int j = 0; j < nsteps; ++j) {
+        const int par = j & 1;
+        // ---- inner products of the raw column j with every panel column, over the rows below the diagonal row
+        cplx acc = mk(0.0, 0.0);
+        if (warp == 0) {
+            s_row[par * kBW + lane] = s_top[j * kQrP + lane];
+            if (rank == 0) acc = qr_dots(s_top, j + 1, kBW, j, lane);
+        } else if (r1 > r0) {
+            acc = qr_dots(s_P, r0, r1, j, lane);
+        }
+        // (double-buffered: a warp that is through the exchange of step j may write its step j + 1 partial while a slower
+        // warp of this CTA is still summing the partials of step j)
+        cplx *sp = s_part + par * kQrWarps * kBW;
+        sp[warp * kBW + lane] = acc;
+        __syncthreads();
+        if (warp < kQrCl / 2) {
+            cplx tot = sp[lane];
+#pragma unroll
+            for (int w = 1; w < kQrWarps; ++w) tot = tot + sp[w * kBW + lane];
+            const unsigned dst = cx_smem_u32(s_land + (par * kQrCl + rank) * kBW + lane);
+            const unsigned mb = mbar0 + 8u * par;
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int peer = 2 * warp + t;
+                cx_st_async(cx_mapa(dst, peer), tot, cx_mapa(mb, peer));
+            }
+        }
+        cx_wait(mbar0 + 8u * par, (unsigned)(j >> 1) & 1u);
+        if (tid == 0) cx_arm(mbar0 + 8u * par, kQrCl * kBW * (unsigned)sizeof(cplx));      // for step j + 2
+        // ---- every warp: totals (fixed order: bit-identical in all CTAs), Householder scalars, update coefficients
+        cplx g = s_land[(par * kQrCl) * kBW + lane];
+#pragma unroll
+        for (int p = 1; p < kQrCl; ++p) g = g + s_land[(par * kQrCl + p) * kBW + lane];
+        if (lane < j) g = conj_(g);              // sum conj(P[:,k]) x  for the finished columns k < j
+        const double xnorm2 = __shfl_sync(0xffffffffu, g.x, j);
+        const cplx rowv = s_row[par * kBW + lane];
+        cplx alpha;
+        alpha.x = __shfl_sync(0xffffffffu, rowv.x, j);
+        alpha.y = __shfl_sync(0xffffffffu, rowv.y, j);
+        double beta; cplx tau, scale;
+        qr_householder(alpha, xnorm2, beta, tau, scale);
+        cplx f = mk(0.0, 0.0);
+        if (lane > j) f = conj_(tau) * (rowv + conj_(scale) * g);     // conj(tau) v^H P[:, lane]
+        if (warp == 0) {
+            if (lane > j) s_top[j * kQrP + lane] = rowv - f;
+            else if (lane == j) { s_top[j * kQrP + j] = mk(beta, 0.0); s_tau[j] = tau; s_scl[j] = scale; }
+            qr_update(s_top, j + 1, kBW, j, lane, f, scale);
+            __syncwarp();
+        } else if (r1 > r0) {
+            qr_update(s_P, r0, r1, j, lane, f, scale);
+            __syncwarp();
+        } else if (warp == kQrWarps - 1 && rank == 0) {
+            // column j of T:  T(0:j, j) = -tau T(0:j, 0:j) (V(:, 0:j)^H v_j),  T(j, j) = tau   (zlarft, forward columnwise)
+            // V[:, k] = P[:, k] scl[k] below its unit entry, so  V(:,k)^H v_j = conj(V[j,k]) + conj(scl_k) scale sum_{l>j} conj(P[l,k]) P[l,j]
+            if (lane < j) {
+                const cplx sk = conj_(s_scl[lane]);
+                s_qw[lane] = sk * conj_(rowv) + (sk * scale) * g;
+            }
+            __syncwarp();
+            if (lane < j) {
+                cplx s = mk(0.0, 0.0);
+                for (int k = lane; k < j; ++k) cfma(s, s_T[lane * kQrP + k], s_qw[k]);
+                s_T[lane * kQrP + j] = mk(-tau.x, -tau.y) * s;
+            } else if (lane == j) s_T[j * kQrP + j] = tau;
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    // ---- results: V (unit diagonal explicit; zeros above come from the memset of V1), R -> band, tau, T
+    if (warp >= 1 && warp <= 8) {
+        const int r = r0 + lane;
+        if (r < cnt) {
+            cplx *dst = a.V1 + (size_t)j0 * a.ldv + g0 + kBW + lo + r;
+#pragma unroll 8
+            for (int k = 0; k < kBW; ++k) dst[(size_t)k * a.ldv] = s_P[r * kQrP + k] * s_scl[k];
+        }
+    }
+    if (rank == 0) {
+        for (int e = tid; e < kBW * kBW; e += kQrThreads) {
+            const int l = e % kBW, k = e / kBW;
+            if (l < m) {
+                if (l > k) a.V1[(size_t)(j0 + k) * a.ldv + g0 + l] = s_top[l * kQrP + k] * s_scl[k];
+                else {
+                    if (l == k) a.V1[(size_t)(j0 + k) * a.ldv + g0 + l] = mk(1.0, 0.0);
+                    a.AB[(size_t)(j0 + k) * a.ldab + (kBW + l - k)] = s_top[l * kQrP + k];
+                }
+            }
+            a.Tk[e] = s_T[l * kQrP + k];          // column-major b x b
+        }
+        if (tid < kBW) a.tau1[j0 + tid] = s_tau[tid];
+    }
+    cx_barrier();                                // no CTA of the cluster exits while a peer may still address its memory
+}
+
+// last diagonal block(s): no panel below them
+__global__ void he2hb_tail_kernel(int n, int j0, const cplx *__restrict__ A, int lda, cplx *__restrict__ AB, int ldab) {
+    const int w = n - j0;
+    for (int e = threadIdx.x; e < w * w; e += blockDim.x) {
+        const int r = e % w, c = e / w;
+        if (r >= c) AB[(size_t)(j0 + c) * ldab + (r - c)] = A[(size_t)(j0 + c) * lda + j0 + r];
+    }
+}
+
+// ---------------------------------------------------------------- trailing update
+constexpr int HM_MI = 4, HM_NI = 2, HM_WM = 2, HM_WN = 2;       // 64 x 32 CTA tile, 4 warps
+constexpr int HM_THREADS = HM_WM * HM_WN * 32;
+
+struct HemmArgs {
+    int m, lda, ldv, ldz, chunk;
+    const cplx *A22, *V;
+    cplx *Zp;
+};
+struct StoreEpi2 {
+    cplx *C; int ld;
+    __device__ __forceinline__ void operator()(int i, int j, double re, double im) const { C[(size_t)j * ld + i] = mk(re, im); }
+};
+
+// Zp[s] = A22[:, k0:k0+chunk] V[k0:k0+chunk, :]   (blockIdx.x = 64-row tile, blockIdx.y = s)
+__global__ void __launch_bounds__(HM_THREADS, 2) he2hb_hemm_kernel(HemmArgs h) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int k0 = blockIdx.y * h.chunk;
+    int klen = h.m - k0; if (klen > h.chunk) klen = h.chunk; if (klen < 0) klen = 0;
+    GemmProblem<cplx, cplx> p;
+    p.A = h.A22 + (size_t)k0 * h.lda; p.lda = h.lda;
+    p.B = h.V + k0; p.ldb = h.ldv;
+    p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = h.m; p.N = kBW; p.K = klen; p.K2 = 0;
+    StoreEpi2 epi{h.Zp + (size_t)blockIdx.y * h.ldz * kBW, h.ldz};
+    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, HM_MI, HM_NI, HM_WM, HM_WN, false, 2>(p, blockIdx.x, 0, smem_raw, epi);
+}
+
+struct SlabArgs {
+    int m, ldv, ldz, splits, nslabs;
+    const cplx *V, *Zp, *Tk;
+    cplx *Z, *Gp, *S;
+    unsigned *counter;
+};
+
+// 64-row slab: Z = sum_s Zp[s], partial Gram G_c = V_slab^H Z_slab; the last CTA to finish sums the partials in a fixed
+// order (deterministic) and forms S = -1/2 T^H G T.
+__global__ void __launch_bounds__(128) he2hb_slab_kernel(SlabArgs s) {
+    extern __shared__ __align__(16) unsigned char slab_smem[];
+    cplx (*sZ)[kBW + 1] = reinterpret_cast<cplx (*)[kBW + 1]>(slab_smem);
+    cplx (*sV)[kBW + 1] = sZ + 64;
+    __shared__ bool is_last;
+    const int tid = threadIdx.x;
+    const int r0 = blockIdx.x * 64;
+    for (int e = tid; e < 64 * kBW; e += 128) {
+        const int r = e % 64, c = e / 64;
+        cplx z = mk(0.0, 0.0), v = mk(0.0, 0.0);
+        if (r0 + r < s.m) {
+            for (int k = 0; k < s.splits; ++k) z = z + s.Zp[((size_t)k * kBW + c) * s.ldz + r0 + r];
+            s.Z[(size_t)c * s.ldz + r0 + r] = z;
+            v = s.V[(size_t)c * s.ldv + r0 + r];
+        }
+        sZ[r][c] = z; sV[r][c] = v;
+    }
+    __syncthreads();
+    // G[a][c] = sum_r conj(V[r][a]) Z[r][c]: thread = (a, 8 columns)
+    {
+        const int a = tid >> 2, c0 = (tid & 3) * 8;
+        cplx acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = mk(0.0, 0.0);
+        for (int r = 0; r < 64; ++r) {
+            const cplx v = sV[r][a];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) cfma_conj(acc[q], v, sZ[r][c0 + q]);
+        }
+        cplx *gp = s.Gp + (size_t)blockIdx.x * kBW * kBW;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) gp[(c0 + q) * kBW + a] = acc[q];
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned prev = atomicAdd(s.counter, 1u);
+        is_last = (prev == (unsigned)s.nslabs - 1u);
+        if (is_last) *s.counter = 0u;              // self-resetting: the next panel's launch is stream-ordered after this kernel
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // G (into sZ[0..31]), T (into sV[0..31])
+    for (int e = tid; e < kBW * kBW; e += 128) {
+        const int r = e % kBW, c = e / kBW;
+        cplx g = mk(0.0, 0.0);
+        for (int k = 0; k < s.nslabs; ++k) g = g + ldcg_(s.Gp + (size_t)k * kBW * kBW + e);
+        sZ[r][c] = g;
+        sV[r][c] = s.Tk[e];
+    }
+    __syncthreads();
+    // M = G T  (into sZ[32..63])
+    for (int e = tid; e < kBW * kBW; e += 128) {
+        const int r = e % kBW, c = e / kBW;
+        cplx acc = mk(0.0, 0.0);
+        for (int k = 0; k <= c; ++k) cfma(acc, sZ[r][k], sV[k][c]);        // T upper triangular
+        sZ[32 + r][c] = acc;
+    }
+    __syncthreads();
+    // S = -1/2 T^H M
+    for (int e = tid; e < kBW * kBW; e += 128) {
+        const int r = e % kBW, c = e / kBW;
+        cplx acc = mk(0.0, 0.0);
+        for (int k = 0; k <= r; ++k) cfma_conj(acc, sV[k][r], sZ[32 + k][c]);
+        s.S[e] = mk(-0.5 * acc.x, -0.5 * acc.y);
+    }
+}
+
+struct XArgs {
+    int m, ldv, ldz;
+    const cplx *Z, *V, *Tk, *S;
+    cplx *X;
+};
+// X = Z T + V S     (blockIdx.x = 64-row tile)
+__global__ void __launch_bounds__(HM_THREADS, 2) he2hb_x_kernel(XArgs x) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    GemmProblem<cplx, cplx> p;
+    p.A = x.Z; p.lda = x.ldz; p.B = x.Tk; p.ldb = kBW;
+    p.A2 = x.V; p.lda2 = x.ldv; p.B2 = x.S; p.ldb2 = kBW;
+    p.M = x.m; p.N = kBW; p.K = kBW; p.K2 = kBW;
+    StoreEpi2 epi{x.X, x.ldz};
+    gemm_tile_body<cplx, cplx, MNMAJ, KMAJ, false, false, HM_MI, HM_NI, HM_WM, HM_WN, false, 2>(p, blockIdx.x, 0, smem_raw, epi);
+}
+
+// A22 -= X V^H + V X^H on the lower tiles; every updated element is mirrored into the upper triangle, so that the
+// next panel's HEMM reads a plain full matrix
+struct Her2kFullEpi {
+    cplx *C; int ldc;
+    static constexpr bool kRmw = true;
+    __device__ __forceinline__ cplx load(int i, int j) const { return C[(size_t)j * ldc + i]; }
+    __device__ __forceinline__ void store(int i, int j, cplx v, double re, double im) const {
+        v.x -= re; v.y -= im;
+        if (i == j) v.y = 0.0;
+        C[(size_t)j * ldc + i] = v;
+        if (i != j) C[(size_t)i * ldc + j] = conj_(v);
+    }
+};
+constexpr int H2F_MI = 4, H2F_NI = 4, H2F_WM = 2, H2F_WN = 2;
+__global__ void __launch_bounds__(H2F_WM *H2F_WN * 32, 3) he2hb_her2k_kernel(GemmProblem<cplx, cplx> p, Her2kFullEpi epi) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (blockIdx.y > blockIdx.x) return;
+    gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, H2F_MI, H2F_NI, H2F_WM, H2F_WN, true, 2>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+}
+__global__ void __launch_bounds__(H2F_WM *H2F_WN * 32) he2hb_her2k_small_kernel(GemmProblem<cplx, cplx> p, Her2kFullEpi epi) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (blockIdx.y > blockIdx.x) return;
+    gemm_tile_body<cplx, cplx, MNMAJ, MNMAJ, false, true, 2, 2, H2F_WM, H2F_WN, true>(p, blockIdx.x, blockIdx.y, smem_raw, epi);
+}
+
+// ---------------------------------------------------------------- host driver
+static int g_ts_init_dev = -1;
+static int g_ts_ok = 0;
+constexpr size_t kSmemHemm = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, HM_MI, HM_NI, HM_WM, HM_WN, 2>();
+constexpr size_t kSmemH2F = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2F_MI, H2F_NI, H2F_WM, H2F_WN, 2>();
+constexpr size_t kSmemH2Fs = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2F_WM, H2F_WN>();
+constexpr size_t kSmemSlab = sizeof(cplx) * 2 * 64 * (kBW + 1);
+
+int hb2st_init();
+int backq2_init();
+
+static void qr_launch_cfg(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *at, cudaStream_t st) {
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = dim3(kQrCl); cfg.blockDim = dim3(kQrThreads); cfg.dynamicSmemBytes = QrSmem::total; cfg.stream = st;
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kQrCl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+}
+
+int twostage_init() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (g_ts_init_dev == dev) return 0;
+    g_ts_ok = 0;
+    if (cudaFuncSetAttribute(he2hb_hemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemHemm) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(he2hb_slab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemSlab) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(he2hb_x_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemHemm) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(he2hb_her2k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemH2F) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(he2hb_her2k_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemH2Fs) != cudaSuccess) return HPSD_ECUDA_;
+    int rc = hb2st_init();
+    if (rc) return rc;
+    rc = backq2_init();
+    if (rc) return rc;
+    if (cudaFuncSetAttribute(he2hb_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)QrSmem::total) == cudaSuccess &&
+        cudaFuncSetAttribute(he2hb_panel_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+        cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
+        qr_launch_cfg(cfg, at, nullptr);
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, he2hb_panel_kernel, &cfg) == cudaSuccess && nclusters >= 1) g_ts_ok = 1;
+    }
+    cudaGetLastError();            // a device without 16-CTA clusters is not an error: the one-stage path serves it
+    g_ts_init_dev = dev;
+    return 0;
+}
+
+int twostage_available() {
+    if (twostage_init()) return 0;
+    return g_ts_ok;
+}
+
+int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
+    const int n = w.n;
+    int rc = twostage_init();
+    if (rc) return rc;
+    if (!g_ts_ok) return HPSD_ECUDA_;
+    if ((n - 2 * kBW + kQrCl - 1) / kQrCl > kQrRows) return HPSD_ECUDA_;      // rows of the first panel exceed the cluster's shared memory
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    HPSD_CUDA_OK(cudaMemsetAsync(w.V1, 0, sizeof(cplx) * (size_t)w.ldv * n, st));
+    HPSD_CUDA_OK(cudaMemsetAsync(w.AB, 0, sizeof(cplx) * (size_t)w.ldab * n, st));
+    HPSD_CUDA_OK(cudaMemsetAsync(w.tau1, 0, sizeof(cplx) * (size_t)n, st));
+    HPSD_CUDA_OK(cudaMemsetAsync(w.counter, 0, sizeof(unsigned), st));
+    int kp = 0;
+    for (int j0 = 0; j0 < n; j0 += kBW, ++kp) {
+        const int m = n - j0 - kBW;
+        if (m <= 0) {
+            he2hb_tail_kernel<<<1, 256, 0, st>>>(n, j0, w.A, w.lda, w.AB, w.ldab);
+            HPSD_LAUNCH_CHECK();
+            break;
+        }
+        cplx *Tk = w.Tk + (size_t)kp * kBW * kBW;
+        const cplx *V = w.V1 + (size_t)j0 * w.ldv + j0 + kBW;
+        cplx *A22 = w.A + (size_t)(j0 + kBW) * w.lda + j0 + kBW;
+        prof_begin(ST_PANEL, st);
+        {
+            QrArgs a{n, w.lda, w.ldv, w.ldab, j0, w.A, w.V1, w.tau1, Tk, w.AB};
+            cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
+            qr_launch_cfg(cfg, at, st);
+            const cudaError_t e = cudaLaunchKernelEx(&cfg, he2hb_panel_kernel, a);
+            g_launches++;
+            if (e != cudaSuccess) return HPSD_ECUDA_;
+        }
+        prof_end(ST_PANEL, st);
+        prof_begin(ST_HER2K, st);
+        const int mt = (m + 63) / 64;
+        int splits = (2 * sms + mt - 1) / mt;
+        if (splits > kHemmSplitMax) splits = kHemmSplitMax;
+        int chunk = (((m + splits - 1) / splits) + 15) & ~15;
+        splits = (m + chunk - 1) / chunk;
+        HemmArgs h{m, w.lda, w.ldv, w.ldz2, chunk, A22, V, w.Zp};
+        he2hb_hemm_kernel<<<dim3(mt, splits), HM_THREADS, kSmemHemm, st>>>(h);
+        HPSD_LAUNCH_CHECK();
+        SlabArgs s{m, w.ldv, w.ldz2, splits, mt, V, w.Zp, Tk, w.Z, w.Gp, w.S, w.counter};
+        he2hb_slab_kernel<<<mt, 128, kSmemSlab, st>>>(s);
+        HPSD_LAUNCH_CHECK();
+        XArgs x{m, w.ldv, w.ldz2, w.Z, V, Tk, w.S, w.X};
+        he2hb_x_kernel<<<mt, HM_THREADS, kSmemHemm, st>>>(x);
+        HPSD_LAUNCH_CHECK();
+        GemmProblem<cplx, cplx> gp;
+        gp.A = w.X; gp.lda = w.ldz2; gp.B = V; gp.ldb = w.ldv;
+        gp.A2 = V; gp.lda2 = w.ldv; gp.B2 = w.X; gp.ldb2 = w.ldz2;
+        gp.M = m; gp.N = m; gp.K = kBW; gp.K2 = kBW;
+        Her2kFullEpi epi{A22, w.lda};
+        if (m <= 1536) {
+            const int nt = (m + 31) / 32;
+            he2hb_her2k_small_kernel<<<dim3(nt, nt), H2F_WM * H2F_WN * 32, kSmemH2Fs, st>>>(gp, epi);
+        } else {
+            const int nt = (m + 63) / 64;
+            he2hb_her2k_kernel<<<dim3(nt, nt), H2F_WM * H2F_WN * 32, kSmemH2F, st>>>(gp, epi);
+        }
+        HPSD_LAUNCH_CHECK();
+        prof_end(ST_HER2K, st);
+    }
+    return 0;
+}
+
+}  // namespace hpsd

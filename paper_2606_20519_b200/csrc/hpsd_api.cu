@@ -13,6 +13,7 @@
 #include "large.h"
 #include "largepath.h"
 #include "prof.h"
+#include "twostage.h"
 
 namespace hpsd {
 
@@ -379,6 +380,16 @@ int hpsd_set_option(const char *name, int value) {
         g_cluster_tridiag = (value != 0);
         return HPSD_OK;
     }
+    if (std::strcmp(name, "two_stage") == 0) {
+        if (value < 0 || value > 2) return HPSD_EINVAL;
+        g_two_stage = value;
+        return HPSD_OK;
+    }
+    if (std::strcmp(name, "two_stage_min_n") == 0) {
+        if (value < 2) return HPSD_EINVAL;
+        g_two_stage_min_n = value;
+        return HPSD_OK;
+    }
     if (std::strcmp(name, "medium_max_n") == 0) {
         if (value < 0 || value > kMediumMaxN) return HPSD_EINVAL;
         g_opt.medium_max_n = value;
@@ -393,7 +404,8 @@ int hpsd_profile_stage_count(void) { return ST_COUNT; }
 
 const char *hpsd_profile_stage_name(int stage) {
     static const char *names[ST_COUNT] = {"S1_unpack", "S2S3_tridiag_panel", "S2_her2k_trailing", "S4_stedc",
-                                          "S5S6_backtransform", "S7S8_herk_pack", "S9_jacobi", "S10_householder_ql", "n1_clamp"};
+                                          "S5S6_backtransform", "S7S8_herk_pack", "S9_jacobi", "S10_householder_ql", "n1_clamp",
+                                          "S3_bulge_chasing", "S5_backtransform_q2"};
     return (stage >= 0 && stage < ST_COUNT) ? names[stage] : "";
 }
 
@@ -643,6 +655,17 @@ int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void
     int rc = single_large_setup(n, &ws, &pl);
     if (rc) return rc;
     return largepath_tridiag_only(n, in_svec, d, e, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+}
+
+int hpsd_band_width(void) { return kBW; }
+
+int hpsd_reduce_to_band(int n, const double *in_svec, double *band, void *stream) {
+    if (n < 2 || n > kMaxLargeN || !in_svec || !band) return HPSD_EINVAL;
+    g_launches = 0;
+    void *ws; Plan *pl;
+    int rc = single_large_setup(n, &ws, &pl);
+    if (rc) return rc;
+    return largepath_band_only(n, in_svec, reinterpret_cast<cplx *>(band), reinterpret_cast<unsigned char *>(ws) + 256, (cudaStream_t)stream);
 }
 
 int hpsd_release(void) {

@@ -90,6 +90,11 @@ __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const lo
     }
     __syncthreads();
     const double fro2 = sm.red[0];
+    if (nonfinite(fro2)) {                     // NaN / Inf in the block (block-uniform): all-NaN output, info = 2
+        io_fill_nan(io, base, n, tid, THREADS);
+        if (info != nullptr && tid == 0) info[info_idx[blockIdx.x]] = kInfoNonFinite;
+        return;
+    }
     // |a_pq| <= eps ||A||_F / m is negligible: leaves off(A) <= eps ||A||_F in total
     const double tol2 = (kEps * kEps) * fro2 / ((double)m * (double)m);
     __syncthreads();

@@ -32,7 +32,7 @@ extern int g_cluster_tridiag;            // option "cluster_tridiag" (default 1)
 int tridiag_cluster_init();
 int tridiag_cluster_size_ok(int n);      // device-independent part of the test below
 int tridiag_cluster_fits(int n);         // 1 when this device and this n are served by the cluster kernel
-int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st);
+int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf = nullptr);
 
 
 // ---- stedc.cu (S4) ------------------------------------------------------------
@@ -70,6 +70,7 @@ constexpr int kSplitK = 8;        // split of the long K dimension of X = V^H Z
 
 struct BackWs {
     int n, lda, ldz;
+    int voff;          // reflector c has its unit entry at row c + voff: 1 (one-stage reduction) or the band width (two-stage, Q1)
     const cplx *A;     // reflectors V (lower part, cleaned), lda x n
     const cplx *tau;   // n (tau[n-1] = 0)
     cplx *VT;          // lda x n : V_b T_b per block
@@ -77,11 +78,15 @@ struct BackWs {
     cplx *Zc;          // ldz x n : complex scaled eigenvectors of the positive part
     cplx *Xp;          // kSplitK x kNBT x n partial products
     cplx *X;           // kNBT x n
-    int *cnt;          // [0] = p0 (#lambda <= 0), [1] = kpos
+    int *cnt;          // [0] = p0 (#lambda <= 0), [1] = kpos, [2] = non-finite input flag (set by S1)
+    int *info;         // per-block status word (may be null)
 };
 int backherk_init();
 // lam ascending (n), Zt real eigenvectors of T (ldzt x n); writes the projection's svec (and the ADMM v update) through io.
-int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done = false);
+struct TwoStageWs;
+// ts != nullptr: two-stage reduction, Z <- Q1 (Q2 Z) with Q2 from the bulge chasing (backq2.cu, factors already formed)
+int launch_back_herk(const BackWs &w, const double *lam, const double *Zt, int ldzt, const SvecIo &io, cudaStream_t st, bool factors_done = false,
+                     const TwoStageWs *ts = nullptr);
 // the part of S5 that needs the reflectors only (Gram, T_b, V_b T_b); launch_back_herk(..., factors_done = true) then skips it
 int launch_bt_factors(const BackWs &w, cudaStream_t st);
 

@@ -326,13 +326,6 @@ __device__ void med_ql_apply(const MedSmem &sm, int n, int ld) {
     }
 }
 
-#ifdef HPSD_PANEL_TRACE
-__device__ long long g_med_trace[8];
-extern "C" int hpsd_debug_medium(long long *out) { cudaMemcpyFromSymbol(out, g_med_trace, sizeof(long long) * 8); return 0; }
-#define MTRACE(k) do { if (threadIdx.x == 0 && blockIdx.x == 0) g_med_trace[k] = clock64(); } while (0)
-#else
-#define MTRACE(k) do {} while (0)
-#endif
 
 __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const long long *__restrict__ offs,
                                                                    SvecIo io,
@@ -345,34 +338,33 @@ __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const 
     const size_t base = (size_t)offs[blockIdx.x];
 
     // ---- S1: unpack into shared memory, both triangles
+    int bad = 0;
     for (int t = tid; t < n * n; t += kMedThreads) {
         const int j = t / n, i = t % n;
         if (i < j) continue;
         const size_t c = base + svec_col_off(n, j);
-        if (i == j) A[(size_t)j * ld + i] = mk(io_load(io, c), 0.0);
+        if (i == j) { const double d = io_load(io, c); bad |= nonfinite(d); A[(size_t)j * ld + i] = mk(d, 0.0); }
         else {
             const int k = i - j - 1;
             const cplx v = mk(io_load(io, c + 1 + 2 * k) / kSqrt2, io_load(io, c + 2 + 2 * k) / kSqrt2);
+            bad |= nonfinite(v.x) | nonfinite(v.y);
             A[(size_t)j * ld + i] = v;
             A[(size_t)i * ld + j] = conj_(v);
         }
     }
     if (tid < 16) sm.ctl[tid] = 0;
-    __syncthreads();
+    if (__syncthreads_or(bad)) {               // NaN / Inf in the block: all-NaN output, info = 2
+        io_fill_nan(io, base, n, tid, kMedThreads);
+        if (info != nullptr && tid == 0) info[info_idx[blockIdx.x]] = kInfoNonFinite;
+        return;
+    }
 
-    MTRACE(0);
     med_tridiagonalize(sm, n, ld);
-    MTRACE(1);
     med_form_q(sm, n, ld);
-    MTRACE(2);
 
-    if (tid == 0) { med_ql_generate(sm, n); MTRACE(3); }
+    if (tid == 0) med_ql_generate(sm, n);
     else if (tid >= 32) med_ql_apply(sm, n, ld);
     __syncthreads();
-    MTRACE(4);
-#ifdef HPSD_PANEL_TRACE
-    if (tid == 0 && blockIdx.x == 0) g_med_trace[6] = sm.ctl[0];
-#endif
     if (info != nullptr && tid == 0) info[info_idx[blockIdx.x]] = sm.ctl[2] ? 4 : 0;
 
     // ---- S6: clamp, W = Q_+ diag(sqrt(lambda_+)); the positive columns are scaled in place
@@ -409,7 +401,6 @@ __global__ void __launch_bounds__(kMedThreads) hhql_project_kernel(int n, const 
             io_store(io, c + 2 + 2 * k, kSqrt2 * acc.y);
         }
     }
-    MTRACE(5);
 }
 
 // =====================================================================================================
@@ -436,21 +427,33 @@ __global__ void __launch_bounds__(kMedThreads) meddc_tridiag_kernel(int n, const
     cplx *A = sm.A;
     const int tid = threadIdx.x, t = blockIdx.x;
     const size_t base = (size_t)offs[t];
+    int bad = 0;
     for (int q = tid; q < n * n; q += kMedThreads) {
         const int j = q / n, i = q % n;
         if (i < j) continue;
         const size_t c = base + svec_col_off(n, j);
-        if (i == j) A[(size_t)j * ld + i] = mk(io_load(io, c), 0.0);
+        if (i == j) { const double d = io_load(io, c); bad |= nonfinite(d); A[(size_t)j * ld + i] = mk(d, 0.0); }
         else {
             const int k = i - j - 1;
             const cplx v = mk(io_load(io, c + 1 + 2 * k) / kSqrt2, io_load(io, c + 2 + 2 * k) / kSqrt2);
+            bad |= nonfinite(v.x) | nonfinite(v.y);
             A[(size_t)j * ld + i] = v;
             A[(size_t)i * ld + j] = conj_(v);
         }
     }
-    __syncthreads();
-    med_tridiagonalize(sm, n, ld);
     cplx *Ag = w.Ar + (size_t)t * n * w.ld;
+    if (__syncthreads_or(bad)) {
+        // NaN / Inf in the block: the group's divide & conquer gets a zero tridiagonal for it; tau[n-1] (always zero
+        // otherwise) carries the flag to meddc_back_kernel, which writes the all-NaN output
+        for (int q = tid; q < n * n; q += kMedThreads) { const int j = q / n, i = q % n; if (i > j) Ag[(size_t)j * w.ld + i] = mk(0.0, 0.0); }
+        for (int i = tid; i < n; i += kMedThreads) {
+            w.tau[(size_t)t * n + i] = (i == n - 1) ? mk(nan_(), 0.0) : mk(0.0, 0.0);
+            w.d[(size_t)t * n + i] = 0.0;
+            w.e[(size_t)t * n + i] = 0.0;
+        }
+        return;
+    }
+    med_tridiagonalize(sm, n, ld);
     for (int q = tid; q < n * n; q += kMedThreads) {
         const int j = q / n, i = q % n;
         if (i > j) Ag[(size_t)j * w.ld + i] = A[(size_t)j * ld + i];
@@ -481,6 +484,11 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
     }
     for (int i = tid; i < n; i += kMedThreads) { tau[i] = w.tau[(size_t)t * n + i]; lm[i] = lam[(size_t)t * n + i]; }
     __syncthreads();
+    if (tau[n - 1].x != tau[n - 1].x) {        // flag of meddc_tridiag_kernel: non-finite input (block-uniform)
+        io_fill_nan(io, (size_t)offs[t], n, tid, kMedThreads);
+        if (info != nullptr && tid == 0) info[info_idx[t]] = kInfoNonFinite;
+        return;
+    }
     if (tid == 0) {
         int lo = 0, hi = n;                                      // eigenvalues ascending: first index with lam > 0
         while (lo < hi) { const int mid = (lo + hi) >> 1; if (lm[mid] > 0.0) hi = mid; else lo = mid + 1; }

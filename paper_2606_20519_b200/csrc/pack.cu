@@ -8,7 +8,8 @@ namespace hpsd {
 // One CTA handles a chunk of one column j: rows i = j .. n-1.
 // svec column j: [X_jj, s Re X_{j+1,j}, s Im X_{j+1,j}, ...]
 template <int FULL>
-__global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__restrict__ sv, const double *__restrict__ sub, cplx *__restrict__ A, int lda) {
+__global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__restrict__ sv, const double *__restrict__ sub, cplx *__restrict__ A, int lda,
+                                                     int *__restrict__ nf) {
     const int j = blockIdx.y;
     const double *c = sv + svec_col_off(n, j);
     const double *cs = sub ? sub + svec_col_off(n, j) : nullptr;
@@ -22,6 +23,10 @@ __global__ void __launch_bounds__(256) unpack_kernel(int n, const double *__rest
             if (cs) { re -= cs[1 + 2 * k]; im -= cs[2 + 2 * k]; }     // u~ - v of Eq. (D33)
             // division, not multiplication by 1/sqrt2: bit-identical to vec_R^-1 as defined
             v = mk(re / kSqrt2, im / kSqrt2);
+        }
+        if (nonfinite(v.x) || nonfinite(v.y)) {       // the path computes on a sanitised copy; the flag turns the output into NaN
+            v = mk(0.0, 0.0);
+            if (nf) *nf = 1;
         }
         A[(size_t)j * lda + i] = v;
         if (FULL && i != j) A[(size_t)i * lda + j] = conj_(v);
@@ -57,11 +62,11 @@ static dim3 col_grid(int n) {
     return dim3(gx, n, 1);
 }
 
-int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st) {
+int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st, int *nf) {
     if (n <= 0) return 0;
     if (n > 65535) return -1;
-    if (full) unpack_kernel<1><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda);
-    else unpack_kernel<0><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda);
+    if (full) unpack_kernel<1><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda, nf);
+    else unpack_kernel<0><<<col_grid(n), 256, 0, st>>>(n, svec, sub, A, lda, nf);
     HPSD_LAUNCH_CHECK();
     return 0;
 }

@@ -8,14 +8,16 @@ namespace hpsd {
 
 enum Stage {
     ST_UNPACK = 0,      // S1
-    ST_PANEL,           // S2/S3 panel kernel (Householder vectors + Hermitian mat-vec)
-    ST_HER2K,           // S2 trailing update
+    ST_PANEL,           // S2/S3 panel kernel (one-stage: Householder vectors + Hermitian mat-vec; two-stage: panel QR)
+    ST_HER2K,           // S2 trailing update (two-stage: HEMM + corrections + HER2K)
     ST_STEDC,           // S4
     ST_BACK,            // S5 + S6
     ST_HERK_PACK,       // S7 + S8
     ST_JACOBI,          // S9
     ST_MEDIUM,          // S10
     ST_SCALAR,          // n = 1 blocks
+    ST_BULGE,           // S3 band -> tridiagonal (two-stage reduction)
+    ST_BACKQ2,          // S5, second back-transformation (two-stage reduction)
     ST_COUNT
 };
 

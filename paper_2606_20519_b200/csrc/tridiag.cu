@@ -51,20 +51,6 @@ struct PanelArgs {
     const int2 *tiles;      // lower-triangle tile list, tile column descending
 };
 
-#ifdef HPSD_PANEL_TRACE
-// dev-only: per-column phase timestamps of CTA 0 and CTA G/2 (clock64) of panel number (armed - 1)
-__device__ long long g_trace[2 * 32 * 16];
-__device__ int g_trace_armed = 0;
-#define TRACE(slot)                                                                                   \
-    do {                                                                                              \
-        if (trace_on)                                                                                 \
-            g_trace[((g == 0 ? 0 : 1) * 32 + i) * 16 + (slot)] = clock64();                             \
-    } while (0)
-#define TRACE_USE(val) do { if (trace_on && (val) == 1.2345e300) g_trace[0] = 0; } while (0)
-#else
-#define TRACE(slot) do {} while (0)
-#define TRACE_USE(val) do {} while (0)
-#endif
 
 __device__ __forceinline__ cplx group8_sum(cplx v) {
 #pragma unroll
@@ -177,9 +163,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
     const int g = blockIdx.x, G = p.G;
     const int n = p.n, lda = p.lda, ldw = p.ldw, ldp = p.ldp;
     cplx *A = p.A, *W = p.W;
-#ifdef HPSD_PANEL_TRACE
-    const bool trace_on = (tid == 0 && g_trace_armed >= 1 && p.j0 == (g_trace_armed - 1) * kNB && (g == 0 || g == G / 2));
-#endif
     constexpr int PSTRIDE = 2 * kNB + 1;
     const int T = p.T, q = p.q;
     const bool streaming = q > kSlots;
@@ -252,7 +235,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         const int c = p.j0 + i;
         if (c >= n - 1) break;
         // ================= phase A: y = A22 v over this CTA's tiles (no block-level sync) =================
-        TRACE(0);
         // raw pieces of column c for this warp's first tiles: issued before anything that waits
         // Tiles are walked forwards on even columns and backwards on odd ones: when they stream, the tail
         // of one pass is the head of the next, so it is still in the slots / in L2.
@@ -322,7 +304,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         }
         __syncthreads();
         const cplx tau = s_sc[0], scale = s_sc[1];
-        TRACE(1);
         if (reducer && lane == 0)     // row c+1 term (v = 1 there) plus scale * sum over rows >= c+2
             p.tot[(g / kNB) * kNB + (g % kNB)] = conj_(red_top) + scale * red_s;
         double qacc = 0.0;
@@ -481,7 +462,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         }
         if (!wide) qacc = warp_sum(qacc);
         if (lane == 0) s_q[warp] = qacc;
-        TRACE(2);
         __syncthreads();
         if (tid == 0 && g < T) {
             double t = 0.0;
@@ -490,7 +470,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
         }
         grid.sync();
 
-        TRACE(3);
         // ================= phase B: rows spread over the CTAs; one dependent L2 round trip =================
         // lane = row (31 consecutive rows per CTA; lane 31 is the helper row c+1, whose w every CTA needs
         // for the next-column update); warp w serves tile columns b = J0 + w (mod 8) of the partials and
@@ -531,7 +510,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 // in L2: ~1000 requests per line per column at n = 4096, queued for microseconds)
                 cplx totV = mk(0.0, 0.0), totW = mk(0.0, 0.0);
                 if (warp == 2 && lane < i) { totV = ldx_(&p.tot[lane]); totW = ldx_(&p.tot[kNB + lane]); }
-                TRACE(8);
                 cplx Vr[kNB / 8], Wr[kNB / 8];
 #pragma unroll
                 for (int k = 0; k < kNB / 8; ++k) {
@@ -557,11 +535,6 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                         p1 = p1 + (((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7])));
                     }
                 }
-                TRACE(9);
-                TRACE_USE(ar.x + anx.x);
-                TRACE(10);
-                TRACE_USE(p1.x);
-                TRACE(11);
                 if (warp == 1) qv = warp_sum((qv0 + qv1) + (qv2 + qv3) + qv4);
                 if (warp == 2) { s_cV[lane] = totV; s_cW[lane] = totW; }
                 __syncthreads();                                  // cV, cW visible; previous pass / previous column readers done
@@ -581,13 +554,11 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                     cfma(p2, Vr[k], conj_(w1)); cfma(p2, Wr[k], conj_(v1));
                     re += cvk.x * cwk.x + cvk.y * cwk.y;
                 }
-                TRACE(4);
                 s_p1[warp * 32 + lane] = p1;
                 s_p2[warp * 32 + lane] = p2;
                 if (lane == 0) s_re[warp] = re;
                 if (warp == 1 && lane == 0) s_q[8] = qv;
                 __syncthreads();
-                TRACE(5);
                 cplx ys = mk(0.0, 0.0), upd = mk(0.0, 0.0);
                 double ret = 0.0;
 #pragma unroll
@@ -634,9 +605,7 @@ __global__ void __launch_bounds__(kPanelThreads, 1) tridiag_panel_kernel(PanelAr
                 }
             }
         }
-        TRACE(6);
         if (i + 1 < p.nbp) grid.sync();
-        TRACE(7);
     }
     // no bulk copy may be in flight when the CTA exits (a one-column last panel never reads its tiles)
     if (wide) { if (warp < 2 && warp < q && g + warp * G < T) mbar_wait(mbar0 + 8u * warp, 0u); }
@@ -703,13 +672,6 @@ int tridiag_init() {
     return 0;
 }
 
-#ifdef HPSD_PANEL_TRACE
-extern "C" int hpsd_debug_trace(int arm, long long *out) {
-    if (arm >= 0) cudaMemcpyToSymbol(g_trace_armed, &arm, sizeof(int));
-    if (out) cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 2 * 32 * 16);
-    return 0;
-}
-#endif
 
 int tridiag_tile_size(int) { return kTS; }
 

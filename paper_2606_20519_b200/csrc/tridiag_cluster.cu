@@ -35,7 +35,7 @@
 //
 // Measured on B200 (round 1), S1+S2+S3 alone: n = 200 0.70 ms (grid-wide panel kernel 1.31), n = 400 1.97 (2.70),
 // n = 625 3.93 (4.37).  Every warp walks a serial chain of ~10 trips of ~1500 cycles per column step (t_j warp
-// reductions and the issue overhead around the 16 DFMA per element), so the FP64 pipe is ~25 % busy at n = 625.
+// reductions and the issue overhead around the 16 DFMA per element), so the FP64 pipe of the 16 SMs is 17 % busy at n = 625 (ncu, profiles/r1_cluster_ncu_full.md).
 #include <cooperative_groups.h>
 #include "kernels.h"
 #include "large.h"
@@ -91,6 +91,7 @@ struct ClusterArgs {
     cplx *raw;                     // 2 x lda ring of exported raw columns
     double *d, *e;
     cplx *tau;
+    int *nf;                       // device flag: non-finite input seen
 };
 
 __host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + kCl - 1) / kCl : 0; }
@@ -140,25 +141,21 @@ __device__ __forceinline__ void cl_householder(cplx alpha, double xnorm2, double
 }
 
 // element (i, j), i >= j, of the input matrix from the svec (Eq. D10 inverted; same arithmetic as unpack_kernel)
-__device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, const double *__restrict__ sub, int n, int i, int j) {
+// non-finite entries are replaced by zero and *nf is set (common.cuh: the output block becomes NaN)
+__device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, const double *__restrict__ sub, int n, int i, int j, int *nf) {
     const size_t o = svec_col_off(n, j);
-    if (i == j) return mk(sub ? sv[o] - sub[o] : sv[o], 0.0);
-    const size_t k = o + 1 + 2 * (size_t)(i - j - 1);
-    double re = sv[k], im = sv[k + 1];
-    if (sub) { re -= sub[k]; im -= sub[k + 1]; }
-    return mk(re / kSqrt2, im / kSqrt2);
+    cplx v;
+    if (i == j) v = mk(sub ? sv[o] - sub[o] : sv[o], 0.0);
+    else {
+        const size_t k = o + 1 + 2 * (size_t)(i - j - 1);
+        double re = sv[k], im = sv[k + 1];
+        if (sub) { re -= sub[k]; im -= sub[k + 1]; }
+        v = mk(re / kSqrt2, im / kSqrt2);
+    }
+    if (nonfinite(v.x) || nonfinite(v.y)) { v = mk(0.0, 0.0); if (nf) *nf = 1; }
+    return v;
 }
 
-#ifdef HPSD_PANEL_TRACE
-// dev-only: clock64 at eight points of every 8th column step, CTA 0 / thread 0
-__device__ long long g_cltrace[128 * 8];
-__device__ long long g_cltrace2[8 * 16 * 4];
-#define CLT2(pt) do { if (r == 0 && lane == 0 && c == 0) g_cltrace2[(wp * 16 + (((jl - jl0) >> 2) & 15)) * 4 + (pt)] = clock64(); } while (0)
-#define CLTRACE(slot) do { if (r == 0 && tid == 0 && (c & 7) == 0 && (c >> 3) < 128) g_cltrace[(c >> 3) * 8 + (slot)] = clock64(); } while (0)
-#else
-#define CLTRACE(slot) do {} while (0)
-#define CLT2(pt) do {} while (0)
-#endif
 
 // One row chunk x kKT own columns of the fused pass.  x holds A(i, j_k) (zero where the element does not exist), m says
 // where it exists.  Branch-free: masks are selects (a predicate-free variant behind a warp-uniform branch was slower).
@@ -207,7 +204,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
     for (int jl = wp; jl < nc; jl += kClWarps) {
         const int j = r + kCl * jl;
         cplx *col = stor + cl_col_off(n, r, jl);
-        for (int i = j + lane; i < n; i += 32) col[i - j] = cl_load_svec(p.in, p.sub, n, i, j);
+        for (int i = j + lane; i < n; i += 32) col[i - j] = cl_load_svec(p.in, p.sub, n, i, j, p.nf);
     }
     int row[kClR], dest[kClR], dslot[kClR];
     cplx v[kClR], w[kClR], u[kClR], z[kClR], raw[kClR];
@@ -216,7 +213,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         row[s] = 32 * cl_chunk(s, wp) + lane;
         dest[s] = row[s] / RS; dslot[s] = row[s] - dest[s] * RS;       // reducer CTA of the row and its slot there
         v[s] = w[s] = u[s] = z[s] = mk(0.0, 0.0);
-        raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0) : mk(0.0, 0.0);
+        raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0, p.nf) : mk(0.0, 0.0);
     }
     cplx wc = mk(0.0, 0.0);
     const unsigned mbar1 = (unsigned)__cvta_generic_to_shared(smem_raw + L.mbar), mbar2 = mbar1 + 8;
@@ -243,7 +240,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
 
     for (int c = 0; c < n; ++c) {
         // ================= [A] column c of the current matrix, Householder vector =================
-        CLTRACE(0);
         cplx a[kClR];
         double xn = 0.0;
 #pragma unroll
@@ -263,7 +259,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         xn = warp_sum(xn);
         if (lane == 0) s_red[kRedN + wp] = xn;
         __syncthreads();
-        CLTRACE(1);
         const double dc = s_red[kRedS + 2];
         if (c == n - 1) {
             if (r == (c & (kCl - 1))) {
@@ -294,7 +289,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             for (int s = 0; s < kClR; ++s) if (row[s] < n) p.A[(size_t)c * lda + row[s]] = u[s];   // zero for rows <= c
         }
         __syncthreads();
-        CLTRACE(2);
 
         // ================= [B] fused rank-2 update (step c-1) + Hermitian mat-vec (step c) =================
         // Four own columns per trip: twelve independent element chains per thread hide the shared-memory
@@ -333,7 +327,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         for (; jl < nc; jl += kKT) {
             const int j0 = r + kCl * jl;
             if (j0 >= top_end) break;                              // warp-uniform
-            CLT2(0);
             cplx cv[kKT], cw[kKT], cu[kKT], tj[kKT];
             cplx *col[kKT];
 #pragma unroll
@@ -359,7 +352,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                     if (m[s][k]) x[s][k] = col[k][i0];
                 }
             }
-            CLT2(1);
 #pragma unroll
             for (int s = 0; s < kClR; ++s) {
                 const int i0 = 32 * cl_chunk(s, wp), i = i0 + lane;
@@ -368,7 +360,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 // warp-uniform branch costs more than the ~11 select/compare instructions per element it saves)
                 cl_elems(x[s], m[s], i, j0, col, i0, v[s], w[s], u[s], cv, cw, cu, z[s], tj);
             }
-            CLT2(2);
             // halving butterfly: kKT values x 32 lanes -> lane 32 q / kKT holds the total of column q
             {
                 cplx kp;
@@ -396,7 +387,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 const int idx = lane / (32 / kKT);
                 if ((lane & (32 / kKT - 1)) == 0 && jl + idx < nc) tpart[wp * ncw + jl + idx] = kp;
             }
-            CLT2(3);
         }
         for (int q = jl + lane; q < nc; q += 32) tpart[wp * ncw + q] = mk(0.0, 0.0);   // columns beyond this warp's rows
         if (owner) {
@@ -407,7 +397,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             if (lane < kCl) cl_st_async(cl_mapa(tok_a + 8u * (unsigned)wp, lane), 1.0, cl_mapa(mbar1, lane));
         }
         __syncthreads();
-        CLTRACE(3);
 
         // ================= [C] contributions to y = A v: reduce-scatter through DSMEM =================
         // Rows [rho RS, (rho+1) RS) are summed by CTA rho, so a warp's 32 consecutive rows go to at most two
@@ -430,7 +419,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         qp = warp_sum(qp);
         if (lane == 0) s_red[kRedQ + wp] = qp;
         __syncthreads();
-        CLTRACE(4);
         cl_wait(mbar1, c & 1);                                    // every contribution to my rows has landed
         if (tid == 0) cl_arm(mbar1, bytes_r(c + 1));
         if (tid < kCl) {
@@ -442,7 +430,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
             for (int k = 0; k < kClWarps; ++k) q += s_red[kRedQ + k];
             cl_st_async(cl_mapa(sq_a + 8u * (unsigned)((c & 1) * kCl + r), tid), q, cl_mapa(mbar2, tid));
         }
-        CLTRACE(5);
 
         // ================= [D] sum the contributions of my rows, broadcast tau y =================
         const cplx *rawc = p.raw + (size_t)((c + 1) & 1) * lda;
@@ -467,7 +454,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
                 for (int k = 0; k < 4; ++k) cl_st_async(cl_mapa(wbuf_a + 16u * (unsigned)i, 4 * part + k), ty, cl_mapa(mbar2, 4 * part + k));
             }
         }
-        CLTRACE(6);
         cl_wait(mbar2, c & 1);                                    // all of tau y has landed
         // one 8-byte token to every CTA on phase 1 of the NEXT step: a peer completes that phase only after I have
         // completed phase 2 of this step, so its phase-2 traffic of step c+1 cannot arrive here early
@@ -477,7 +463,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         for (int k = 0; k < kCl; ++k) q += s_q[(c & 1) * kCl + k];
         const double alphap = -0.5 * abs2(tau) * q;
         if (tid == 0) cl_arm(mbar2, bytes_w(c + 1));
-        CLTRACE(7);
 #pragma unroll
         for (int s = 0; s < kClR; ++s) {
             const int i = row[s];
@@ -489,14 +474,6 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
 }
 
 // ---------------------------------------------------------------- host side
-#ifdef HPSD_PANEL_TRACE
-extern "C" int hpsd_debug_cltrace2(long long *out) {
-    return cudaMemcpyFromSymbol(out, g_cltrace2, sizeof(long long) * 8 * 16 * 4) == cudaSuccess ? 0 : -1;
-}
-extern "C" int hpsd_debug_cltrace(long long *out) {
-    return cudaMemcpyFromSymbol(out, g_cltrace, sizeof(long long) * 128 * 8) == cudaSuccess ? 0 : -1;
-}
-#endif
 int g_cluster_tridiag = 1;
 static int g_cl_init_dev = -1;
 static int g_cl_ok = 0;            // 1: 16-CTA clusters with the maximum shared memory are launchable on this device
@@ -544,9 +521,9 @@ int tridiag_cluster_fits(int n) {
 }
 
 // S1 + S2 + S3 in one launch.  w.W (ldw x kNB) hosts the raw-column ring.
-int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st) {
+int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf) {
     ClusterArgs a;
-    a.n = w.n; a.lda = w.lda; a.in = in; a.sub = sub; a.A = w.A; a.raw = w.W; a.d = w.d; a.e = w.e; a.tau = w.tau;
+    a.n = w.n; a.lda = w.lda; a.in = in; a.sub = sub; a.A = w.A; a.raw = w.W; a.d = w.d; a.e = w.e; a.tau = w.tau; a.nf = nf;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(kCl); cfg.blockDim = dim3(kClThreads); cfg.dynamicSmemBytes = cl_smem_max(w.n); cfg.stream = st;
     cudaLaunchAttribute at[1];

@@ -27,6 +27,16 @@ def hp():
     return lib
 
 
+def _record(what, errs):
+    """Append observed parity errors to gpurun_out/parity_observed.txt (a run log, not an expected value)."""
+    try:
+        os.makedirs("gpurun_out", exist_ok=True)
+        with open("gpurun_out/parity_observed.txt", "a") as f:
+            f.write(what + ": " + ", ".join(f"n={k} rel_err={v:.3e}" for k, v in errs.items()) + "\n")
+    except OSError:
+        pass
+
+
 def force_large(hp, on):
     """Route every block through S1..S8 of the multi-kernel path (on) or restore the defaults (off)."""
     hp.set_option("jacobi_max_n", 1 if on else 32)
@@ -71,9 +81,21 @@ def check_vs_oracle(orc, hp, sizes, sv, nthreads=1):
     return got, want
 
 
-def check_invariants(hp, sizes, sv, out):
-    """Projection invariants on the GPU output alone: idempotence,
-    Moreau X = P(X) - P(-X), <P, P - X> = 0, and P(-X) = P(X) - X >= 0."""
+def _cholesky_ok(M):
+    try:
+        np.linalg.cholesky(M)
+        return True
+    except np.linalg.LinAlgError:
+        return False
+
+
+def check_invariants(orc, hp, sizes, sv, out):
+    """Projection invariants on the GPU output.  The KKT triple of the projection onto a
+    self-dual cone (Moreau) is a COMPLETE certificate of P = Pi(X):
+        P >= 0,   P - X >= 0,   <P, P - X> = 0.
+    Both semidefiniteness tests are host-side Cholesky factorisations (numpy/LAPACK) of P + tol I and
+    (P - X) + tol I, i.e. independent of the library under test; the inner product is an svec dot product
+    (PAPER.md:1224-1226).  Idempotence and X = P(X) - P(-X) go through the library again."""
     n = max(sizes)
     nx = np.linalg.norm(sv)
     p2 = gpu_project(hp, sizes, out)
@@ -81,13 +103,15 @@ def check_invariants(hp, sizes, sv, out):
     pm = gpu_project(hp, sizes, -sv)
     assert np.linalg.norm(out - pm - sv) <= TOL * n * nx
     assert abs(out @ (out - sv)) <= TOL * n * nx * nx
-    # PSD: the smallest eigenvalue of P (through the library's own eigenvalue entry) is >= -tol
-    import torch
     off = 0
     for nb in sizes:
-        if nb >= 2:
-            lam = hp.eigvalsh(torch.from_numpy(out[off:off + nb * nb].copy()).cuda(), nb).cpu().numpy()
-            assert lam.min() >= -TOL * nb * max(np.linalg.norm(sv[off:off + nb * nb]), 1e-300)
+        if nb >= 1:
+            seg_x, seg_p = sv[off:off + nb * nb], out[off:off + nb * nb]
+            tol = TOL * nb * max(np.linalg.norm(seg_x), 1e-300)
+            P = orc.unpack(seg_p, nb)
+            assert _cholesky_ok(P + tol * np.eye(nb)), ("P not PSD", nb, off)
+            assert _cholesky_ok(orc.unpack(seg_p - seg_x, nb) + tol * np.eye(nb)), ("P - X not PSD", nb, off)
+            assert abs(seg_p @ (seg_p - seg_x)) <= TOL * nb * max(np.linalg.norm(seg_x), 1e-300) ** 2
         off += nb * nb
 
 
@@ -116,14 +140,14 @@ def test_config1_n16(orc, hp):
     b = w.blocks[0]
     closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
     assert rel_err(got, closed) <= TOL * 16
-    check_invariants(hp, w.sizes, sv, got)
+    check_invariants(orc, hp, w.sizes, sv, got)
 
 
 def test_config2_256x81(orc, hp):
     w = workloads.make(2)
     sv = pack_all(orc, [b.X for b in w.blocks])
     got, _ = check_vs_oracle(orc, hp, w.sizes, sv, nthreads=1)
-    check_invariants(hp, w.sizes, sv, got)
+    check_invariants(orc, hp, w.sizes, sv, got)
 
 
 def test_config3_n625(orc, hp):
@@ -133,26 +157,27 @@ def test_config3_n625(orc, hp):
     b = w.blocks[0]
     closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
     assert rel_err(got, closed) <= TOL * 625
-    check_invariants(hp, w.sizes, sv, got)
+    check_invariants(orc, hp, w.sizes, sv, got)
 
 
 def test_config4_mixed_full_size(orc, hp):
-    """Full config 4 in ONE call (1296 + 2401 + 64 x 36).  Oracle element by element on the n=1296
-    block and all n=36 blocks; the n=2401 block (oracle: minutes) by invariants, and by the oracle
-    too when HPSD_FULL_ORACLE=1."""
+    """Full config 4 in ONE call (1296 + 2401 + 64 x 36): every block element by element against the oracle
+    (the n = 2401 block, the only GUE-type matrix above n = 1296, takes the threaded oracle about a minute),
+    then the library-independent KKT certificate."""
     w = workloads.make(4)
     sizes = w.sizes
     sv = pack_all(orc, [b.X for b in w.blocks])
     got = gpu_project(hp, sizes, sv)
     offs = np.concatenate([[0], np.cumsum([n * n for n in sizes])])
-    full = os.environ.get("HPSD_FULL_ORACLE") == "1"
+    worst = {}
     for k, n in enumerate(sizes):
-        if n == 2401 and not full:
-            continue
         seg = sv[offs[k]:offs[k + 1]]
         want = orc.project([n], seg, nthreads=orc.max_threads() if n > 100 else 1)
-        assert rel_err(got[offs[k]:offs[k + 1]], want) <= TOL * n, (k, n)
-    check_invariants(hp, sizes, sv, got)
+        err = rel_err(got[offs[k]:offs[k + 1]], want)
+        worst[n] = max(worst.get(n, 0.0), err)
+        assert err <= TOL * n, (k, n, err)
+    _record("config4 vs oracle", {str(k): v for k, v in worst.items()})
+    check_invariants(orc, hp, sizes, sv, got)
 
 
 def test_config4_permuted_block_order(orc, hp):
@@ -184,10 +209,13 @@ def test_config5_n4096_closed_form_and_invariants(orc, hp):
     got = gpu_project(hp, [4096], sv)
     closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
     assert rel_err(got, closed) <= TOL * 4096
-    check_invariants(hp, [4096], sv, got)
+    check_invariants(orc, hp, [4096], sv, got)
+    _record("config5 vs closed form", {"4096": rel_err(got, closed)})
     if os.environ.get("HPSD_FULL_ORACLE") == "1":
         want = orc.project([4096], sv, nthreads=orc.max_threads())
-        assert rel_err(got, want) <= TOL * 4096
+        err = rel_err(got, want)
+        _record("config5 vs oracle", {"4096": err})
+        assert err <= TOL * 4096
 
 
 @pytest.mark.parametrize("n", [1891, 1930])
@@ -202,7 +230,7 @@ def test_panel_kernel_first_streamed_sizes_closed_form(orc, hp, n):
     got = gpu_project(hp, [n], sv)
     closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
     assert rel_err(got, closed) <= TOL * n
-    check_invariants(hp, [n], sv, got)
+    check_invariants(orc, hp, [n], sv, got)
 
 
 # ------------------------------------------------------------------ sizes across both paths
@@ -216,7 +244,7 @@ def test_small_path_sizes(orc, hp, n):
     hp.set_option("jacobi_max_n", 84)
     try:
         got, _ = check_vs_oracle(orc, hp, sizes, sv)
-        check_invariants(hp, sizes, sv, got)
+        check_invariants(orc, hp, sizes, sv, got)
     finally:
         hp.set_option("jacobi_max_n", 32)
 
@@ -230,7 +258,7 @@ def test_medium_path_sizes(orc, hp, n):
     hp.set_option("medium_reroute", 0)          # keep the one-CTA kernels on the path (3 blocks of 84..116 would be rerouted)
     try:
         got, _ = check_vs_oracle(orc, hp, sizes, sv)
-        check_invariants(hp, sizes, sv, got)
+        check_invariants(orc, hp, sizes, sv, got)
     finally:
         hp.set_option("medium_reroute", 1)
     rerouted, _ = check_vs_oracle(orc, hp, sizes, sv)  # default dispatch (large path for few blocks of 84..116)
@@ -280,10 +308,156 @@ def test_large_path_sizes(orc, hp, n, cluster):
     hp.set_option("cluster_tridiag", cluster)
     try:
         got, _ = check_vs_oracle(orc, hp, [n], sv, nthreads=orc.max_threads() if n > 150 else 1)
-        check_invariants(hp, [n], sv, got)
+        check_invariants(orc, hp, [n], sv, got)
     finally:
         force_large(hp, False)
         hp.set_option("cluster_tridiag", 1)
+
+
+# ------------------------------------------------------------------ two-stage reduction (S2 dense -> band, S3 bulge chasing, Q2)
+
+TS_SIZES = [96, 97, 127, 128, 129, 160, 200, 257, 320, 449, 625]
+
+
+def _band_to_dense(band, n, b):
+    B = np.zeros((n, n), complex)
+    for t in range(min(2 * b, n)):
+        idx = np.arange(n - t)
+        B[idx + t, idx] = band[:n - t, t]
+    return B + np.tril(B, -1).conj().T
+
+
+@pytest.mark.parametrize("n", TS_SIZES + [1296])
+def test_two_stage_band_reduction(orc, hp, n):
+    """S2 alone (hpsd_reduce_to_band): the band matrix is unitarily similar to the input (eigenvalues against numpy's
+    eigvalsh of the input, a third opinion), Hermitian with a real diagonal, and nothing is stored
+    outside the band width (rows b+1.. of the band storage are the bulge area of S3 and must be zero)."""
+    import torch
+    rng = np.random.default_rng(700 + n)
+    X = herm(rng, n, 1 / np.sqrt(n))
+    b = hp.band_width()
+    band = hp.reduce_to_band(torch.from_numpy(orc.pack(X)).cuda(), n).cpu().numpy()
+    assert np.abs(band[:, b + 1:]).max() == 0.0
+    assert np.abs(band[:, 0].imag).max() == 0.0
+    lam = np.linalg.eigvalsh(X)
+    lb = np.linalg.eigvalsh(_band_to_dense(band, n, b))
+    assert np.abs(lb - lam).max() <= 50 * n * EPS * np.abs(lam).max()
+    assert abs(np.linalg.norm(band[:, 0]) ** 2 + 2 * np.linalg.norm(band[:, 1:]) ** 2 - np.linalg.norm(X) ** 2) <= 1e-12 * n * np.linalg.norm(X) ** 2
+
+
+@pytest.mark.parametrize("n", TS_SIZES + [1296])
+def test_two_stage_tridiagonal(orc, hp, n):
+    """S2 + S3 (option two_stage = 1): the REAL tridiagonal (d, e) has the eigenvalues of the input."""
+    import torch
+    rng = np.random.default_rng(720 + n)
+    X = herm(rng, n, 1 / np.sqrt(n))
+    hp.set_option("two_stage", 1)
+    try:
+        d, e = hp.tridiagonalize(torch.from_numpy(orc.pack(X)).cuda(), n)
+        d, e = d.cpu().numpy(), e.cpu().numpy()
+    finally:
+        hp.set_option("two_stage", 0)
+    lam = np.linalg.eigvalsh(X)
+    lt = np.linalg.eigvalsh(np.diag(d) + np.diag(e, 1) + np.diag(e, -1))
+    assert np.abs(lt - lam).max() <= 50 * n * EPS * np.abs(lam).max()
+
+
+@pytest.mark.parametrize("n", TS_SIZES)
+def test_two_stage_whole_path(orc, hp, n):
+    """The whole projection through S2 (band) + S3 (bulge chasing) + S4 + Q2 + Q1 + HERK against the oracle, and
+    against the one-stage route of the same block."""
+    rng = np.random.default_rng(740 + n)
+    sv = orc.pack(herm(rng, n))
+    force_large(hp, True)
+    try:
+        one = gpu_project(hp, [n], sv)
+        hp.set_option("two_stage", 1)
+        got, _ = check_vs_oracle(orc, hp, [n], sv, nthreads=orc.max_threads() if n > 150 else 1)
+        check_invariants(orc, hp, [n], sv, got)
+        assert rel_err(got, one) <= TOL * n
+    finally:
+        hp.set_option("two_stage", 0)
+        force_large(hp, False)
+
+
+@pytest.mark.parametrize("n", [150, 300])
+def test_two_stage_degenerate_inputs(orc, hp, n):
+    """Edge cases of the method on the two-stage route: already banded / tridiagonal / diagonal input (every
+    reflector is trivial), rank one, exactly repeated eigenvalues, zero."""
+    rng = np.random.default_rng(760 + n)
+    force_large(hp, True)
+    hp.set_option("two_stage", 1)
+    try:
+        for name, X in _special_cases(rng, n).items():
+            X = 0.5 * (X + X.conj().T)
+            sv = orc.pack(X)
+            got = gpu_project(hp, [n], sv)
+            want = orc.project([n], sv, nthreads=orc.max_threads())
+            assert parity_err(got, want, sv, n) <= TOL * n, name
+    finally:
+        hp.set_option("two_stage", 0)
+        force_large(hp, False)
+
+
+@pytest.mark.parametrize("n", [1296, 2401])
+def test_two_stage_config_sizes_closed_form(orc, hp, n):
+    """Paper sizes d = 6, 7 on the two-stage route against the closed form from the generator's own Q and lambda
+    (no eigensolver involved) and the library-independent KKT certificate."""
+    rng = np.random.default_rng(workloads.BASE_SEED + 300 + n)
+    b = workloads.from_spectrum(rng, workloads.spectrum_admm_lowrank(rng, n, n_big=8, sd=1e-1))
+    sv = orc.pack(b.X)
+    hp.set_option("two_stage", 1)
+    try:
+        got = gpu_project(hp, [n], sv)
+        closed = orc.pack((b.Q * np.maximum(b.lam, 0)[None, :]) @ b.Q.conj().T)
+        err = rel_err(got, closed)
+        _record("two-stage vs closed form", {str(n): err})
+        assert err <= TOL * n
+        check_invariants(orc, hp, [n], sv, got)
+    finally:
+        hp.set_option("two_stage", 0)
+
+
+# ------------------------------------------------------------------ non-finite input
+
+@pytest.mark.parametrize("n,route", [(16, "jacobi"), (40, "meddc"), (100, "hhql"), (150, "cluster"), (150, "panel"), (150, "two_stage")])
+@pytest.mark.parametrize("bad", [np.nan, np.inf, -np.inf])
+def test_nonfinite_input_gives_nan_block(orc, hp, n, route, bad):
+    """include/hpsd.h: a block with a NaN/Inf entry gets an all-NaN output block and info = 2; its neighbours in
+    the same call are projected as usual (the paper is silent on non-finite input, DESIGN.md readings)."""
+    import torch
+    rng = np.random.default_rng(900 + n)
+    mats = [herm(rng, n), herm(rng, n), herm(rng, 5)]
+    sv = pack_all(orc, mats)
+    sizes = [n, n, 5]
+    clean = sv.copy()
+    sv[n * n + (n * n) // 3] = bad                        # somewhere inside block 1
+    hp.set_option("medium_reroute", 0)
+    if route in ("cluster", "panel", "two_stage"):
+        force_large(hp, True)
+        hp.set_option("jacobi_max_n", 8)                  # the 5 x 5 neighbour stays on the Jacobi kernel
+    if route == "panel":
+        hp.set_option("cluster_tridiag", 0)
+    if route == "two_stage":
+        hp.set_option("two_stage", 1)
+    try:
+        t = torch.from_numpy(sv).cuda()
+        ws = torch.empty(hp.workspace_size(sizes), dtype=torch.uint8, device="cuda")
+        info = torch.zeros(len(sizes), dtype=torch.int32, device="cuda")
+        out = torch.empty_like(t)
+        hp.project_ws(sizes, t, out, ws, info=info)
+        torch.cuda.synchronize()
+        got, inf = out.cpu().numpy(), info.cpu().numpy()
+        want = orc.project(sizes, clean)
+    finally:
+        force_large(hp, False)
+        hp.set_option("medium_reroute", 1)
+        hp.set_option("cluster_tridiag", 1)
+        hp.set_option("two_stage", 0)
+    assert np.isnan(got[n * n:2 * n * n]).all()
+    assert list(inf) == [0, 2, 0]
+    assert rel_err(got[:n * n], want[:n * n]) <= TOL * n
+    assert rel_err(got[2 * n * n:], want[2 * n * n:]) <= TOL * n
 
 
 # ------------------------------------------------------------------ degenerate inputs
