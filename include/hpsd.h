@@ -67,7 +67,10 @@ const char *hpsd_strerror(int code);
  *   in_svec   DEVICE pointer, sum_b n_b^2 doubles, layout above (read only)
  *   out_svec  DEVICE pointer, same length (may equal in_svec)
  *   stream    cudaStream_t
- * Uses a library-owned, per-device workspace that grows on demand. */
+ * Uses a library-owned, per-device workspace that grows on demand and a cached plan per size list.  Calls on
+ * different streams (or from different host threads) are safe: they are ordered on the shared workspace with an
+ * event, i.e. they serialise; use one hpsd_plan (or hpsd_project_ws with a workspace) per stream for concurrency.
+ * A call captured by the caller into a CUDA graph is the caller's to order against other users of the library. */
 int hpsd_project(int n_blocks, const int *sizes,
                  const double *in_svec, double *out_svec, void *stream);
 
@@ -81,6 +84,28 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes);
 int hpsd_project_ws(int n_blocks, const int *sizes,
                     const double *in_svec, double *out_svec,
                     void *ws, size_t ws_bytes, int *info_dev, void *stream);
+
+/* Explicit plan handle: what an ADMM loop keeps across iterations.  A plan owns the routing of
+ * its size list (size class per block, svec offsets, lanes), the options in force when it was created (later
+ * hpsd_set_option calls do not touch it), its own DEVICE workspace, the per-block status words and the CUDA graphs
+ * captured for the buffers it has been run with.  hpsd_plan_create allocates and may synchronise; the execute calls
+ * only enqueue on `stream` (first call with a new set of buffers: plain launches; second: capture; later: one
+ * cudaGraphLaunch), may be captured by the caller, and never run route or size computations on the host.
+ * Calls on ONE plan from different streams are ordered with an event (they share its workspace); different plans
+ * are independent and may run concurrently.  Destroying a plan synchronises the device.
+ *   hpsd_plan_project    out = Pi_C(in)                         (Eq. D33)
+ *   hpsd_plan_admm_step  u = Pi_C(u~ - v), v <- v - u~ + u     (Eqs. D33-D34)
+ *   hpsd_plan_info       DEVICE pointer to the n_blocks status words of the last execution (0, 1/4 = an iteration
+ *                        did not converge, 2 = non-finite input) and the plan's workspace size in bytes
+ * All pointers passed to the execute calls are DEVICE pointers with the layout and aliasing rules of hpsd_project. */
+typedef struct hpsd_plan hpsd_plan;
+int hpsd_plan_create(int n_blocks, const int *sizes, hpsd_plan **plan);
+int hpsd_plan_destroy(hpsd_plan *plan);
+int hpsd_plan_project(hpsd_plan *plan, const double *in_svec, double *out_svec, void *stream);
+int hpsd_plan_admm_step(hpsd_plan *plan, const double *utilde, double *v, double *u, void *stream);
+int hpsd_plan_info(hpsd_plan *plan, const int **info_dev, size_t *workspace_bytes);
+/* Copies the n_blocks status words to HOST memory on `stream` and synchronises that stream. */
+int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream);
 
 /* One ADMM cone step, Eqs. (D33)-(D34), fused into the projection:
  *     u = Pi_C(u~ - v),      v <- v - u~ + u

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     HpsdError,
     admm_step_,
     eigvalsh,
+    Plan,
     reduce_to_band,
     band_width,
     fp64_peak_probe,

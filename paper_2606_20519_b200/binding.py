@@ -18,6 +18,7 @@ EXPORTS = [
     "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
     "hpsd_reduce_to_band", "hpsd_band_width",
+    "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info",
 ]
 
 
@@ -52,6 +53,12 @@ def load_library():
         lib.hpsd_tridiagonalize.argtypes = [c_int, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_eigvalsh.argtypes = [c_int, c_vp, c_vp, c_vp]
         lib.hpsd_reduce_to_band.argtypes = [c_int, c_vp, c_vp, c_vp]
+        lib.hpsd_plan_create.argtypes = [c_int, ip, ctypes.POINTER(c_vp)]
+        lib.hpsd_plan_destroy.argtypes = [c_vp]
+        lib.hpsd_plan_project.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_plan_admm_step.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_plan_info.argtypes = [c_vp, ctypes.POINTER(c_vp), ctypes.POINTER(c_sz)]
+        lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
         lib.hpsd_set_option.argtypes = [ctypes.c_char_p, c_int]
         lib.hpsd_last_launch_count.restype = c_int
         lib.hpsd_release.restype = c_int
@@ -208,6 +215,56 @@ def tridiagonalize(svec: torch.Tensor, n: int, stream: Optional[torch.cuda.Strea
     with torch.cuda.device(svec.device):
         _check(load_library().hpsd_tridiagonalize(n, svec.data_ptr(), d.data_ptr(), e.data_ptr(), _stream(stream)), "hpsd_tridiagonalize")
     return d, e
+
+
+class Plan:
+    """hpsd_plan_*: explicit plan handle (routing, options, workspace, status words and captured graphs of one size
+    list).  Argument marshalling only; every step runs in the library's kernels."""
+
+    def __init__(self, sizes: Sequence[int], device: Optional[torch.device] = None):
+        self.sizes = [int(n) for n in sizes]
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self._h = ctypes.c_void_p()
+        arr, nb = _sizes(self.sizes)
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_plan_create(nb, arr, ctypes.byref(self._h)), "hpsd_plan_create")
+
+    def project_(self, in_svec: torch.Tensor, out_svec: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        _need_cuda_f64(in_svec, "in_svec"); _need_cuda_f64(out_svec, "out_svec")
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_plan_project(self._h, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)), "hpsd_plan_project")
+        return out_svec
+
+    def admm_step_(self, utilde: torch.Tensor, v: torch.Tensor, u: torch.Tensor, stream: Optional[torch.cuda.Stream] = None):
+        for t, nm in ((utilde, "utilde"), (v, "v"), (u, "u")):
+            _need_cuda_f64(t, nm)
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_plan_admm_step(self._h, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)), "hpsd_plan_admm_step")
+        return u, v
+
+    def info(self, stream: Optional[torch.cuda.Stream] = None):
+        """hpsd_plan_read_info: status words of the last execution on `stream` as a list (synchronises the stream)."""
+        nb = len(self.sizes)
+        host = (ctypes.c_int * max(nb, 1))()
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_plan_read_info(self._h, host, _stream(stream)), "hpsd_plan_read_info")
+        return [int(host[i]) for i in range(nb)]
+
+    def workspace_bytes(self) -> int:
+        ptr, nbytes = ctypes.c_void_p(), ctypes.c_size_t()
+        _check(load_library().hpsd_plan_info(self._h, ctypes.byref(ptr), ctypes.byref(nbytes)), "hpsd_plan_info")
+        return int(nbytes.value)
+
+    def destroy(self):
+        if self._h:
+            load_library().hpsd_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 def band_width() -> int:

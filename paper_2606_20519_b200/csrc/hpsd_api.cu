@@ -5,8 +5,10 @@
 #include <algorithm>
 #include <map>
 #include <memory>
+#include <new>
 #include <mutex>
 #include <vector>
+#include <functional>
 
 #include "../../include/hpsd.h"
 #include "kernels.h"
@@ -56,7 +58,28 @@ struct Options {
     int graph_replay = 1;             // replay repeated calls (same buffers) as a CUDA graph
     int medium_reroute = 1;           // few medium blocks of one size go through the cluster-resident large path
     int large_lanes = 1;              // several cluster-sized blocks of one call run on parallel lane streams
+    int cluster_tridiag = 1;          // 116 < n <= ~631: S1+S2+S3 in one 16-CTA cluster
+    int overlap_factors = 1;          // compact-WY factors of S5 on a side stream next to S4
+    int two_stage = 0;                // 0 one-stage reduction, 1 two-stage for every large block, 2 two-stage from two_stage_min_n on
+    int two_stage_min_n = 1024;
+    bool same_routing(const Options &o) const {
+        return jacobi_max_n == o.jacobi_max_n && medium_max_n == o.medium_max_n && medium_dc == o.medium_dc && medium_reroute == o.medium_reroute &&
+               large_lanes == o.large_lanes && cluster_tridiag == o.cluster_tridiag && overlap_factors == o.overlap_factors &&
+               two_stage == o.two_stage && two_stage_min_n == o.two_stage_min_n;
+    }
 } g_opt;
+
+// the large path reads its switches from globals (largepath.h); they are set from the plan's options under g_mu
+void apply_runtime_options(const Options &o) {
+    g_cluster_tridiag = o.cluster_tridiag;
+    g_overlap_factors = o.overlap_factors;
+    g_two_stage = o.two_stage;
+    g_two_stage_min_n = o.two_stage_min_n;
+}
+bool takes_two_stage(const Options &o, int n) {
+    if (n < kTwoStageMinN || n > kTwoStageMaxN) return false;
+    return o.two_stage == 1 || (o.two_stage == 2 && n >= o.two_stage_min_n);
+}
 
 inline bool use_meddc(const Options &o, int n) { return o.medium_dc && n > o.jacobi_max_n && n <= o.medium_max_n && n <= kMedDcMaxN; }
 
@@ -84,7 +107,8 @@ struct GraphEntry {
 struct Plan {
     std::vector<GraphEntry> graphs;
     std::vector<int> sizes;
-    int jacobi_max_n, medium_max_n, medium_dc, medium_reroute, large_lanes;
+    Options opt;                       // the options this plan was routed with (frozen: a plan never changes its routing)
+    size_t ws_need = 0;                // hpsd_workspace_size of this size list (device-independent bound)
     std::vector<JacobiGroup> groups;
     std::vector<LargeBlock> large;
     int n_scalar = 0;
@@ -116,11 +140,12 @@ struct DeviceState {
     unsigned long long stamp = 0;
     std::vector<std::unique_ptr<Plan>> plans;
     void *ws = nullptr; size_t ws_bytes = 0;
+    cudaEvent_t ws_event = nullptr; cudaStream_t ws_stream = nullptr; bool ws_busy = false;   // last user of the library workspace
     double *stage_in = nullptr, *stage_out = nullptr; size_t stage_elems = 0;
     bool inited = false;
 };
 
-std::mutex g_mu;
+std::recursive_mutex g_mu;      // every entry point holds it from plan lookup through the last enqueue
 std::map<int, DeviceState> g_dev;
 
 int init_device(DeviceState &ds) {
@@ -142,13 +167,13 @@ int init_device(DeviceState &ds) {
 // device-independent size test and with "never" and takes the larger result, so its answer bounds every device's plan.
 int cluster_never(int) { return 0; }
 
-void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*fits)(int), std::vector<long long> &ll, std::vector<int> &ints) {
+void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*cluster_fits)(int), std::vector<long long> &ll, std::vector<int> &ints) {
     pl.sizes.assign(sizes, sizes + n_blocks);
-    pl.jacobi_max_n = g_opt.jacobi_max_n;
-    pl.medium_max_n = g_opt.medium_max_n;
-    pl.medium_dc = g_opt.medium_dc;
-    pl.medium_reroute = g_opt.medium_reroute;
-    pl.large_lanes = g_opt.large_lanes;
+    pl.opt = g_opt;
+    // the cluster-resident reduction serves size n (and occupies only 16 SMs, so such blocks run on lanes): not when the
+    // option is off, not when the block takes the two-stage reduction
+    const Options opt = g_opt;
+    std::function<bool(int)> fits = [cluster_fits, opt](int n) { return opt.cluster_tridiag && !takes_two_stage(opt, n) && cluster_fits(n) != 0; };
     const int lim = small_limit(g_opt);
     std::map<int, std::vector<std::pair<long long, int>>> by_n;
     std::vector<long long> scalars;
@@ -177,7 +202,7 @@ void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*fits)(int), std:
         }
         JacobiGroup g;
         g.n = kv.first; g.count = (int)kv.second.size();
-        g.medium = g.n > pl.jacobi_max_n;
+        g.medium = g.n > pl.opt.jacobi_max_n;
         g.dc = use_meddc(g_opt, g.n);
         g.off_index = ll.size(); g.idx_index = ints.size();
         for (auto &pr : kv.second) { ll.push_back(pr.first); ints.push_back(pr.second); }
@@ -205,9 +230,22 @@ void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*fits)(int), std:
     pl.ws_bytes = pl.base_ws + pl.n_lanes * pl.lane_ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
 }
 
+size_t workspace_bound(int n_blocks, const int *sizes) {
+    size_t ws = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        Plan tmp;
+        std::vector<long long> ll;
+        std::vector<int> ints;
+        route_plan(n_blocks, sizes, tmp, pass == 0 ? tridiag_cluster_size_ok : cluster_never, ll, ints);
+        ws = std::max(ws, tmp.ws_bytes);
+    }
+    return ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int) + 4, 256) + 256;
+}
+
 int build_plan(int n_blocks, const int *sizes, Plan &pl) {
     std::vector<long long> ll;
     std::vector<int> ints;
+    pl.ws_need = workspace_bound(n_blocks, sizes);
     route_plan(n_blocks, sizes, pl, tridiag_cluster_fits, ll, ints);
     pl.n_ll = ll.size(); pl.n_int = ints.size();
     const size_t bytes = ll.size() * sizeof(long long) + ints.size() * sizeof(int);
@@ -236,7 +274,7 @@ int build_plan(int n_blocks, const int *sizes, Plan &pl) {
 // synchronises (cudaMalloc/cudaMemcpy); later calls with the same list are launch-only.
 int get_plan(DeviceState &ds, int n_blocks, const int *sizes, Plan **out) {
     for (auto &p : ds.plans) {
-        if ((int)p->sizes.size() == n_blocks && p->jacobi_max_n == g_opt.jacobi_max_n && p->medium_max_n == g_opt.medium_max_n && p->medium_dc == g_opt.medium_dc && p->medium_reroute == g_opt.medium_reroute && p->large_lanes == g_opt.large_lanes &&
+        if ((int)p->sizes.size() == n_blocks && p->opt.same_routing(g_opt) &&
             (n_blocks == 0 || std::memcmp(p->sizes.data(), sizes, sizeof(int) * n_blocks) == 0)) {
             *out = p.get();
             return 0;
@@ -275,6 +313,7 @@ bool lanes_ready(DeviceState &ds, int n) {
 
 int run_plan(DeviceState &ds, const Plan &pl, const SvecIo &io, void *ws, int *info_dev, cudaStream_t st) {
     // info lives at the start of the workspace when the caller gave none
+    apply_runtime_options(pl.opt);
     int *info = info_dev ? info_dev : reinterpret_cast<int *>(ws);
     unsigned char *scratch = reinterpret_cast<unsigned char *>(ws) + align_up(pl.sizes.size() * sizeof(int) + 4, 256);
     if (!pl.sizes.empty()) {
@@ -344,9 +383,8 @@ const char *hpsd_strerror(int code) {
 
 int hpsd_set_option(const char *name, int value) {
     if (!name) return HPSD_EINVAL;
-    std::lock_guard<std::mutex> lk(g_mu);
-    for (auto &kv : g_dev)                      // a captured call froze the options it ran with
-        for (auto &pl : kv.second.plans) pl->drop_graphs();
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    // routing options are frozen into each plan (and its captured graphs): a change only selects a different plan
     if (std::strcmp(name, "large_lanes") == 0) {
         g_opt.large_lanes = (value != 0);
         return HPSD_OK;
@@ -373,21 +411,21 @@ int hpsd_set_option(const char *name, int value) {
         return HPSD_OK;
     }
     if (std::strcmp(name, "overlap_factors") == 0) {
-        g_overlap_factors = (value != 0);
+        g_opt.overlap_factors = (value != 0);
         return HPSD_OK;
     }
     if (std::strcmp(name, "cluster_tridiag") == 0) {
-        g_cluster_tridiag = (value != 0);
+        g_opt.cluster_tridiag = (value != 0);
         return HPSD_OK;
     }
     if (std::strcmp(name, "two_stage") == 0) {
         if (value < 0 || value > 2) return HPSD_EINVAL;
-        g_two_stage = value;
+        g_opt.two_stage = value;
         return HPSD_OK;
     }
     if (std::strcmp(name, "two_stage_min_n") == 0) {
         if (value < 2) return HPSD_EINVAL;
-        g_two_stage_min_n = value;
+        g_opt.two_stage_min_n = value;
         return HPSD_OK;
     }
     if (std::strcmp(name, "medium_max_n") == 0) {
@@ -411,7 +449,7 @@ const char *hpsd_profile_stage_name(int stage) {
 
 int hpsd_profile_read(double *ms, int *spans, int n) {
     if (n < ST_COUNT || !ms) return HPSD_EINVAL;
-    std::lock_guard<std::mutex> lk(g_mu);
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
     for (int i = 0; i < ST_COUNT; ++i) { ms[i] = 0.0; if (spans) spans[i] = 0; }
     for (const ProfSpan &sp : g_spans) {
         if (cudaEventSynchronize(sp.b) != cudaSuccess) return HPSD_ECUDA;
@@ -428,38 +466,33 @@ int hpsd_workspace_size(int n_blocks, const int *sizes, size_t *bytes) {
     size_t total;
     int rc = check_args(n_blocks, sizes, (void *)1, (void *)1, &total);
     if (rc) return rc;
-    size_t ws = 0;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);       // the options are read under the lock
-        for (int pass = 0; pass < 2; ++pass) {
-            Plan tmp;
-            std::vector<long long> ll;
-            std::vector<int> ints;
-            route_plan(n_blocks, sizes, tmp, pass == 0 ? tridiag_cluster_size_ok : cluster_never, ll, ints);
-            ws = std::max(ws, tmp.ws_bytes);
-        }
-    }
-    *bytes = ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int) + 4, 256) + 256;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);       // the options are read under the lock
+    *bytes = workspace_bound(n_blocks, sizes);
     return HPSD_OK;
 }
+
+static int execute_plan(DeviceState &ds, Plan &plan, const SvecIo &io, void *ws, size_t ws_bytes, int *info_dev, cudaStream_t st);
 
 static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void *ws, size_t ws_bytes, int *info_dev, void *stream) {
     g_launches = 0;
     if (n_blocks == 0) return HPSD_OK;
-    size_t need;
-    int rc = hpsd_workspace_size(n_blocks, sizes, &need);
-    if (rc) return rc;
-    if (ws == nullptr || ws_bytes < need || (reinterpret_cast<uintptr_t>(ws) & 255u)) return HPSD_EWORKSPACE;
     int dev;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
-    std::lock_guard<std::mutex> lk(g_mu);
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
     DeviceState &ds = g_dev[dev];
-    rc = init_device(ds);
+    int rc = init_device(ds);
     if (rc) return rc;
     Plan *pl;
-    rc = get_plan(ds, n_blocks, sizes, &pl);
+    rc = get_plan(ds, n_blocks, sizes, &pl);           // the plan carries the workspace bound: no routing dry-runs per call
     if (rc) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
+    return execute_plan(ds, *pl, io, ws, ws_bytes, info_dev, (cudaStream_t)stream);
+}
+
+// Run a plan on `st`: plain launches the first time a set of buffers is seen, a captured CUDA graph afterwards.
+static int execute_plan(DeviceState &ds, Plan &plan, const SvecIo &io, void *ws, size_t ws_bytes, int *info_dev, cudaStream_t st) {
+    Plan *pl = &plan;
+    int rc = 0;
+    if (ws == nullptr || ws_bytes < pl->ws_need || (reinterpret_cast<uintptr_t>(ws) & 255u)) return HPSD_EWORKSPACE;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (!g_opt.graph_replay || g_profile || cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
         cudaGetLastError();
@@ -510,23 +543,59 @@ static int project_io_ws(int n_blocks, const int *sizes, const SvecIo &io, void 
     return cudaGraphLaunch(ge->exec, st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
 }
 
-// library-owned workspace of the current device, grown on demand
-static int library_workspace(int n_blocks, const int *sizes, void **ws, size_t *bytes) {
-    size_t need;
-    int rc = hpsd_workspace_size(n_blocks, sizes, &need);
-    if (rc) return rc;
-    int dev;
-    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
-    std::lock_guard<std::mutex> lk(g_mu);
-    DeviceState &ds = g_dev[dev];
+// Library-owned workspace of the current device, grown on demand (g_mu held by the caller, through the last enqueue).
+// Calls on different streams share it: each call is ordered after the previous user with an event, so two in-flight
+// calls never overwrite each other's scratch (they serialise; callers that want concurrency use hpsd_plan_create or
+// hpsd_project_ws with a workspace per stream).  A capturing stream cannot wait on or record a plain event: captured
+// calls are the caller's to order.
+static bool stream_capturing(cudaStream_t st) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
+    return cs != cudaStreamCaptureStatusNone;
+}
+static int order_after(cudaEvent_t &ev, cudaStream_t &last, bool &busy, cudaStream_t st) {
+    if (busy && last != st && !stream_capturing(st))
+        if (cudaStreamWaitEvent(st, ev, 0) != cudaSuccess) return HPSD_ECUDA;
+    return HPSD_OK;
+}
+static int mark_user(cudaEvent_t &ev, cudaStream_t &last, bool &busy, cudaStream_t st) {
+    if (stream_capturing(st)) return HPSD_OK;
+    if (!ev && cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { ev = nullptr; return HPSD_ECUDA; }
+    if (cudaEventRecord(ev, st) != cudaSuccess) return HPSD_ECUDA;
+    last = st; busy = true;
+    return HPSD_OK;
+}
+static int library_workspace(DeviceState &ds, size_t need, cudaStream_t st, void **ws, size_t *bytes) {
     if (ds.ws_bytes < need) {
-        if (ds.ws) cudaFree(ds.ws);   // synchronises; only when the workspace grows
-        ds.ws = nullptr; ds.ws_bytes = 0;
+        if (ds.ws) cudaFree(ds.ws);   // synchronises the device; only when the workspace grows
+        ds.ws = nullptr; ds.ws_bytes = 0; ds.ws_busy = false;
         if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
         ds.ws_bytes = need;
     }
     *ws = ds.ws; *bytes = ds.ws_bytes;
-    return 0;
+    return order_after(ds.ws_event, ds.ws_stream, ds.ws_busy, st);
+}
+
+// hpsd_project / hpsd_admm_step: library workspace, cached plan
+static int project_io_lib(int n_blocks, const int *sizes, const SvecIo &io, void *stream) {
+    g_launches = 0;
+    if (n_blocks == 0) return HPSD_OK;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    int rc = init_device(ds);
+    if (rc) return rc;
+    Plan *pl;
+    rc = get_plan(ds, n_blocks, sizes, &pl);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    void *ws; size_t bytes;
+    rc = library_workspace(ds, pl->ws_need, st, &ws, &bytes);
+    if (rc) return rc;
+    rc = execute_plan(ds, *pl, io, ws, bytes, nullptr, st);
+    const int rc2 = mark_user(ds.ws_event, ds.ws_stream, ds.ws_busy, st);
+    return rc ? rc : rc2;
 }
 
 int hpsd_project_ws(int n_blocks, const int *sizes, const double *in_svec, double *out_svec,
@@ -543,23 +612,16 @@ int hpsd_admm_step(int n_blocks, const int *sizes, const double *utilde, double 
     int rc = check_args(n_blocks, sizes, utilde, u, &total);
     if (rc) return rc;
     if (total > 0 && v == nullptr) return HPSD_EINVAL;
-    if (n_blocks == 0) { g_launches = 0; return HPSD_OK; }
-    void *ws; size_t bytes;
-    rc = library_workspace(n_blocks, sizes, &ws, &bytes);
-    if (rc) return rc;
     const SvecIo io{utilde, v, u, v};
-    return project_io_ws(n_blocks, sizes, io, ws, bytes, nullptr, stream);
+    return project_io_lib(n_blocks, sizes, io, stream);
 }
 
 int hpsd_project(int n_blocks, const int *sizes, const double *in_svec, double *out_svec, void *stream) {
     size_t total;
     int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
     if (rc) return rc;
-    if (n_blocks == 0) { g_launches = 0; return HPSD_OK; }
-    void *ws; size_t bytes;
-    rc = library_workspace(n_blocks, sizes, &ws, &bytes);
-    if (rc) return rc;
-    return hpsd_project_ws(n_blocks, sizes, in_svec, out_svec, ws, bytes, nullptr, stream);
+    const SvecIo io{in_svec, nullptr, out_svec, nullptr};
+    return project_io_lib(n_blocks, sizes, io, stream);
 }
 
 int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, double *out_host, void *stream) {
@@ -570,8 +632,10 @@ int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, dou
     int dev;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
     double *din, *dout;
+    static std::mutex host_mu;                       // the staging buffers serve one host call at a time (the call is synchronous)
+    std::lock_guard<std::mutex> host_lk(host_mu);
     {
-        std::lock_guard<std::mutex> lk(g_mu);
+        std::lock_guard<std::recursive_mutex> lk(g_mu);
         DeviceState &ds = g_dev[dev];
         if (ds.stage_elems < total) {
             if (ds.stage_in) cudaFree(ds.stage_in);
@@ -607,54 +671,145 @@ int hpsd_unpack(int n, const double *svec, void *A, int lda, void *stream) {
 // S2+S3 alone: real symmetric tridiagonal (d[n], e[n-1]) unitarily similar to the block.
 int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream);
 
-// shared by hpsd_tridiagonalize / hpsd_eigvalsh: plan + workspace for a single block forced onto the large path
-static int single_large_setup(int n, void **ws_out, Plan **pl_out) {
+// shared by hpsd_tridiagonalize / hpsd_eigvalsh / hpsd_reduce_to_band: one block forced onto the large path, on the
+// library workspace (ordered against every other user of it); g_mu is held through the enqueue
+static int single_large(int n, cudaStream_t st, const std::function<int(unsigned char *, const int2 *)> &run) {
     int dev;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
     const int sizes[1] = {n};
-    std::lock_guard<std::mutex> lk(g_mu);
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
     DeviceState &ds = g_dev[dev];
     int rc = init_device(ds);
     if (rc) return rc;
     const Options saved = g_opt;
     g_opt.jacobi_max_n = 1;                 // force the large-path plan for any n >= 2
     g_opt.medium_max_n = 0;
-    rc = get_plan(ds, 1, sizes, pl_out);
+    Plan *pl = nullptr;
+    rc = get_plan(ds, 1, sizes, &pl);
     g_opt = saved;
     if (rc) return rc;
-    const size_t need = largepath_ws_bytes(n) + 1024;
-    if (ds.ws_bytes < need) {
-        if (ds.ws) cudaFree(ds.ws);
-        ds.ws = nullptr; ds.ws_bytes = 0;
-        if (cudaMalloc(&ds.ws, need) != cudaSuccess) return HPSD_EALLOC;
-        ds.ws_bytes = need;
-    }
-    *ws_out = ds.ws;
-    return 0;
+    void *ws; size_t bytes;
+    rc = library_workspace(ds, largepath_ws_bytes(n) + 1024, st, &ws, &bytes);
+    if (rc) return rc;
+    apply_runtime_options(pl->opt);
+    rc = run(reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n));
+    const int rc2 = mark_user(ds.ws_event, ds.ws_stream, ds.ws_busy, st);
+    return rc ? rc : rc2;
 }
 
 int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream) {
     if (n < 0 || n > kMaxLargeN || (n > 0 && (!in_svec || !lambda))) return HPSD_EINVAL;
     if (n == 0) return HPSD_OK;
     g_launches = 0;
-    if (n == 1)
-        return cudaMemcpyAsync(lambda, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
-    void *ws; Plan *pl;
-    int rc = single_large_setup(n, &ws, &pl);
-    if (rc) return rc;
-    return largepath_eigvals(n, in_svec, lambda, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n == 1) return cudaMemcpyAsync(lambda, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    return single_large(n, st, [&](unsigned char *scratch, const int2 *tiles) { return largepath_eigvals(n, in_svec, lambda, scratch, tiles, st); });
 }
 
 int hpsd_tridiagonalize(int n, const double *in_svec, double *d, double *e, void *stream) {
     if (n < 0 || n > kMaxLargeN || (n > 0 && (!in_svec || !d)) || (n > 1 && !e)) return HPSD_EINVAL;
     if (n == 0) return HPSD_OK;
     g_launches = 0;
-    if (n == 1)
-        return cudaMemcpyAsync(d, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
-    void *ws; Plan *pl;
-    int rc = single_large_setup(n, &ws, &pl);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n == 1) return cudaMemcpyAsync(d, in_svec, sizeof(double), cudaMemcpyDeviceToDevice, st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+    return single_large(n, st, [&](unsigned char *scratch, const int2 *tiles) { return largepath_tridiag_only(n, in_svec, d, e, scratch, tiles, st); });
+}
+
+// ---- explicit plan handle: routing, options, workspace and captured graphs live in the plan ----
+struct hpsd_plan {
+    int dev = -1;
+    std::unique_ptr<Plan> pl;
+    void *ws = nullptr; size_t ws_bytes = 0;
+    cudaEvent_t done = nullptr; cudaStream_t last = nullptr; bool busy = false;
+};
+
+int hpsd_plan_create(int n_blocks, const int *sizes, hpsd_plan **plan) {
+    if (!plan) return HPSD_EINVAL;
+    *plan = nullptr;
+    size_t total;
+    int rc = check_args(n_blocks, sizes, (void *)1, (void *)1, &total);
     if (rc) return rc;
-    return largepath_tridiag_only(n, in_svec, d, e, reinterpret_cast<unsigned char *>(ws) + 256, pl->tiles_dev.at(n), (cudaStream_t)stream);
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    rc = init_device(ds);
+    if (rc) return rc;
+    std::unique_ptr<hpsd_plan> hp(new (std::nothrow) hpsd_plan());
+    if (!hp) return HPSD_EALLOC;
+    hp->dev = dev;
+    hp->pl.reset(new (std::nothrow) Plan());
+    if (!hp->pl) return HPSD_EALLOC;
+    rc = build_plan(n_blocks, sizes, *hp->pl);
+    if (rc) return rc;
+    hp->ws_bytes = hp->pl->ws_need;
+    if (cudaMalloc(&hp->ws, hp->ws_bytes) != cudaSuccess) return HPSD_EALLOC;
+    *plan = hp.release();
+    return HPSD_OK;
+}
+
+int hpsd_plan_destroy(hpsd_plan *plan) {
+    if (!plan) return HPSD_OK;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != plan->dev) cudaSetDevice(plan->dev);
+    if (plan->ws) cudaFree(plan->ws);              // synchronises: nothing of this plan is in flight afterwards
+    if (plan->done) cudaEventDestroy(plan->done);
+    plan->pl.reset();
+    if (cur >= 0 && cur != plan->dev) cudaSetDevice(cur);
+    delete plan;
+    return HPSD_OK;
+}
+
+static int plan_execute(hpsd_plan *plan, const SvecIo &io, void *stream) {
+    g_launches = 0;
+    if (plan->pl->sizes.empty()) return HPSD_OK;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    if (dev != plan->dev) return HPSD_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    int rc = order_after(plan->done, plan->last, plan->busy, st);
+    if (rc) return rc;
+    rc = execute_plan(ds, *plan->pl, io, plan->ws, plan->ws_bytes, nullptr, st);
+    const int rc2 = mark_user(plan->done, plan->last, plan->busy, st);
+    return rc ? rc : rc2;
+}
+
+int hpsd_plan_project(hpsd_plan *plan, const double *in_svec, double *out_svec, void *stream) {
+    if (!plan || !plan->pl) return HPSD_EINVAL;
+    size_t total = 0;
+    for (int n : plan->pl->sizes) total += (size_t)n * n;
+    if (total > 0 && (!in_svec || !out_svec)) return HPSD_EINVAL;
+    const SvecIo io{in_svec, nullptr, out_svec, nullptr};
+    return plan_execute(plan, io, stream);
+}
+
+int hpsd_plan_admm_step(hpsd_plan *plan, const double *utilde, double *v, double *u, void *stream) {
+    if (!plan || !plan->pl) return HPSD_EINVAL;
+    size_t total = 0;
+    for (int n : plan->pl->sizes) total += (size_t)n * n;
+    if (total > 0 && (!utilde || !v || !u)) return HPSD_EINVAL;
+    const SvecIo io{utilde, v, u, v};
+    return plan_execute(plan, io, stream);
+}
+
+int hpsd_plan_info(hpsd_plan *plan, const int **info_dev, size_t *workspace_bytes) {
+    if (!plan || !plan->pl) return HPSD_EINVAL;
+    if (info_dev) *info_dev = reinterpret_cast<const int *>(plan->ws);      // run_plan keeps the status words at the head of the workspace
+    if (workspace_bytes) *workspace_bytes = plan->ws_bytes;
+    return HPSD_OK;
+}
+
+int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream) {
+    if (!plan || !plan->pl || (!info_host && !plan->pl->sizes.empty())) return HPSD_EINVAL;
+    const size_t nb = plan->pl->sizes.size();
+    if (nb == 0) return HPSD_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(info_host, plan->ws, nb * sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return HPSD_ECUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
 }
 
 int hpsd_band_width(void) { return kBW; }
@@ -662,16 +817,14 @@ int hpsd_band_width(void) { return kBW; }
 int hpsd_reduce_to_band(int n, const double *in_svec, double *band, void *stream) {
     if (n < 2 || n > kMaxLargeN || !in_svec || !band) return HPSD_EINVAL;
     g_launches = 0;
-    void *ws; Plan *pl;
-    int rc = single_large_setup(n, &ws, &pl);
-    if (rc) return rc;
-    return largepath_band_only(n, in_svec, reinterpret_cast<cplx *>(band), reinterpret_cast<unsigned char *>(ws) + 256, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    return single_large(n, st, [&](unsigned char *scratch, const int2 *) { return largepath_band_only(n, in_svec, reinterpret_cast<cplx *>(band), scratch, st); });
 }
 
 int hpsd_release(void) {
     int dev;
     if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
-    std::lock_guard<std::mutex> lk(g_mu);
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
     auto it = g_dev.find(dev);
     if (it != g_dev.end()) {
         cudaDeviceSynchronize();

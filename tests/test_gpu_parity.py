@@ -832,3 +832,105 @@ def test_random_cone_lists(orc, hp):
                 sl = slice(off, off + n * n)
                 assert parity_err(got[sl], want[sl], sv[sl], n) <= TOL * max(n, 1), (sizes, n, rep)
                 off += n * n
+
+
+# ------------------------------------------------------------------ explicit plan handle, streams
+
+def test_plan_api_admm_loop_under_capture(orc, hp):
+    """hpsd_plan_create / execute / destroy.  One plan serves a 100-iteration ADMM cone-step loop
+    (Eqs. D33-D34) captured by the CALLER into a CUDA graph; the iterates match the oracle's loop step by step for the
+    first steps and the fixed point at the end (v_k converges: u = P(u~ - v), v <- v - u~ + u with constant u~
+    gives v -> P(-(u~))-like limits; we simply compare against the oracle's own 100 steps)."""
+    import torch
+    rng = np.random.default_rng(31)
+    sizes = [16, 36, 1, 150, 16]
+    ut = pack_all(orc, [herm(rng, n) for n in sizes])
+    v0 = pack_all(orc, [herm(rng, n) * 0.1 for n in sizes])
+    plan = hp.Plan(sizes)
+    try:
+        assert plan.workspace_bytes() >= hp.workspace_size(sizes) - 4096
+        t_ut, t_v, t_u = torch.from_numpy(ut).cuda(), torch.from_numpy(v0.copy()).cuda(), torch.empty(len(ut), dtype=torch.float64, device="cuda")
+        # eager steps first (plain launches, then the library's own graph), checked against the oracle
+        v = v0.copy()
+        for _ in range(3):
+            plan.admm_step_(t_ut, t_v, t_u)
+            u, v = orc.admm_step(sizes, ut, v, nthreads=orc.max_threads())
+        torch.cuda.synchronize()
+        assert rel_err(t_u.cpu().numpy(), u) <= TOL * max(sizes)
+        assert rel_err(t_v.cpu().numpy(), v) <= TOL * max(sizes)
+        assert plan.info() == [0] * len(sizes)
+        # caller-side capture of one step, replayed 97 times
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                plan.admm_step_(t_ut, t_v, t_u, stream=side)
+        for _ in range(97):
+            g.replay()
+            u, v = orc.admm_step(sizes, ut, v, nthreads=orc.max_threads())
+        torch.cuda.synchronize()
+        assert rel_err(t_u.cpu().numpy(), u) <= 100 * TOL * max(sizes)      # 100 steps of rounding in the v recursion
+        assert rel_err(t_v.cpu().numpy(), v) <= 100 * TOL * max(sizes)
+        # plain projection through the same plan
+        out = torch.empty_like(t_ut)
+        plan.project_(t_ut, out)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), gpu_project(hp, sizes, ut))
+    finally:
+        plan.destroy()
+
+
+def test_plan_options_are_frozen_at_creation(orc, hp):
+    """A plan keeps the options it was created with: changing a routing option afterwards does not alter its result
+    bits, and a plan created under the new option takes the new route."""
+    import torch
+    rng = np.random.default_rng(32)
+    n = 200
+    sv = orc.pack(herm(rng, n))
+    t = torch.from_numpy(sv).cuda()
+    a = hp.Plan([n])
+    out_a = a.project_(t, torch.empty_like(t)).cpu().numpy()
+    hp.set_option("cluster_tridiag", 0)
+    try:
+        b = hp.Plan([n])
+        out_a2 = a.project_(t, torch.empty_like(t)).cpu().numpy()
+        out_b = b.project_(t, torch.empty_like(t)).cpu().numpy()
+    finally:
+        hp.set_option("cluster_tridiag", 1)
+    assert np.array_equal(out_a, out_a2)
+    assert not np.array_equal(out_a, out_b)                      # other kernels, other rounding
+    want = orc.project([n], sv, nthreads=orc.max_threads())
+    assert rel_err(out_a, want) <= TOL * n and rel_err(out_b, want) <= TOL * n
+    a.destroy(); b.destroy()
+
+
+def test_two_streams_share_the_library_workspace(orc, hp):
+    """hpsd_project from two streams without host synchronisation in between: the calls share the library
+    workspace and are ordered on it with an event, so both results are right; two explicit plans on two
+    streams run independently."""
+    import torch
+    rng = np.random.default_rng(33)
+    na, nb = 300, 310
+    sva, svb = orc.pack(herm(rng, na)), orc.pack(herm(rng, nb))
+    ta, tb = torch.from_numpy(sva).cuda(), torch.from_numpy(svb).cuda()
+    oa, ob = torch.empty_like(ta), torch.empty_like(tb)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(5):
+        hp.project_([na], ta, oa, stream=s1)
+        hp.project_([nb], tb, ob, stream=s2)
+    torch.cuda.synchronize()
+    wa = orc.project([na], sva, nthreads=orc.max_threads())
+    wb = orc.project([nb], svb, nthreads=orc.max_threads())
+    assert rel_err(oa.cpu().numpy(), wa) <= TOL * na
+    assert rel_err(ob.cpu().numpy(), wb) <= TOL * nb
+    pa, pb = hp.Plan([na]), hp.Plan([nb])
+    oa2, ob2 = torch.empty_like(ta), torch.empty_like(tb)
+    for _ in range(5):
+        pa.project_(ta, oa2, stream=s1)
+        pb.project_(tb, ob2, stream=s2)
+    torch.cuda.synchronize()
+    assert np.array_equal(oa2.cpu().numpy(), oa.cpu().numpy())
+    assert np.array_equal(ob2.cpu().numpy(), ob.cpu().numpy())
+    pa.destroy(); pb.destroy()
