@@ -31,6 +31,7 @@ struct Q2Args {
     cplx *T2;
     cplx *Zc;
     const int *cnt;
+    int *flags;          // per (slab, group): blocks finished (release/acquire)
 };
 
 __device__ __forceinline__ bool q2_exists(int n, int s, int k) { return s < n - 1 && s + 1 + k * kBW < n; }
@@ -88,41 +89,73 @@ struct Q2Smem {
     cplx T[kQ2G * kQ2TP];
 };
 
+__device__ __forceinline__ int q2_ld_acquire(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void q2_st_release(int *p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+constexpr int kQ2Done = 1 << 30;
+
+// Each slab of 32 columns of Z is served by P = gridDim.x / (active slabs) CTAs: CTA (slab, p) takes the sweep groups
+// ng-1-p, ng-1-p-P, ...  Group gi follows group gi+1 (it must see gi+1's result wherever their rows overlap): block
+// (gi, k) overlaps (gi+1, k-2 .. k), so it waits until group gi+1 has published k+1 finished blocks; the P CTAs of a
+// slab therefore run as a pipeline one block apart.  Cooperative launch (all CTAs resident: a CTA spins on another's flag).
 __global__ void __launch_bounds__(kQ2Threads, 2) q2_apply_kernel(Q2Args a) {
     extern __shared__ __align__(16) unsigned char q2_smem[];
     Q2Smem &S = *reinterpret_cast<Q2Smem *>(q2_smem);
     const int kpos = a.cnt[1];
-    const int c0 = blockIdx.x * kQ2NC;
-    if (c0 >= kpos) return;
+    const int nact = (kpos + kQ2NC - 1) / kQ2NC;           // active slabs
+    if (nact == 0) return;
+    int P = (int)gridDim.x / nact; if (P < 1) P = 1;
+    if (P > a.ng) P = a.ng;
+    const int slab = blockIdx.x % nact, p = blockIdx.x / nact;
+    if (p >= P) return;
+    const int c0 = slab * kQ2NC;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int fr = lane >> 2, fk = lane & 3;
     const int n = a.n;
     cplx *Zg = a.Zc + (size_t)c0 * a.ldz;
     const int ncol = (kpos - c0 < kQ2NC) ? kpos - c0 : kQ2NC;
+    int *flags = a.flags + (size_t)slab * a.ng;
 
-    for (int gi = a.ng - 1; gi >= 0; --gi) {
+    for (int gi = a.ng - 1 - p; gi >= 0; gi -= P) {
         const int s0 = gi * kQ2G;
         for (int k = 0; k < a.nk; ++k) {
             if (!q2_exists(n, s0, k)) break;
             const int R0 = s0 + 1 + k * kBW;
             const int wlen = (n - R0 < kBW + kQ2G - 1) ? n - R0 : kBW + kQ2G - 1;
-            // ---- stage the block: window of Z (row-major), compact reflectors, T
+            // ---- reflectors and T of this block: read-only data, no dependency
+            for (int e = tid; e < kQ2G * kBW; e += kQ2Threads) {
+                const int i = e / kBW, t = e % kBW;
+                const bool ok = q2_exists(n, s0 + i, k);
+                cp_async_16(&S.Vs[i * kQ2VP + t], ok ? a.V2 + ((size_t)k * n + s0 + i) * kBW + t : a.V2, ok);
+            }
+            {
+                const cplx *Tg = a.T2 + ((size_t)gi * a.nk + k) * kQ2G * kQ2G;
+                for (int e = tid; e < kQ2G * kQ2G; e += kQ2Threads) cp_async_16(&S.T[(e / kQ2G) * kQ2TP + (e % kQ2G)], Tg + e, true);
+            }
+            // ---- the window of Z: after the previous group has finished its blocks up to k
+            if (gi + 1 < a.ng) {
+                if (tid == 0) {
+                    const int *pf = flags + gi + 1;
+                    while (q2_ld_acquire(pf) < k + 1) { }
+                }
+                __syncthreads();
+            }
             {
                 const int rr = tid & 63, ch = tid >> 6;
 #pragma unroll 4
                 for (int t = 0; t < 16; ++t) {
                     const int c = ch * 16 + t;
-                    S.Zw[rr * kQ2ZP + c] = (rr < wlen && c < ncol) ? Zg[(size_t)c * a.ldz + R0 + rr] : mk(0.0, 0.0);
+                    const bool ok = rr < wlen && c < ncol;
+                    cp_async_16(&S.Zw[rr * kQ2ZP + c], ok ? Zg + (size_t)c * a.ldz + R0 + rr : Zg, ok);
                 }
             }
-            for (int e = tid; e < kQ2G * kBW; e += kQ2Threads) {
-                const int i = e / kBW, t = e % kBW;
-                S.Vs[i * kQ2VP + t] = q2_exists(n, s0 + i, k) ? a.V2[((size_t)k * n + s0 + i) * kBW + t] : mk(0.0, 0.0);
-            }
-            {
-                const cplx *Tg = a.T2 + ((size_t)gi * a.nk + k) * kQ2G * kQ2G;
-                for (int e = tid; e < kQ2G * kQ2G; e += kQ2Threads) S.T[(e / kQ2G) * kQ2TP + (e % kQ2G)] = Tg[e];
-            }
+            cp_async_commit();
+            cp_async_wait<0>();
             __syncthreads();
             // ---- X = V^H Zw: warp = 8 rows i of X, all 32 columns; K runs over window rows 8 warp .. 8 warp + 39
             {
@@ -199,28 +232,23 @@ __global__ void __launch_bounds__(kQ2Threads, 2) q2_apply_kernel(Q2Args a) {
                         dmma(im[cb][0], im[cb][1], av.y, bv.x);
                     }
                 }
+                // straight from the accumulators to global memory (C fragment: row rw, column pairs)
+                if (rw < wlen) {
 #pragma unroll
-                for (int cb = 0; cb < 4; ++cb)
+                    for (int cb = 0; cb < 4; ++cb)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        cplx z = S.Zw[rw * kQ2ZP + cb * 8 + 2 * fk + e];
-                        z.x -= re[cb][e]; z.y -= im[cb][e];
-                        S.Zw[rw * kQ2ZP + cb * 8 + 2 * fk + e] = z;
-                    }
-            }
-            __syncthreads();
-            // ---- window back to global
-            {
-                const int rr = tid & 63, ch = tid >> 6;
-                if (rr < wlen) {
-#pragma unroll 4
-                    for (int t = 0; t < 16; ++t) {
-                        const int c = ch * 16 + t;
-                        if (c < ncol) Zg[(size_t)c * a.ldz + R0 + rr] = S.Zw[rr * kQ2ZP + c];
-                    }
+                        for (int e = 0; e < 2; ++e) {
+                            const int c = cb * 8 + 2 * fk + e;
+                            if (c < ncol) {
+                                cplx z = S.Zw[rw * kQ2ZP + c];
+                                z.x -= re[cb][e]; z.y -= im[cb][e];
+                                Zg[(size_t)c * a.ldz + R0 + rw] = z;
+                            }
+                        }
                 }
             }
-            __syncthreads();
+            __syncthreads();                                     // all stores issued; the staging buffers are free
+            if (tid == 0) q2_st_release(flags + gi, q2_exists(n, s0, k + 1) && k + 1 < a.nk ? k + 1 : kQ2Done);
         }
     }
 }
@@ -241,7 +269,7 @@ size_t twostage_q2_blocks(int n) { return (size_t)q2_groups(n) * twostage_hops(n
 int launch_q2_factors(const TwoStageWs &w, cudaStream_t st) {
     const int n = w.n;
     if (n <= 1) return 0;
-    Q2Args a{n, 0, (int)twostage_hops(n), q2_groups(n), w.V2, w.tau2, w.T2, nullptr, nullptr};
+    Q2Args a{n, 0, (int)twostage_hops(n), q2_groups(n), w.V2, w.tau2, w.T2, nullptr, nullptr, nullptr};
     q2_tfactor_kernel<<<dim3(a.nk, a.ng), kQ2Threads, 0, st>>>(a);
     HPSD_LAUNCH_CHECK();
     return 0;
@@ -252,12 +280,20 @@ int launch_q2_apply(const TwoStageWs &w, cplx *Zc, int ldz, const int *cnt, cuda
     if (n <= 1) return 0;
     int rc = backq2_init();
     if (rc) return rc;
-    Q2Args a{n, ldz, (int)twostage_hops(n), q2_groups(n), w.V2, w.tau2, w.T2, Zc, cnt};
+    Q2Args a{n, ldz, (int)twostage_hops(n), q2_groups(n), w.V2, w.tau2, w.T2, Zc, cnt, w.q2flags};
+    const int nslab = (n + kQ2NC - 1) / kQ2NC;
+    HPSD_CUDA_OK(cudaMemsetAsync(w.q2flags, 0, sizeof(int) * (size_t)nslab * a.ng, st));
+    int dev = 0, sms = 148, per_sm = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, q2_apply_kernel, kQ2Threads, sizeof(Q2Smem)) != cudaSuccess || per_sm < 1) per_sm = 1;
+    if (per_sm > 2) per_sm = 2;
+    void *args[] = {&a};
     prof_begin(ST_BACKQ2, st);
-    q2_apply_kernel<<<(n + kQ2NC - 1) / kQ2NC, kQ2Threads, sizeof(Q2Smem), st>>>(a);
+    const cudaError_t e = cudaLaunchCooperativeKernel((void *)q2_apply_kernel, dim3(sms * per_sm), dim3(kQ2Threads), args, sizeof(Q2Smem), st);
     prof_end(ST_BACKQ2, st);
-    HPSD_LAUNCH_CHECK();
-    return 0;
+    g_launches++;
+    return e == cudaSuccess ? 0 : HPSD_ECUDA_;
 }
 
 }  // namespace hpsd

@@ -133,13 +133,18 @@ __device__ __forceinline__ void bc_two_sided(BcSmem &S, cplx *AB, int ldab, int 
 __device__ __forceinline__ void bc_load_diag(BcSmem &S, const cplx *AB, int ldab, int r0, int len, int tid) {
     const int c = tid >> 2, p8 = (tid & 3) * 8;
     const cplx *src = AB + (size_t)(r0 + c) * ldab;
+    cplx val[8];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {             // eight independent loads in flight per thread
+        const int rr = p8 + t;
+        val[t] = (rr >= c && rr < len && c < len) ? src[rr - c] : mk(0.0, 0.0);
+    }
 #pragma unroll
     for (int t = 0; t < 8; ++t) {
         const int rr = p8 + t;
         if (rr >= c) {
-            const cplx val = (rr < len && c < len) ? ldcg_(src + (rr - c)) : mk(0.0, 0.0);
-            S.D[rr * kBcP + c] = val;
-            if (rr > c) S.D[c * kBcP + rr] = conj_(val);
+            S.D[rr * kBcP + c] = val[t];
+            if (rr > c) S.D[c * kBcP + rr] = conj_(val[t]);
         }
     }
 }
@@ -169,7 +174,7 @@ __global__ void __launch_bounds__(kBcThreads) hb2st_kernel(BcArgs a) {
             if (k == 0) {
                 // column s below the diagonal
                 cplx x = mk(0.0, 0.0);
-                if (tid < kBW && tid < len) x = ldcg_(a.AB + (size_t)s * ldab + 1 + tid);
+                if (tid < kBW && tid < len) x = a.AB[(size_t)s * ldab + 1 + tid];
                 bc_load_diag(S, a.AB, ldab, r0, len, tid);
                 if (warp == 0) {
                     double p2 = (lane >= 1) ? abs2(x) : 0.0;
@@ -181,7 +186,7 @@ __global__ void __launch_bounds__(kBcThreads) hb2st_kernel(BcArgs a) {
                     S.v[lane] = (lane == 0) ? mk(1.0, 0.0) : (lane < len ? x * scale : mk(0.0, 0.0));
                     if (lane == 0) {
                         S.alpha = tau; S.red[4] = beta;
-                        a.d[s] = ldcg_(a.AB + (size_t)s * ldab).x;
+                        a.d[s] = a.AB[(size_t)s * ldab].x;
                         a.e[s] = beta;
                     }
                 }
@@ -193,13 +198,13 @@ __global__ void __launch_bounds__(kBcThreads) hb2st_kernel(BcArgs a) {
                 {
                     const int c = tid >> 2, p8 = (tid & 3) * 8;
                     const cplx *src = a.AB + (size_t)(p0 + c) * ldab + (kBW - c);
+                    cplx val[8];
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) {
-                        const int rr = p8 + t;
-                        S.Bk[rr * kBcP + c] = (rr < len) ? ldcg_(src + rr) : mk(0.0, 0.0);
-                    }
+                    for (int t = 0; t < 8; ++t) val[t] = (p8 + t < len) ? src[p8 + t] : mk(0.0, 0.0);
+                    bc_load_diag(S, a.AB, ldab, r0, len, tid);
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) S.Bk[(p8 + t) * kBcP + c] = val[t];
                 }
-                bc_load_diag(S, a.AB, ldab, r0, len, tid);
                 __syncthreads();
                 // ---- right: B <- B (I - tau_p vp vp^H)
                 cplx b8[8];
@@ -258,10 +263,8 @@ __global__ void __launch_bounds__(kBcThreads) hb2st_kernel(BcArgs a) {
             if (tid == 0) a.tau2[(size_t)k * n + s] = tau;
             tau_prev = tau;
             __syncthreads();                         // all stores of this hop are issued; vp is in place
-            if (tid == 0) {
-                __threadfence();
-                bc_st_release(a.prog + s, (k == nhops - 1) ? kBcDone : k + 1);
-            }
+            // release at gpu scope is cumulative over the stores the block barrier ordered before it: no separate fence
+            if (tid == 0) bc_st_release(a.prog + s, (k == nhops - 1) ? kBcDone : k + 1);
         }
         if (s == n - 2 && tid == 0) a.d[n - 1] = S.D[0].x;      // the 1 x 1 block of the last hop
     }

@@ -106,6 +106,7 @@ LargeWs carve(int n, unsigned char *base) {
         w.q.prog = itg(N);
         w.q.d = w.t.d; w.q.e = w.t.e;
         w.q.T2 = cpx(twostage_q2_blocks(n) * kQ2G * kQ2G);
+        w.q.q2flags = itg(((size_t)n / 32 + 1) * ((size_t)n / kQ2G + 1));
     }
     w.bytes = off;
     return w;

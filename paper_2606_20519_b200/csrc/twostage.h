@@ -35,6 +35,7 @@ struct TwoStageWs {
     int *prog;           // hops completed per sweep (release/acquire flags)
     double *d, *e;       // the real tridiagonal
     cplx *T2;            // kQ2G x kQ2G triangular factor per diamond block
+    int *q2flags;        // (n / 32 slabs) x (sweep groups): pipeline flags of the Q2 kernel
 };
 
 int twostage_init();
