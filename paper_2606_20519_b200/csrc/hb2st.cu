@@ -7,21 +7,33 @@
 //   hop 0:  H_0 from A[s+1 : s+1+b, s];  D_0 <- H_0^H D_0 H_0                 (D_k = A[r_k, r_k], r_k = s+1+kb .. +b)
 //   hop k:  B_k = A[r_k, r_{k-1}] <- B_k H_{k-1};  H_k from column 0 of B_k;  B_k <- H_k^H B_k;  D_k <- H_k^H D_k H_k
 // Every reflector comes from zlarfg (complex tau, REAL beta), so the final sub-diagonal is real without a phase pass.
-// Dependencies: (s, k) needs (s, k-1) and (s-1, k+1).  One CTA runs one sweep at a time (sweep s on CTA s mod G) and
-// publishes its progress with a release store; the next sweep's CTA polls it with acquire loads, so the sweeps run as
-// a pipeline two hops apart over the SMs.  The band lives in L2 (16 * 2b * n bytes: 4.2 MB at n = 4096).
-// The reflectors are kept for the back-transformation (backq2.cu): (s, k) at V2[(k n + s) b], tau2[k n + s].
-#include <cooperative_groups.h>
+//
+// Dependencies: (s, k) needs (s, k-1) and (s-1, k+1): consecutive sweeps run two hops apart and the whole stage is a
+// chain of ~2n hops, i.e. latency-bound.  One CTA runs one sweep at a time (sweep s on CTA s mod G)
+// and publishes its progress with a release store that the next sweep's CTA polls.  Inside a CTA two warp groups
+// split a hop, so that only the B_k work is on the sweep's own chain:
+//   group B (warps 0-3): B_k right update, reflector H_k, left update; hands v_k to group D through shared memory
+//   group D (warps 4-7): D_k two-sided update (at most two hops behind), then the release of hop k
+// Every thread keeps its 8 block elements in registers (loaded straight from the band in L2, stored straight back).
+// The band lives in L2 (16 * 2b * n bytes: 4.2 MB at n = 4096).  The reflectors are kept for the back-transformation
+// (backq2.cu): (s, k) at V2[(k n + s) b], tau2[k n + s].
 #include "kernels.h"
 #include "twostage.h"
 #include "prof.h"
 
 namespace hpsd {
 
-constexpr int kBcThreads = 128;
-constexpr int kBcP = kBW + 4;            // shared-memory pitch of the blocks (elements): thread tiles (row, 4 lanes) conflict free
+constexpr int kBcGroup = 128;                 // threads per warp group
+constexpr int kBcThreads = 2 * kBcGroup;
+constexpr int kBcP = kBW + 2;                 // pitch of the transposed staging of B_k (row index contiguous)
 constexpr int kBcDone = 1 << 30;
-static_assert(kBW == 32 && kBcThreads == 128, "thread tiling of the bulge-chasing kernel");
+static_assert(kBW == 32 && kBcGroup == 128, "thread tiling of the bulge-chasing kernel: 4 threads per block row");
+
+// named barriers (0 is left to __syncthreads).  VREADY: B arrives, D waits.  VFREE: D arrives, B waits (two hops later).
+// BSTORED: B arrives, D waits.  The [slot] variants alternate with the hop counter.
+enum { BAR_B = 1, BAR_D = 2, BAR_VREADY = 3, BAR_VFREE = 5, BAR_BSTORED = 7 };
+__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
 struct BcArgs {
     int n, ldab;
@@ -40,16 +52,20 @@ __device__ __forceinline__ void bc_st_release(int *p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+// zlarfg scalars with one reciprocal square root and one reciprocal on the dependent chain
 __device__ __forceinline__ void bc_householder(cplx alpha, double xnorm2, double &beta, cplx &tau, cplx &scale) {
     if (xnorm2 == 0.0 && alpha.y == 0.0) {
         beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
     } else {
-        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        const double s = alpha.x * alpha.x + alpha.y * alpha.y + xnorm2;
+        double rinv = rsqrt(s);
+        rinv = fma(0.5 * rinv, fma(-s * rinv, rinv, 1.0), rinv);      // one Newton step: full accuracy
+        const double nrm = s * rinv;
         beta = -copysign(nrm, alpha.x);
-        const double ib = 1.0 / beta;
+        const double ib = -copysign(rinv, alpha.x);
         tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
         const cplx den = mk(alpha.x - beta, alpha.y);
-        const double id2 = 1.0 / abs2(den);
+        const double id2 = __drcp_rn(abs2(den));
         scale = mk(den.x * id2, -den.y * id2);
     }
 }
@@ -71,202 +87,177 @@ __device__ __forceinline__ double oct_sum(double v) {
 }
 
 struct BcSmem {
-    cplx Bk[kBW * kBcP];
-    cplx D[kBW * kBcP];
-    cplx v[kBW], vp[kBW], w[kBW];
-    double red[8];
+    cplx Bt[kBW * kBcP];           // B_k transposed staging for the left update: Bt[c][r]
+    cplx v[2][kBW];                // reflector ring (slot = hop counter & 1)
+    cplx w[kBW];
+    cplx tau[2];
+    double redB[4], redD[4];
     cplx alpha;
-    int flag;
 };
 
-// D (len x len, full in shared memory) <- H^H D H with H = I - tau v v^H (zhetd2 arithmetic): x = tau D v,
-// w = x - 1/2 tau (x^H v) v,  D -= v w^H + w v^H.  The lower triangle goes back to the band.
-__device__ __forceinline__ void bc_two_sided(BcSmem &S, cplx *AB, int ldab, int r0, int len, cplx tau, int tid) {
-    const int r = tid >> 2, q = tid & 3, lane = tid & 31, warp = tid >> 5;
-    cplx y = mk(0.0, 0.0);
-#pragma unroll
-    for (int t = 0; t < 8; ++t) cfma(y, S.D[r * kBcP + q + 4 * t], S.v[q + 4 * t]);
-    y = quad_sum(y);
-    // dot = v^H y (real for Hermitian D; the imaginary rounding residue is dropped)
-    double part = (q == 0) ? (S.v[r].x * y.x + S.v[r].y * y.y) : 0.0;
-    part = oct_sum(part);
-    if (lane == 0) S.red[warp] = part;
-    __syncthreads();
-    const double dot = (S.red[0] + S.red[1]) + (S.red[2] + S.red[3]);
-    // w_r = tau y_r - 1/2 |tau|^2 dot v_r
-    if (q == 0) {
-        const double c = 0.5 * abs2(tau) * dot;
-        const cplx vr = S.v[r];
-        const cplx ty = tau * y;
-        S.w[r] = mk(ty.x - c * vr.x, ty.y - c * vr.y);
-    }
-    __syncthreads();
-    {
-        const cplx vr = S.v[r], wr = S.w[r];
-#pragma unroll
-        for (int t = 0; t < 8; ++t) {
-            const int c = q + 4 * t;
-            cplx dv = S.D[r * kBcP + c];
-            const cplx vc = conj_(S.v[c]), wc = conj_(S.w[c]);
-            cfma(dv, mk(-vr.x, -vr.y), wc);
-            cfma(dv, mk(-wr.x, -wr.y), vc);
-            if (r == c) dv.y = 0.0;
-            S.D[r * kBcP + c] = dv;
-        }
-    }
-    __syncthreads();
-    // lower triangle -> band: column c = tid / 4, rows part of 8
-    {
-        const int c = tid >> 2, p8 = (tid & 3) * 8;
-        if (c < len) {
-            cplx *dst = AB + (size_t)(r0 + c) * ldab;
-#pragma unroll
-            for (int t = 0; t < 8; ++t) {
-                const int rr = p8 + t;
-                if (rr >= c && rr < len) dst[rr - c] = S.D[rr * kBcP + c];
-            }
-        }
-    }
-}
-
-// load D = A[r0 : r0+len, r0 : r0+len] from the band (lower stored) as a full Hermitian block, zero padded to b x b
-__device__ __forceinline__ void bc_load_diag(BcSmem &S, const cplx *AB, int ldab, int r0, int len, int tid) {
-    const int c = tid >> 2, p8 = (tid & 3) * 8;
-    const cplx *src = AB + (size_t)(r0 + c) * ldab;
-    cplx val[8];
-#pragma unroll
-    for (int t = 0; t < 8; ++t) {             // eight independent loads in flight per thread
-        const int rr = p8 + t;
-        val[t] = (rr >= c && rr < len && c < len) ? src[rr - c] : mk(0.0, 0.0);
-    }
-#pragma unroll
-    for (int t = 0; t < 8; ++t) {
-        const int rr = p8 + t;
-        if (rr >= c) {
-            S.D[rr * kBcP + c] = val[t];
-            if (rr > c) S.D[c * kBcP + rr] = conj_(val[t]);
-        }
-    }
-}
-
-__global__ void __launch_bounds__(kBcThreads) hb2st_kernel(BcArgs a) {
+__global__ void __launch_bounds__(kBcThreads, 1) hb2st_kernel(BcArgs a) {
     extern __shared__ __align__(16) unsigned char bc_smem[];
     BcSmem &S = *reinterpret_cast<BcSmem *>(bc_smem);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x;
+    const bool isB = tid < kBcGroup;
+    const int gt = tid & (kBcGroup - 1), lane = tid & 31, gw = gt >> 5;     // thread / warp inside the group
+    const int r = gt >> 2, q = gt & 3;                                      // block row, column residue (columns q + 4t)
     const int n = a.n, ldab = a.ldab;
-    const int r = tid >> 2, q = tid & 3;
+    unsigned h = 0;                                                         // hop counter of this CTA (both groups count alike)
 
     for (int s = blockIdx.x; s < n - 1; s += gridDim.x) {
         const int nhops = (n - 1 - s + kBW - 1) / kBW;
         cplx tau_prev = mk(0.0, 0.0);
-        for (int k = 0; k < nhops; ++k) {
-            // ---- wait for sweep s-1 to be two hops ahead
+        for (int k = 0; k < nhops; ++k, ++h) {
+            const int slot = h & 1;
+            const int r0 = s + 1 + k * kBW;
+            const int len = (n - r0 < kBW) ? n - r0 : kBW;
+            // ---- wait for sweep s-1 to be two hops ahead (each group polls for itself, then loads its own block;
+            //      the acquire invalidates this SM's L1, so the plain loads below see what the other SM published)
             if (s > 0) {
-                if (tid == 0) {
+                if (gt == 0) {
                     const int *pp = a.prog + (s - 1);
                     while (bc_ld_acquire(pp) < k + 2) { }
                 }
-                __syncthreads();
+                bar_sync(isB ? BAR_B : BAR_D, kBcGroup);
             }
-            const int r0 = s + 1 + k * kBW;
-            const int len = (n - r0 < kBW) ? n - r0 : kBW;
-            double beta; cplx tau, scale;
-            if (k == 0) {
-                // column s below the diagonal
-                cplx x = mk(0.0, 0.0);
-                if (tid < kBW && tid < len) x = a.AB[(size_t)s * ldab + 1 + tid];
-                bc_load_diag(S, a.AB, ldab, r0, len, tid);
-                if (warp == 0) {
-                    double p2 = (lane >= 1) ? abs2(x) : 0.0;
-                    p2 = warp_sum(p2);
-                    cplx alpha;
-                    alpha.x = __shfl_sync(0xffffffffu, x.x, 0);
-                    alpha.y = __shfl_sync(0xffffffffu, x.y, 0);
-                    bc_householder(alpha, p2, beta, tau, scale);
-                    S.v[lane] = (lane == 0) ? mk(1.0, 0.0) : (lane < len ? x * scale : mk(0.0, 0.0));
-                    if (lane == 0) {
-                        S.alpha = tau; S.red[4] = beta;
-                        a.d[s] = a.AB[(size_t)s * ldab].x;
-                        a.e[s] = beta;
-                    }
-                }
-                __syncthreads();
-                tau = S.alpha;
-            } else {
-                const int p0 = r0 - kBW;
-                // ---- load B_k = A[r0 : r0+len, p0 : p0+b] (column c: band offsets b - c ..) and D_k
-                {
-                    const int c = tid >> 2, p8 = (tid & 3) * 8;
-                    const cplx *src = a.AB + (size_t)(p0 + c) * ldab + (kBW - c);
-                    cplx val[8];
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) val[t] = (p8 + t < len) ? src[p8 + t] : mk(0.0, 0.0);
-                    bc_load_diag(S, a.AB, ldab, r0, len, tid);
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) S.Bk[(p8 + t) * kBcP + c] = val[t];
-                }
-                __syncthreads();
-                // ---- right: B <- B (I - tau_p vp vp^H)
+            if (isB) {
+                // =========================== group B: reflector of this hop ===========================
+                double beta = 0.0; cplx tau = mk(0.0, 0.0), scale = mk(0.0, 0.0);
                 cplx b8[8];
-                {
+                cplx x0 = mk(0.0, 0.0);                              // hop 0, warp 0: column s below the diagonal
+                if (k == 0) {
+                    if (gw == 0) {
+                        if (lane < len) x0 = a.AB[(size_t)s * ldab + 1 + lane];
+                        double p2 = (lane >= 1) ? abs2(x0) : 0.0;
+                        p2 = warp_sum(p2);
+                        cplx alpha;
+                        alpha.x = __shfl_sync(0xffffffffu, x0.x, 0);
+                        alpha.y = __shfl_sync(0xffffffffu, x0.y, 0);
+                        bc_householder(alpha, p2, beta, tau, scale);
+                    }
+                } else {
+                    const int p0 = r0 - kBW;
+                    // B_k = A[r0 : r0+len, p0 : p0+b]: element (r, c) at band offset b + r - c of column p0 + c
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) {
+                        const int c = q + 4 * t;
+                        b8[t] = (r < len) ? a.AB[(size_t)(p0 + c) * ldab + (kBW + r - c)] : mk(0.0, 0.0);
+                    }
+                    // right: B <- B (I - tau_p vp vp^H)
+                    const cplx *vp = S.v[slot ^ 1];
+                    cplx vpc[8];
                     cplx wv = mk(0.0, 0.0);
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) { b8[t] = S.Bk[r * kBcP + q + 4 * t]; cfma(wv, b8[t], S.vp[q + 4 * t]); }
+                    for (int t = 0; t < 8; ++t) { vpc[t] = vp[q + 4 * t]; cfma(wv, b8[t], vpc[t]); }
                     wv = quad_sum(wv);
                     const cplx tw = tau_prev * wv;
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) cfma(b8[t], mk(-tw.x, -tw.y), conj_(S.vp[q + 4 * t]));
-                }
-                // ---- new reflector from column 0 (threads with q == 0 hold it in b8[0])
-                {
+                    for (int t = 0; t < 8; ++t) cfma(b8[t], mk(-tw.x, -tw.y), conj_(vpc[t]));
+                    // new reflector from column 0 (threads with q == 0 hold it in b8[0])
                     double p2 = (q == 0 && r >= 1) ? abs2(b8[0]) : 0.0;
                     p2 = oct_sum(p2);
-                    if (lane == 0) S.red[warp] = p2;
-                    if (tid == 0) S.alpha = b8[0];
-                }
-                __syncthreads();
-                {
-                    const double xn2 = (S.red[0] + S.red[1]) + (S.red[2] + S.red[3]);
+                    if (lane == 0) S.redB[gw] = p2;
+                    if (gt == 0) S.alpha = b8[0];
+                    bar_sync(BAR_B, kBcGroup);
+                    const double xn2 = (S.redB[0] + S.redB[1]) + (S.redB[2] + S.redB[3]);
                     bc_householder(S.alpha, xn2, beta, tau, scale);
+                }
+                // the slot of the reflector ring is free once group D is through hop h - 2
+                if (h >= 2) bar_sync(BAR_VFREE + slot, kBcThreads);
+                // ---- publish v_k, tau_k (and B_k, transposed, for the left update)
+                if (k == 0) {
+                    if (gw == 0) {
+                        S.v[slot][lane] = (lane == 0) ? mk(1.0, 0.0) : (lane < len ? x0 * scale : mk(0.0, 0.0));
+                        if (lane == 0) {
+                            S.tau[slot] = tau;
+                            a.d[s] = a.AB[(size_t)s * ldab].x;
+                            a.e[s] = beta;
+                        }
+                    }
+                } else {
                     if (q == 0) {
-                        S.v[r] = (r == 0) ? mk(1.0, 0.0) : (r < len ? b8[0] * scale : mk(0.0, 0.0));
+                        S.v[slot][r] = (r == 0) ? mk(1.0, 0.0) : (r < len ? b8[0] * scale : mk(0.0, 0.0));
                         b8[0] = (r == 0) ? mk(beta, 0.0) : mk(0.0, 0.0);
+                        if (r == 0) S.tau[slot] = tau;
                     }
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) S.Bk[r * kBcP + q + 4 * t] = b8[t];
+                    for (int t = 0; t < 8; ++t) S.Bt[(q + 4 * t) * kBcP + r] = b8[t];
                 }
-                __syncthreads();
-                // ---- left: columns 1 .. b-1:  B <- B - conj(tau) v (v^H B)     (thread = column c, rows q + 4t)
-                {
-                    const int c = tid >> 2;
-                    cplx col[8];
+                bar_sync(BAR_B, kBcGroup);
+                tau = S.tau[slot];
+                bar_arrive(BAR_VREADY + slot, kBcThreads);          // group D may start on D_k
+                if (gt < kBW) a.V2[((size_t)k * n + s) * kBW + gt] = S.v[slot][gt];
+                if (gt == 0) a.tau2[(size_t)k * n + s] = tau;
+                if (k > 0) {
+                    // left: columns 1 .. b-1:  B <- B - conj(tau) v (v^H B)     (thread = column c, rows q + 4t)
+                    const int p0 = r0 - kBW;
+                    const int c = gt >> 2;
+                    cplx col[8], vv[8];
                     cplx z = mk(0.0, 0.0);
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) { col[t] = S.Bk[(q + 4 * t) * kBcP + c]; cfma_conj(z, S.v[q + 4 * t], col[t]); }
+                    for (int t = 0; t < 8; ++t) { col[t] = S.Bt[c * kBcP + q + 4 * t]; vv[t] = S.v[slot][q + 4 * t]; cfma_conj(z, vv[t], col[t]); }
                     z = quad_sum(z);
                     const cplx ctz = conj_(tau) * z;
                     cplx *dst = a.AB + (size_t)(p0 + c) * ldab + (kBW - c);
 #pragma unroll
                     for (int t = 0; t < 8; ++t) {
                         const int rr = q + 4 * t;
-                        if (c >= 1) cfma(col[t], mk(-ctz.x, -ctz.y), S.v[rr]);
+                        if (c >= 1) cfma(col[t], mk(-ctz.x, -ctz.y), vv[t]);
                         if (rr < len) dst[rr] = col[t];
                     }
                 }
+                tau_prev = tau;
+                bar_arrive(BAR_BSTORED + slot, kBcThreads);         // B_k is on its way to L2
+            } else {
+                // =========================== group D: two-sided update of D_k ===========================
+                cplx d8[8];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const int c = q + 4 * t;
+                    // stored lower: (r, c) with r < c is the conjugate of (c, r); one load either way, no branch
+                    const int lo = r < c ? r : c, df = r < c ? c - r : r - c;
+                    cplx val = (r < len && c < len) ? a.AB[(size_t)(r0 + lo) * ldab + df] : mk(0.0, 0.0);
+                    if (r < c) val.y = -val.y;
+                    d8[t] = val;
+                }
+                bar_sync(BAR_VREADY + slot, kBcThreads);            // v_k, tau_k are in the ring
+                const cplx *v = S.v[slot];
+                const cplx tau = S.tau[slot];
+                cplx vc[8];
+                cplx y = mk(0.0, 0.0);
+#pragma unroll
+                for (int t = 0; t < 8; ++t) { vc[t] = v[q + 4 * t]; cfma(y, d8[t], vc[t]); }
+                y = quad_sum(y);
+                const cplx vr = v[r];
+                // dot = v^H y (real for Hermitian D; the imaginary rounding residue is dropped)
+                double part = (q == 0) ? (vr.x * y.x + vr.y * y.y) : 0.0;
+                part = oct_sum(part);
+                if (lane == 0) S.redD[gw] = part;
+                if (q == 0) S.w[r] = y;                              // y, not w: every thread finishes w_c itself (one exchange)
+                bar_sync(BAR_D, kBcGroup);
+                const double dot = (S.redD[0] + S.redD[1]) + (S.redD[2] + S.redD[3]);
+                // w_r = tau y_r - 1/2 |tau|^2 dot v_r     (zhetd2: x = tau D v, w = x - 1/2 tau (x^H v) v)
+                const double cc = 0.5 * abs2(tau) * dot;
+                const cplx ty = tau * y;
+                const cplx wr = mk(ty.x - cc * vr.x, ty.y - cc * vr.y);
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const int c = q + 4 * t;
+                    const cplx tyc = tau * S.w[c];
+                    const cplx wc = mk(tyc.x - cc * vc[t].x, -(tyc.y - cc * vc[t].y));      // conj(w_c)
+                    cfma(d8[t], mk(-vr.x, -vr.y), wc);
+                    cfma(d8[t], mk(-wr.x, -wr.y), conj_(vc[t]));
+                    if (r == c) d8[t].y = 0.0;
+                    if (r >= c && r < len) a.AB[(size_t)(r0 + c) * ldab + (r - c)] = d8[t];
+                }
+                if (s == n - 2 && gt == 0) a.d[n - 1] = d8[0].x;   // the 1 x 1 block of the last sweep
+                bar_sync(BAR_BSTORED + slot, kBcThreads);           // group B's stores of this hop are issued as well
+                // release at gpu scope is cumulative over the stores the barriers ordered before it
+                if (gt == 0) bc_st_release(a.prog + s, (k == nhops - 1) ? kBcDone : k + 1);
+                bar_arrive(BAR_VFREE + slot, kBcThreads);           // ring slot and S.w are free again
             }
-            // ---- D_k <- H_k^H D_k H_k, reflector out
-            bc_two_sided(S, a.AB, ldab, r0, len, tau, tid);
-            if (tid < kBW) {
-                a.V2[((size_t)k * n + s) * kBW + tid] = S.v[tid];
-                S.vp[tid] = S.v[tid];
-            }
-            if (tid == 0) a.tau2[(size_t)k * n + s] = tau;
-            tau_prev = tau;
-            __syncthreads();                         // all stores of this hop are issued; vp is in place
-            // release at gpu scope is cumulative over the stores the block barrier ordered before it: no separate fence
-            if (tid == 0) bc_st_release(a.prog + s, (k == nhops - 1) ? kBcDone : k + 1);
         }
-        if (s == n - 2 && tid == 0) a.d[n - 1] = S.D[0].x;      // the 1 x 1 block of the last hop
     }
 }
 
