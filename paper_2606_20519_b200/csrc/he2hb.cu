@@ -8,7 +8,7 @@
 //          panel columns; norm, v^H P and the column V^H v of the T recurrence all follow from them.
 //          R goes to the band, V (explicit unit diagonal) to V1, T to Tk.
 //   [HEMM] Zp[s] = A22[:, K_s] V[K_s, :]           split-K complex DMMA GEMM over all SMs (A22 is stored in full)
-//   [SLAB] Z = sum_s Zp[s]; G = V^H Z (last CTA done: S = -1/2 T^H G T)
+//   [ZSUM] Z = sum_s Zp[s];  [GRAM] G = V^H Z (split-K DMMA);  [S] S = -1/2 T^H G T
 //   [X]    X = Z T + V S                            (= A22 V T - 1/2 V T^H V^H A22 V T)
 //   [HER2K] A22 -= X V^H + V X^H                    lower tiles on DMMA, each element mirrored into the upper triangle
 // so that all (16/3) n^3 flops of the reduction are BLAS-3 and the dependent chain is n cluster exchanges instead of
@@ -23,7 +23,7 @@
 namespace hpsd {
 
 constexpr int kQrCl = 16;                 // CTAs per cluster (non-portable size)
-constexpr int kQrWarps = 10;              // warp 0: top b x b block (kept by every CTA), warps 1..8: 32 rows each, warp 9: T
+constexpr int kQrWarps = 10;              // warp 0: top b x b block (kept by every CTA), warps 1..8: one row per thread, warp 9: T
 constexpr int kQrThreads = kQrWarps * 32;
 constexpr int kQrRows = 256;              // ordinary rows per CTA
 constexpr int kQrP = kBW + 1;             // shared-memory pitch (elements): row-wise and column-wise accesses conflict free
@@ -45,8 +45,8 @@ struct QrSmem {
     static constexpr size_t scl = tau + sizeof(cplx) * kBW;                      // [kBW]
     static constexpr size_t top = scl + sizeof(cplx) * kBW;                      // [kBW][kQrP]
     static constexpr size_t tf = top + sizeof(cplx) * kBW * kQrP;                // [kBW][kQrP]
-    static constexpr size_t rows = tf + sizeof(cplx) * kBW * kQrP;               // [kQrRows][kQrP]
-    static constexpr size_t total = rows + sizeof(cplx) * kQrRows * kQrP;
+    static constexpr size_t fb = tf + sizeof(cplx) * kBW * kQrP;                 // [kQrWarps][kBW]: update coefficients per warp
+    static constexpr size_t total = fb + sizeof(cplx) * kQrWarps * kBW;
 };
 
 // zlarfg scalars: H = I - tau v v^H with v = [1; x scale] maps [alpha; x] to [beta; 0], beta real
@@ -54,12 +54,16 @@ __device__ __forceinline__ void qr_householder(cplx alpha, double xnorm2, double
     if (xnorm2 == 0.0 && alpha.y == 0.0) {
         beta = alpha.x; tau = mk(0.0, 0.0); scale = mk(0.0, 0.0);
     } else {
-        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2);
+        // one reciprocal square root (refined by a Newton step to full accuracy) and one reciprocal on the dependent chain
+        const double s = alpha.x * alpha.x + alpha.y * alpha.y + xnorm2;
+        double rinv = rsqrt(s);
+        rinv = fma(0.5 * rinv, fma(-s * rinv, rinv, 1.0), rinv);
+        const double nrm = s * rinv;
         beta = -copysign(nrm, alpha.x);
-        const double ib = 1.0 / beta;
+        const double ib = -copysign(rinv, alpha.x);
         tau = mk((beta - alpha.x) * ib, -alpha.y * ib);
         const cplx den = mk(alpha.x - beta, alpha.y);
-        const double id2 = 1.0 / abs2(den);
+        const double id2 = __drcp_rn(abs2(den));
         scale = mk(den.x * id2, -den.y * id2);
     }
 }
@@ -92,6 +96,28 @@ __device__ __forceinline__ void qr_update(cplx *P, int r0, int r1, int j, int la
     }
 }
 
+// ---- ordinary rows: thread = row, the 32 panel entries of the row live in REGISTERS (shared memory cannot feed one
+// pass over 256 x 32 complex per column step: 3000 cycles of LDS/STS wavefronts per step, measured).  The array is
+// rotated by one position per step, so that the active column is always p[0] and every index is static:
+// after step j, p[k] holds panel column (j + 1 + k) mod 32.
+//
+// Warp-wide sums of the 32 products conj(p[0]) p[k] by a depth-first halving butterfly: the recursion keeps only
+// log2(32) partial sums alive.  Lane L ends up with the sum of index L.
+template <int A, int LEN>
+__device__ __forceinline__ cplx qr_reduce(const cplx (&p)[kBW], cplx x, int lane) {
+    if constexpr (LEN == 1) {
+        cplx c = mk(0.0, 0.0);
+        cfma_conj(c, x, p[A]);
+        return c;
+    } else {
+        const cplx lo = qr_reduce<A, LEN / 2>(p, x, lane);
+        const cplx hi = qr_reduce<A + LEN / 2, LEN / 2>(p, x, lane);
+        const bool up = (lane & (LEN / 2)) != 0;
+        const cplx keep = up ? hi : lo, send = up ? lo : hi;
+        return mk(keep.x + __shfl_xor_sync(0xffffffffu, send.x, LEN / 2), keep.y + __shfl_xor_sync(0xffffffffu, send.y, LEN / 2));
+    }
+}
+
 __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
     extern __shared__ __align__(16) unsigned char sm[];
     cplx *s_land = reinterpret_cast<cplx *>(sm + QrSmem::land);
@@ -102,7 +128,7 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
     cplx *s_scl = reinterpret_cast<cplx *>(sm + QrSmem::scl);
     cplx *s_top = reinterpret_cast<cplx *>(sm + QrSmem::top);
     cplx *s_T = reinterpret_cast<cplx *>(sm + QrSmem::tf);
-    cplx *s_P = reinterpret_cast<cplx *>(sm + QrSmem::rows);
+    cplx *s_f = reinterpret_cast<cplx *>(sm + QrSmem::fb);
     const unsigned mbar0 = cx_smem_u32(sm + QrSmem::mbar);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -130,14 +156,14 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
         s_T[l * kQrP + k] = mk(0.0, 0.0);
     }
     if (tid < kBW) { s_tau[tid] = mk(0.0, 0.0); s_scl[tid] = mk(0.0, 0.0); }
-    // ordinary rows of this CTA: lane = row (coalesced 512-byte segments), one panel column per iteration
-    if (warp >= 1 && warp <= 8) {
-        const int r = (warp - 1) * 32 + lane;
-        if (r < cnt) {
-            const cplx *src = a.A + (size_t)j0 * lda + g0 + kBW + lo + r;
-#pragma unroll 8
-            for (int k = 0; k < kBW; ++k) s_P[r * kQrP + k] = src[(size_t)k * lda];
-        }
+    // ordinary rows of this CTA: thread = row (coalesced 512-byte segments per panel column), straight into registers
+    cplx p[kBW];
+    const int myrow = (warp - 1) * 32 + lane;
+    const bool has_row = warp >= 1 && warp <= 8 && myrow < cnt;
+    {
+        const cplx *src = a.A + (size_t)j0 * lda + g0 + kBW + lo + (has_row ? myrow : 0);
+#pragma unroll
+        for (int k = 0; k < kBW; ++k) p[k] = has_row ? src[(size_t)k * lda] : mk(0.0, 0.0);
     }
     // diagonal block of this panel -> band (final: no later update touches it)
     if (rank == kQrCl - 1) {
@@ -149,8 +175,7 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
     __syncthreads();
     cx_barrier();                                // every mbarrier of the cluster is initialised and armed
 
-    const int r0 = (warp - 1) * 32;
-    const int r1 = (warp >= 1 && warp <= 8) ? (cnt < r0 + 32 ? cnt : r0 + 32) : 0;
+    const bool row_warp = warp >= 1 && warp <= 8 && (warp - 1) * 32 < cnt;      // warp-uniform
 
     for (int j = 0; j < nsteps; ++j) {
         const int par = j & 1;
@@ -159,8 +184,11 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
         if (warp == 0) {
             s_row[par * kBW + lane] = s_top[j * kQrP + lane];
             if (rank == 0) acc = qr_dots(s_top, j + 1, kBW, j, lane);
-        } else if (r1 > r0) {
-            acc = qr_dots(s_P, r0, r1, j, lane);
+        } else if (row_warp) {
+            // index L of the rotated array is panel column (j + L) mod 32
+            const cplx red = qr_reduce<0, kBW>(p, p[0], lane);
+            acc.x = __shfl_sync(0xffffffffu, red.x, (lane - j) & (kBW - 1));
+            acc.y = __shfl_sync(0xffffffffu, red.y, (lane - j) & (kBW - 1));
         }
         // (double-buffered: a warp that is through the exchange of step j may write its step j + 1 partial while a slower
         // warp of this CTA is still summing the partials of step j)
@@ -200,9 +228,21 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
             else if (lane == j) { s_top[j * kQrP + j] = mk(beta, 0.0); s_tau[j] = tau; s_scl[j] = scale; }
             qr_update(s_top, j + 1, kBW, j, lane, f, scale);
             __syncwarp();
-        } else if (r1 > r0) {
-            qr_update(s_P, r0, r1, j, lane, f, scale);
+        } else if (row_warp) {
+            // every thread needs the coefficients of ALL remaining columns: through the warp's own shared-memory line
+            s_f[warp * kBW + lane] = f;
             __syncwarp();
+            const cplx v = p[0] * scale;
+            const cplx nv = mk(-v.x, -v.y);
+#pragma unroll
+            for (int k = 1; k < kBW; ++k)
+                if (k <= kBW - 1 - j) cfma(p[k], s_f[warp * kBW + ((j + k) & (kBW - 1))], nv);      // columns j+1 .. 31 only
+            __syncwarp();
+            // rotate: the next step's column moves to p[0]; the raw column j (V = p scl_j) goes to the end
+            const cplx x = p[0];
+#pragma unroll
+            for (int k = 0; k < kBW - 1; ++k) p[k] = p[k + 1];
+            p[kBW - 1] = x;
         } else if (warp == kQrWarps - 1 && rank == 0) {
             // column j of T:  T(0:j, j) = -tau T(0:j, 0:j) (V(:, 0:j)^H v_j),  T(j, j) = tau   (zlarft, forward columnwise)
             // V[:, k] = P[:, k] scl[k] below its unit entry, so  V(:,k)^H v_j = conj(V[j,k]) + conj(scl_k) scale sum_{l>j} conj(P[l,k]) P[l,j]
@@ -221,13 +261,11 @@ __global__ void __launch_bounds__(kQrThreads, 1) he2hb_panel_kernel(QrArgs a) {
     }
     __syncthreads();
     // ---- results: V (unit diagonal explicit; zeros above come from the memset of V1), R -> band, tau, T
-    if (warp >= 1 && warp <= 8) {
-        const int r = r0 + lane;
-        if (r < cnt) {
-            cplx *dst = a.V1 + (size_t)j0 * a.ldv + g0 + kBW + lo + r;
-#pragma unroll 8
-            for (int k = 0; k < kBW; ++k) dst[(size_t)k * a.ldv] = s_P[r * kQrP + k] * s_scl[k];
-        }
+    if (has_row) {
+        // ordinary rows exist only when the panel has 32 steps: 32 rotations put p[k] back on column k
+        cplx *dst = a.V1 + (size_t)j0 * a.ldv + g0 + kBW + lo + myrow;
+#pragma unroll
+        for (int k = 0; k < kBW; ++k) dst[(size_t)k * a.ldv] = p[k] * s_scl[k];
     }
     if (rank == 0) {
         for (int e = tid; e < kBW * kBW; e += kQrThreads) {
@@ -283,81 +321,64 @@ __global__ void __launch_bounds__(HM_THREADS, 2) he2hb_hemm_kernel(HemmArgs h) {
 }
 
 struct SlabArgs {
-    int m, ldv, ldz, splits, nslabs;
+    int m, ldv, ldz, splits, nslabs;      // nslabs: number of Gram partials
     const cplx *V, *Zp, *Tk;
     cplx *Z, *Gp, *S;
     unsigned *counter;
 };
 
-// 64-row slab: Z = sum_s Zp[s], partial Gram G_c = V_slab^H Z_slab; the last CTA to finish sums the partials in a fixed
-// order (deterministic) and forms S = -1/2 T^H G T.
-__global__ void __launch_bounds__(128) he2hb_slab_kernel(SlabArgs s) {
-    extern __shared__ __align__(16) unsigned char slab_smem[];
-    cplx (*sZ)[kBW + 1] = reinterpret_cast<cplx (*)[kBW + 1]>(slab_smem);
-    cplx (*sV)[kBW + 1] = sZ + 64;
-    __shared__ bool is_last;
-    const int tid = threadIdx.x;
-    const int r0 = blockIdx.x * 64;
-    for (int e = tid; e < 64 * kBW; e += 128) {
-        const int r = e % 64, c = e / 64;
-        cplx z = mk(0.0, 0.0), v = mk(0.0, 0.0);
-        if (r0 + r < s.m) {
-            for (int k = 0; k < s.splits; ++k) z = z + s.Zp[((size_t)k * kBW + c) * s.ldz + r0 + r];
-            s.Z[(size_t)c * s.ldz + r0 + r] = z;
-            v = s.V[(size_t)c * s.ldv + r0 + r];
-        }
-        sZ[r][c] = z; sV[r][c] = v;
-    }
-    __syncthreads();
-    // G[a][c] = sum_r conj(V[r][a]) Z[r][c]: thread = (a, 8 columns)
-    {
-        const int a = tid >> 2, c0 = (tid & 3) * 8;
-        cplx acc[8];
+// Z = sum_s Zp[s]: one element per thread, all split-K partials of the element in flight at once
+// (a load -> add loop would be a chain of L2 round trips)
+__global__ void __launch_bounds__(256) he2hb_zsum_kernel(SlabArgs s) {
+    const int e = blockIdx.x * 256 + threadIdx.x;
+    if (e >= s.m * kBW) return;
+    const int r = e % s.m, c = e / s.m;
+    cplx zp[kHemmSplitMax];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) acc[q] = mk(0.0, 0.0);
-        for (int r = 0; r < 64; ++r) {
-            const cplx v = sV[r][a];
+    for (int k = 0; k < kHemmSplitMax; ++k) zp[k] = (k < s.splits) ? s.Zp[((size_t)k * kBW + c) * s.ldz + r] : mk(0.0, 0.0);
+    cplx z = mk(0.0, 0.0);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) cfma_conj(acc[q], v, sZ[r][c0 + q]);
-        }
-        cplx *gp = s.Gp + (size_t)blockIdx.x * kBW * kBW;
+    for (int k = 0; k < kHemmSplitMax; ++k) z = z + zp[k];
+    s.Z[(size_t)c * s.ldz + r] = z;
+}
+
+// Gp[s] = V[K_s, :]^H Z[K_s, :]: split-K complex DMMA GEMM (32 x 32 output per CTA); summed in a fixed order by he2hb_s_kernel
+constexpr int GR_MI = 2, GR_NI = 2, GR_WM = 2, GR_WN = 2;
+__global__ void __launch_bounds__(GR_WM *GR_WN * 32) he2hb_gram_kernel(SlabArgs s, int chunk) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int k0 = blockIdx.x * chunk;
+    int klen = s.m - k0; if (klen > chunk) klen = chunk; if (klen < 0) klen = 0;
+    GemmProblem<cplx, cplx> p;
+    p.A = s.V + k0; p.lda = s.ldv; p.B = s.Z + k0; p.ldb = s.ldz;
+    p.A2 = nullptr; p.B2 = nullptr; p.lda2 = p.ldb2 = 0; p.M = kBW; p.N = kBW; p.K = klen; p.K2 = 0;
+    StoreEpi2 epi{s.Gp + (size_t)blockIdx.x * kBW * kBW, kBW};
+    gemm_tile_body<cplx, cplx, KMAJ, KMAJ, true, false, GR_MI, GR_NI, GR_WM, GR_WN, false>(p, 0, 0, smem_raw, epi);
+}
+
+// S = -1/2 T^H (sum of the slabs' Gram partials) T, one CTA of 1024 threads (thread = matrix element).  A kernel of its
+// own: the partials come from other CTAs, and reading them inside the slab kernel needs gpu-scope loads
+// (LDG.STRONG.GPU, ~170 issue cycles each: 80 us per panel, measured); across a launch boundary plain loads do.
+__global__ void __launch_bounds__(kBW * kBW) he2hb_s_kernel(SlabArgs s) {
+    __shared__ cplx sG[kBW][kBW], sT[kBW][kBW], sM[kBW][kBW];        // 48 KB
+    const int e = threadIdx.x, r = e % kBW, c = e / kBW;
+    cplx g = mk(0.0, 0.0);
+    for (int k0 = 0; k0 < s.nslabs; k0 += 8) {          // eight independent loads per round trip, fixed summation order
+        cplx gp[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) gp[(c0 + q) * kBW + a] = acc[q];
+        for (int k = 0; k < 8; ++k) gp[k] = (k0 + k < s.nslabs) ? s.Gp[(size_t)(k0 + k) * kBW * kBW + e] : mk(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) g = g + gp[k];
     }
-    __threadfence();
+    sG[r][c] = g;
+    sT[r][c] = s.Tk[e];
     __syncthreads();
-    if (tid == 0) {
-        const unsigned prev = atomicAdd(s.counter, 1u);
-        is_last = (prev == (unsigned)s.nslabs - 1u);
-        if (is_last) *s.counter = 0u;              // self-resetting: the next panel's launch is stream-ordered after this kernel
-    }
+    cplx acc = mk(0.0, 0.0);
+    for (int k = 0; k <= c; ++k) cfma(acc, sG[r][k], sT[k][c]);             // M = G T, T upper triangular
+    sM[r][c] = acc;
     __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    // G (into sZ[0..31]), T (into sV[0..31])
-    for (int e = tid; e < kBW * kBW; e += 128) {
-        const int r = e % kBW, c = e / kBW;
-        cplx g = mk(0.0, 0.0);
-        for (int k = 0; k < s.nslabs; ++k) g = g + ldcg_(s.Gp + (size_t)k * kBW * kBW + e);
-        sZ[r][c] = g;
-        sV[r][c] = s.Tk[e];
-    }
-    __syncthreads();
-    // M = G T  (into sZ[32..63])
-    for (int e = tid; e < kBW * kBW; e += 128) {
-        const int r = e % kBW, c = e / kBW;
-        cplx acc = mk(0.0, 0.0);
-        for (int k = 0; k <= c; ++k) cfma(acc, sZ[r][k], sV[k][c]);        // T upper triangular
-        sZ[32 + r][c] = acc;
-    }
-    __syncthreads();
-    // S = -1/2 T^H M
-    for (int e = tid; e < kBW * kBW; e += 128) {
-        const int r = e % kBW, c = e / kBW;
-        cplx acc = mk(0.0, 0.0);
-        for (int k = 0; k <= r; ++k) cfma_conj(acc, sV[k][r], sZ[32 + k][c]);
-        s.S[e] = mk(-0.5 * acc.x, -0.5 * acc.y);
-    }
+    acc = mk(0.0, 0.0);
+    for (int k = 0; k <= r; ++k) cfma_conj(acc, sT[k][r], sM[k][c]);        // T^H M
+    s.S[e] = mk(-0.5 * acc.x, -0.5 * acc.y);
 }
 
 struct XArgs {
@@ -407,7 +428,8 @@ static int g_ts_ok = 0;
 constexpr size_t kSmemHemm = gemm_smem_bytes<cplx, cplx, MNMAJ, KMAJ, HM_MI, HM_NI, HM_WM, HM_WN, 2>();
 constexpr size_t kSmemH2F = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, H2F_MI, H2F_NI, H2F_WM, H2F_WN, 2>();
 constexpr size_t kSmemH2Fs = gemm_smem_bytes<cplx, cplx, MNMAJ, MNMAJ, 2, 2, H2F_WM, H2F_WN>();
-constexpr size_t kSmemSlab = sizeof(cplx) * 2 * 64 * (kBW + 1);
+constexpr size_t kSmemGram = gemm_smem_bytes<cplx, cplx, KMAJ, KMAJ, GR_MI, GR_NI, GR_WM, GR_WN>();
+constexpr int kGramSplitMax = 32;
 
 int hb2st_init();
 int backq2_init();
@@ -426,7 +448,7 @@ int twostage_init() {
     if (g_ts_init_dev == dev) return 0;
     g_ts_ok = 0;
     if (cudaFuncSetAttribute(he2hb_hemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemHemm) != cudaSuccess) return HPSD_ECUDA_;
-    if (cudaFuncSetAttribute(he2hb_slab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemSlab) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(he2hb_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemGram) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaFuncSetAttribute(he2hb_x_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemHemm) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaFuncSetAttribute(he2hb_her2k_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemH2F) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaFuncSetAttribute(he2hb_her2k_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemH2Fs) != cudaSuccess) return HPSD_ECUDA_;
@@ -494,8 +516,15 @@ int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
         HemmArgs h{m, w.lda, w.ldv, w.ldz2, chunk, A22, V, w.Zp};
         he2hb_hemm_kernel<<<dim3(mt, splits), HM_THREADS, kSmemHemm, st>>>(h);
         HPSD_LAUNCH_CHECK();
-        SlabArgs s{m, w.ldv, w.ldz2, splits, mt, V, w.Zp, Tk, w.Z, w.Gp, w.S, w.counter};
-        he2hb_slab_kernel<<<mt, 128, kSmemSlab, st>>>(s);
+        int gsplit = (m + 255) / 256; if (gsplit > kGramSplitMax) gsplit = kGramSplitMax;
+        const int gchunk = (((m + gsplit - 1) / gsplit) + 15) & ~15;
+        gsplit = (m + gchunk - 1) / gchunk;
+        SlabArgs s{m, w.ldv, w.ldz2, splits, gsplit, V, w.Zp, Tk, w.Z, w.Gp, w.S, w.counter};
+        he2hb_zsum_kernel<<<(m * kBW + 255) / 256, 256, 0, st>>>(s);
+        HPSD_LAUNCH_CHECK();
+        he2hb_gram_kernel<<<gsplit, GR_WM * GR_WN * 32, kSmemGram, st>>>(s, gchunk);
+        HPSD_LAUNCH_CHECK();
+        he2hb_s_kernel<<<1, kBW * kBW, 0, st>>>(s);
         HPSD_LAUNCH_CHECK();
         XArgs x{m, w.ldv, w.ldz2, w.Z, V, Tk, w.S, w.X};
         he2hb_x_kernel<<<mt, HM_THREADS, kSmemHemm, st>>>(x);
