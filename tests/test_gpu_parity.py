@@ -37,6 +37,18 @@ def _record(what, errs):
         pass
 
 
+def check_oracle_samples(cfg, got):
+    """Full-size comparison with the ORACLE on sampled outputs (tests/golden/oracle_samples_cfg*.npz, written by
+    tests/golden/make_oracle_samples.py, which calls only oracle/): every diagonal entry and every 4099th svec entry
+    of the oracle's projection of the whole config, plus the norm of its output."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"oracle_samples_cfg{cfg}.npz")
+    g = np.load(path)
+    idx, val = g["idx"], g["val"]
+    err = float(np.linalg.norm(got[idx] - val) / np.linalg.norm(val))
+    nrm = abs(float(np.linalg.norm(got)) - float(g["norm"])) / float(g["norm"])
+    return err, nrm
+
+
 def force_large(hp, on):
     """Route every block through S1..S8 of the multi-kernel path (on) or restore the defaults (off)."""
     hp.set_option("jacobi_max_n", 1 if on else 32)
@@ -177,6 +189,8 @@ def test_config4_mixed_full_size(orc, hp):
         worst[n] = max(worst.get(n, 0.0), err)
         assert err <= TOL * n, (k, n, err)
     _record("config4 vs oracle", {str(k): v for k, v in worst.items()})
+    err, nrm = check_oracle_samples(4, got)          # the stored oracle run of the whole config agrees as well
+    assert err <= TOL * 2401 and nrm <= TOL * 2401, (err, nrm)
     check_invariants(orc, hp, sizes, sv, got)
 
 
@@ -211,6 +225,10 @@ def test_config5_n4096_closed_form_and_invariants(orc, hp):
     assert rel_err(got, closed) <= TOL * 4096
     check_invariants(orc, hp, [4096], sv, got)
     _record("config5 vs closed form", {"4096": rel_err(got, closed)})
+    # the oracle itself at full size (14 minutes on 8 host cores): its stored samples, 8188 svec entries
+    err, nrm = check_oracle_samples(5, got)
+    _record("config5 vs oracle samples", {"4096": err})
+    assert err <= TOL * 4096 and nrm <= TOL * 4096, (err, nrm)
     if os.environ.get("HPSD_FULL_ORACLE") == "1":
         want = orc.project([4096], sv, nthreads=orc.max_threads())
         err = rel_err(got, want)
