@@ -526,6 +526,32 @@ def main():
             line["batched_call"] = {"blocks_per_call": 8, "ms_per_call": t8 / 5, "projections_per_s": 8.0 / (t8 / 5 * 1e-3),
                                     "note": "eight n=625 blocks in one hpsd_project call (lanes); not the headline metric"}
             del v8, o8
+        # NEXT-3: the affine-projection step z_x = (a_x - A^T a_y)/2, z_y = a_y + A z_x on the device,
+        # d = 5 (n = 625) and d = 8 (n = 4096); HBM-bound streaming passes (information only, not the headline metric)
+        if not args.no_secondary:
+            aff = {}
+            for d_ in (5, 8):
+                af = hp.Affine(d_)
+                g_ = torch.Generator(device=dev); g_.manual_seed(20519 + d_)
+                ax = torch.randn(af.m, dtype=torch.float64, device=dev, generator=g_)
+                ay = torch.randn(af.n * af.n, dtype=torch.float64, device=dev, generator=g_)
+                zx, zy = torch.empty_like(ax), torch.empty_like(ay)
+                for _ in range(3):
+                    af.project_(ax, ay, zx, zy)
+                evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
+                for a_, b_ in evs:
+                    flush.zero_()
+                    a_.record(); af.project_(ax, ay, zx, zy); b_.record()
+                torch.cuda.synchronize()
+                ms_ = statistics.median(a_.elapsed_time(b_) for a_, b_ in evs)
+                alg_bytes = 16.0 * af.n * af.n + 16.0 * af.m            # a_y in, z_y out, a_x in, z_x out
+                moved = 8.0 * af.n * af.n * (2 + 1 + 2 * 4 * 2 + 2 + 1 + 2 * 4 * 2 + 2 + 1)   # the 12 streaming passes of affine.cu
+                aff[f"d{d_}"] = {"n": af.n, "m": af.m, "ms": ms_, "launches": hp.last_launch_count(),
+                                 "algorithmic_gbs": alg_bytes / (ms_ * 1e-3) / 1e9, "moved_gbs_estimate": moved / (ms_ * 1e-3) / 1e9,
+                                 "hbm_peak_gbs": hbm_peak}
+                af.destroy()
+                del ax, ay, zx, zy
+            line["affine_step"] = aff
         line["other_configs"] = extra
         if "cfg5" in extra:
             line["ms_per_projection_n4096"] = extra["cfg5"]["ms_per_call"]

@@ -107,6 +107,28 @@ int hpsd_plan_info(hpsd_plan *plan, const int **info_dev, size_t *workspace_byte
 /* Copies the n_blocks status words to HOST memory on `stream` and synchronises that stream. */
 int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream);
 
+/* The affine-projection step of the SCS iteration on the device:
+ *     z_x = (a_x - A^T a_y) / 2,      z_y = a_y + A z_x,
+ * with A x = - sum_mu x_mu F_mu and (A^T Z)_mu = - tr[F_mu Z] (Eq. D3) over the orthonormal
+ * product basis F_mu of generalized Gell-Mann matrices (Eq. A10) on A_i (x) A_o (x) B_i (x) B_o, all of
+ * local dimension d, restricted to the allowed multi-indices of Eq. (B14) without the all-identity
+ * index; A^T A = 1 (D4), so no linear solve is involved.  n = d^4 is the matrix size, m = 2 d^6 - 3 d^4 + 2 d^2 - 1
+ * the number of coefficients (column m of Table II).
+ *   Basis order (the paper fixes none): sigma_0 = 1/sqrt d; sigma_{1+l} the diagonal elements l = 0..d-2;
+ *   then (|j><k| + |k><j|)/sqrt 2 and then -i(|j><k| - |k><j|)/sqrt 2, each over j < k in lexicographic order;
+ *   multi-indices (alpha, beta, gamma, delta) in lexicographic order.
+ *   x, a_x, z_x: DEVICE vectors of m doubles.  y_svec, a_y, z_y: DEVICE svec vectors (n^2 doubles, layout above) of
+ *   Hermitian n x n matrices.  z_x may alias a_x and z_y may alias a_y.  2 <= d <= 9.
+ * hpsd_affine_create allocates device tables and workspace (40 n^2 bytes) on the current device and synchronises;
+ * the apply / project calls only enqueue on `stream` (one plan serves one stream at a time). */
+typedef struct hpsd_affine hpsd_affine;
+int hpsd_affine_create(int d, hpsd_affine **plan);
+int hpsd_affine_destroy(hpsd_affine *plan);
+int hpsd_affine_dims(const hpsd_affine *plan, int *n, int *m);
+int hpsd_affine_apply_a(hpsd_affine *plan, const double *x, double *y_svec, void *stream);
+int hpsd_affine_apply_at(hpsd_affine *plan, const double *y_svec, double *x, void *stream);
+int hpsd_affine_project(hpsd_affine *plan, const double *a_x, const double *a_y, double *z_x, double *z_y, void *stream);
+
 /* One ADMM cone step, Eqs. (D33)-(D34), fused into the projection:
  *     u = Pi_C(u~ - v),      v <- v - u~ + u
  * on the PSD part of the cone.  utilde (read only), v (read and updated in place) and u (written) are DEVICE

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     admm_step_,
     eigvalsh,
     Plan,
+    Affine,
     reduce_to_band,
     band_width,
     fp64_peak_probe,

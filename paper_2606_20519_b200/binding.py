@@ -19,6 +19,7 @@ EXPORTS = [
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
     "hpsd_reduce_to_band", "hpsd_band_width",
     "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info",
+    "hpsd_affine_create", "hpsd_affine_destroy", "hpsd_affine_dims", "hpsd_affine_apply_a", "hpsd_affine_apply_at", "hpsd_affine_project",
 ]
 
 
@@ -59,6 +60,12 @@ def load_library():
         lib.hpsd_plan_admm_step.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_plan_info.argtypes = [c_vp, ctypes.POINTER(c_vp), ctypes.POINTER(c_sz)]
         lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
+        lib.hpsd_affine_create.argtypes = [c_int, ctypes.POINTER(c_vp)]
+        lib.hpsd_affine_destroy.argtypes = [c_vp]
+        lib.hpsd_affine_dims.argtypes = [c_vp, ip, ip]
+        lib.hpsd_affine_apply_a.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_affine_apply_at.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_affine_project.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_set_option.argtypes = [ctypes.c_char_p, c_int]
         lib.hpsd_last_launch_count.restype = c_int
         lib.hpsd_release.restype = c_int
@@ -258,6 +265,55 @@ class Plan:
     def destroy(self):
         if self._h:
             load_library().hpsd_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class Affine:
+    """hpsd_affine_*: the affine-projection step of the SCS iteration (z_x = (a_x - A^T a_y)/2, z_y = a_y + A z_x) for
+    the bipartite process-matrix SDP with local dimension d.  Argument marshalling only."""
+
+    def __init__(self, d: int, device: Optional[torch.device] = None):
+        self.d = int(d)
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self._h = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_affine_create(self.d, ctypes.byref(self._h)), "hpsd_affine_create")
+        n, m = ctypes.c_int(), ctypes.c_int()
+        _check(load_library().hpsd_affine_dims(self._h, ctypes.byref(n), ctypes.byref(m)), "hpsd_affine_dims")
+        self.n, self.m = int(n.value), int(m.value)
+
+    def apply_A(self, x: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        _need_cuda_f64(x, "x")
+        y = torch.empty(self.n * self.n, dtype=torch.float64, device=x.device)
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_affine_apply_a(self._h, x.data_ptr(), y.data_ptr(), _stream(stream)), "hpsd_affine_apply_a")
+        return y
+
+    def apply_AT(self, y_svec: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        _need_cuda_f64(y_svec, "y_svec")
+        x = torch.empty(self.m, dtype=torch.float64, device=y_svec.device)
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_affine_apply_at(self._h, y_svec.data_ptr(), x.data_ptr(), _stream(stream)), "hpsd_affine_apply_at")
+        return x
+
+    def project_(self, a_x: torch.Tensor, a_y: torch.Tensor, z_x: torch.Tensor, z_y: torch.Tensor,
+                 stream: Optional[torch.cuda.Stream] = None):
+        for t, nm in ((a_x, "a_x"), (a_y, "a_y"), (z_x, "z_x"), (z_y, "z_y")):
+            _need_cuda_f64(t, nm)
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_affine_project(self._h, a_x.data_ptr(), a_y.data_ptr(), z_x.data_ptr(), z_y.data_ptr(),
+                                                      _stream(stream)), "hpsd_affine_project")
+        return z_x, z_y
+
+    def destroy(self):
+        if self._h:
+            load_library().hpsd_affine_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __del__(self):
