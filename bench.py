@@ -103,8 +103,8 @@ def measured_hbm_gbs():
 # captures of THIS round's kernels (profiles/r2_ncu_full.md lists kernel, workload, command and both counters);
 # None where no capture exists for that kernel and workload
 NCU_TRAFFIC = {
-    ("tridiag_cluster_kernel", 3): {"bytes_per_launch": 3.17e6, "source": "profiles/r2_ncu_full.md (n=625, whole reduction in one launch)"},
-    ("tridiag_panel_kernel", 5): {"bytes_per_launch": None, "source": "profiles/r2_ncu_full.md"},
+    ("tridiag_cluster_kernel", 3): {"bytes_per_launch": 3.18e6, "source": "profiles/r2_ncu_full.md (n=625, whole reduction in one launch)"},
+    ("tridiag_panel_kernel", 5): {"bytes_per_launch": 2.019e9, "source": "profiles/r2_ncu_full.md (first panel of n=4096: 1913 MB read + 106 MB written; algorithmic 2.1 GB)"},
 }
 
 
@@ -545,7 +545,7 @@ def main():
                 torch.cuda.synchronize()
                 ms_ = statistics.median(a_.elapsed_time(b_) for a_, b_ in evs)
                 alg_bytes = 16.0 * af.n * af.n + 16.0 * af.m            # a_y in, z_y out, a_x in, z_x out
-                moved = 8.0 * af.n * af.n * (2 + 1 + 2 * 4 * 2 + 2 + 1 + 2 * 4 * 2 + 2 + 1)   # the 12 streaming passes of affine.cu
+                moved = 312.0 * af.n * af.n     # the 12 streaming passes of affine.cu: 24 + 4 x 32 (A^T), 8 + 24 + 3 x 32 + 32 (A) bytes per n^2
                 aff[f"d{d_}"] = {"n": af.n, "m": af.m, "ms": ms_, "launches": hp.last_launch_count(),
                                  "algorithmic_gbs": alg_bytes / (ms_ * 1e-3) / 1e9, "moved_gbs_estimate": moved / (ms_ * 1e-3) / 1e9,
                                  "hbm_peak_gbs": hbm_peak}
