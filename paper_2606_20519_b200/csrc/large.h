@@ -6,6 +6,7 @@
 namespace hpsd {
 
 constexpr int kNB = 32;       // tridiagonalisation panel width
+constexpr int kMaxPanelCtas = 192;   // the cooperative panel kernel runs min(SM count, this) CTAs; sizes its per-CTA partial arrays
 
 // ---- tridiag.cu ---------------------------------------------------------------
 struct TridiagWs {

@@ -48,7 +48,7 @@ LargeWs carve(int n, unsigned char *base) {
     const int N = (int)align_up((size_t)n, 8);
     const int ts = tridiag_tile_size(n);
     const int nblk = (n + ts - 1) / ts;
-    const int G = g_sms > 0 ? g_sms : 148;
+    const int G = kMaxPanelCtas;          // an upper bound, NOT the SM count of the device at hand: the size must not depend on whether init has run
     // ---- S2/S3
     w.t.n = n; w.t.lda = N; w.t.ldw = N; w.t.ldp = nblk * ts;
     w.t.A = cpx((size_t)N * n);

@@ -634,7 +634,7 @@ int stedc_init() {
     int dev = 0;
     cudaGetDevice(&dev);
     if (g_stedc_init_dev == dev) return 0;
-    if (cudaFuncSetAttribute(stedc_merge_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 * kMaxLargeN) != cudaSuccess) return HPSD_ECUDA_;
+    if (cudaFuncSetAttribute(stedc_merge_setup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 24 * (kMaxLargeN + 1))   /* the top merge asks for 24 (n + 1) bytes */ != cudaSuccess) return HPSD_ECUDA_;
     if (cudaFuncSetAttribute(stedc_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStedcGemmSmem) != cudaSuccess) return HPSD_ECUDA_;
     g_stedc_init_dev = dev;
     return 0;

@@ -699,7 +699,7 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int ts = tridiag_tile_size(n);
     PanelArgs p;
-    p.n = n; p.lda = w.lda; p.ldw = w.ldw; p.nblk = (n + ts - 1) / ts; p.G = sms;
+    p.n = n; p.lda = w.lda; p.ldw = w.ldw; p.nblk = (n + ts - 1) / ts; p.G = sms < kMaxPanelCtas ? sms : kMaxPanelCtas;
     if (p.G < 2 * kNB) return HPSD_ECUDA_;   // the reducers of phase A need 64 CTAs
     p.A = w.A; p.W = w.W; p.d = w.d; p.e = w.e; p.tau = w.tau;
     p.ldp = w.ldp; p.PR = w.PR; p.PC = w.PC; p.part = w.part; p.tot = w.tot; p.qpart = w.qpart; p.tiles = w.tiles;
