@@ -129,6 +129,17 @@ int hpsd_affine_apply_a(hpsd_affine *plan, const double *x, double *y_svec, void
 int hpsd_affine_apply_at(hpsd_affine *plan, const double *y_svec, double *x, void *stream);
 int hpsd_affine_project(hpsd_affine *plan, const double *a_x, const double *a_y, double *z_x, double *z_y, void *stream);
 
+/* Factorisation-free APPROXIMATE projection of ONE Hermitian block ("a
+ * composite matrix polynomial constructed solely from matrix-matrix products").  The paper's optimised coefficients
+ * are in its ref. [81], which this build does not have; the composite polynomial used is the `iterations`-fold
+ * composition of the Newton-Schulz cubic g(t) = (3t - t^3)/2 on X / ||X||_F:
+ *     S_0 = X / ||X||_F,   S_{k+1} = (3 S_k - S_k^3) / 2,   out = vec_R((X + X S_K) / 2),
+ * i.e. the filter lambda -> lambda (1 + g^K(lambda/||X||_F)) / 2 on the spectrum; the Frobenius error against the exact
+ * projection is 1/2 || lambda (1 - |g^K(lambda/||X||_F)|) ||_2 and tends to 0 as K grows (K ~ 1.7 log2(||X||_F / |lambda|) + 6
+ * settles an eigenvalue lambda).  2 K + 1 complex n^3 GEMMs on the FP64 tensor pipe; no eigensolver.
+ *   in_svec, out_svec: DEVICE svec of n^2 doubles (may alias); library workspace (64 n^2 bytes); enqueue-only. */
+int hpsd_project_approx(int n, const double *in_svec, double *out_svec, int iterations, void *stream);
+
 /* One ADMM cone step, Eqs. (D33)-(D34), fused into the projection:
  *     u = Pi_C(u~ - v),      v <- v - u~ + u
  * on the PSD part of the cone.  utilde (read only), v (read and updated in place) and u (written) are DEVICE

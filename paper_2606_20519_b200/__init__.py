@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     eigvalsh,
     Plan,
     Affine,
+    project_approx,
     reduce_to_band,
     band_width,
     fp64_peak_probe,

@@ -19,6 +19,7 @@ EXPORTS = [
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
     "hpsd_reduce_to_band", "hpsd_band_width",
     "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info",
+    "hpsd_project_approx",
     "hpsd_affine_create", "hpsd_affine_destroy", "hpsd_affine_dims", "hpsd_affine_apply_a", "hpsd_affine_apply_at", "hpsd_affine_project",
 ]
 
@@ -60,6 +61,7 @@ def load_library():
         lib.hpsd_plan_admm_step.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_plan_info.argtypes = [c_vp, ctypes.POINTER(c_vp), ctypes.POINTER(c_sz)]
         lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
+        lib.hpsd_project_approx.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
         lib.hpsd_affine_create.argtypes = [c_int, ctypes.POINTER(c_vp)]
         lib.hpsd_affine_destroy.argtypes = [c_vp]
         lib.hpsd_affine_dims.argtypes = [c_vp, ip, ip]
@@ -272,6 +274,17 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+def project_approx(svec: torch.Tensor, n: int, iterations: int, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_project_approx: composite-polynomial approximate projection of one block (NEXT-4)."""
+    _need_cuda_f64(svec, "svec")
+    if svec.numel() != n * n:
+        raise HpsdError("svec length != n^2")
+    out = torch.empty_like(svec)
+    with torch.cuda.device(svec.device):
+        _check(load_library().hpsd_project_approx(n, svec.data_ptr(), out.data_ptr(), int(iterations), _stream(stream)), "hpsd_project_approx")
+    return out
 
 
 class Affine:

@@ -16,6 +16,7 @@
 #include "largepath.h"
 #include "prof.h"
 #include "twostage.h"
+#include "approx.h"
 
 namespace hpsd {
 
@@ -810,6 +811,23 @@ int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream) {
     cudaStream_t st = (cudaStream_t)stream;
     if (cudaMemcpyAsync(info_host, plan->ws, nb * sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return HPSD_ECUDA;
     return cudaStreamSynchronize(st) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
+}
+
+int hpsd_project_approx(int n, const double *in_svec, double *out_svec, int iterations, void *stream) {
+    if (n < 0 || n > kMaxLargeN || iterations < 0 || iterations > 1000 || (n > 0 && (!in_svec || !out_svec))) return HPSD_EINVAL;
+    g_launches = 0;
+    if (n == 0) return HPSD_OK;
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HPSD_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    std::lock_guard<std::recursive_mutex> lk(g_mu);
+    DeviceState &ds = g_dev[dev];
+    void *ws; size_t bytes;
+    int rc = library_workspace(ds, approx_ws_bytes(n), st, &ws, &bytes);
+    if (rc) return rc;
+    rc = launch_project_approx(n, in_svec, out_svec, iterations, reinterpret_cast<unsigned char *>(ws), st);
+    const int rc2 = mark_user(ds.ws_event, ds.ws_stream, ds.ws_busy, st);
+    return rc ? rc : rc2;
 }
 
 int hpsd_band_width(void) { return kBW; }

@@ -82,3 +82,32 @@ def test_affine_identities_at_larger_d(orc, hp, d):
         assert rel_err(af.apply_A(af.apply_AT(w)).cpu().numpy(), w.cpu().numpy()) <= TOL * n
     finally:
         af.destroy()
+
+
+# ------------------------------------------------------------------ NEXT-4: approximate projection
+
+@pytest.mark.parametrize("n,K", [(2, 10), (40, 0), (40, 12), (100, 30), (257, 25), (625, 30)])
+def test_approximate_projection_against_oracle(orc, hp, n, K):
+    """hpsd_project_approx against oracle/approx.py (same K, same polynomial) to 1e-12 n, against the exact projection
+    within the error identity 1/2 ||lam (1 - |g^K(lam/s)|)||, and the in-place call."""
+    import torch
+    from oracle import approx
+    rng = np.random.default_rng(870 + n)
+    lam = np.concatenate([rng.uniform(0.5, 2.0, min(4, n)), rng.normal(0, 1e-2, max(n - 4, 0))])
+    g = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    q, _ = np.linalg.qr(g)
+    X = (q * lam[None, :]) @ q.conj().T
+    X = 0.5 * (X + X.conj().T)
+    sv = orc.pack(X)
+    t = torch.from_numpy(sv).cuda()
+    got = hp.project_approx(t, n, K).cpu().numpy()
+    want = orc.pack(approx.project_approx(X, K))
+    assert rel_err(got, want, denom=np.linalg.norm(sv)) <= TOL * n
+    exact = orc.pack((q * np.maximum(lam, 0)[None, :]) @ q.conj().T)
+    s = np.linalg.norm(sv)
+    bound = 0.5 * np.linalg.norm(lam * (1.0 - np.abs(approx.scalar_filter(lam / s, K))))
+    assert abs(np.linalg.norm(got - exact) - bound) <= 10 * TOL * n * s
+    import ctypes
+    rc = hp.load_library().hpsd_project_approx(n, t.data_ptr(), t.data_ptr(), K, None)
+    torch.cuda.synchronize()
+    assert rc == 0 and np.array_equal(t.cpu().numpy(), got)
