@@ -552,6 +552,26 @@ def main():
                 af.destroy()
                 del ax, ay, zx, zy
             line["affine_step"] = aff
+        # host cost of one call through the explicit plan handle: config 1 (one n = 16 block), enqueue only,
+        # no synchronisation inside the loop; the plan replays its CUDA graph from the third call on
+        if not args.no_secondary:
+            s1, v1 = device_inputs(1)
+            o1 = torch.empty_like(v1)
+            pl1 = hp.Plan(s1)
+            for _ in range(5):
+                pl1.project_(v1, o1)
+            torch.cuda.synchronize()
+            reps = 2000
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                pl1.project_(v1, o1)
+            t_enq = (time.perf_counter() - t0) / reps
+            torch.cuda.synchronize()
+            t_all = (time.perf_counter() - t0) / reps
+            pl1.destroy()
+            line["plan_host_overhead"] = {"workload": "cfg1 (1 x n=16) through hpsd_plan_project via the ctypes binding",
+                                          "enqueue_us_per_call": t_enq * 1e6, "us_per_call_back_to_back": t_all * 1e6,
+                                          "note": "enqueue time includes the Python/ctypes marshalling of the binding"}
         line["other_configs"] = extra
         if "cfg5" in extra:
             line["ms_per_projection_n4096"] = extra["cfg5"]["ms_per_call"]

@@ -359,26 +359,32 @@ __global__ void __launch_bounds__(GR_WM *GR_WN * 32) he2hb_gram_kernel(SlabArgs 
 // own: the partials come from other CTAs, and reading them inside the slab kernel needs gpu-scope loads
 // (LDG.STRONG.GPU, ~170 issue cycles each: 80 us per panel, measured); across a launch boundary plain loads do.
 __global__ void __launch_bounds__(kBW * kBW) he2hb_s_kernel(SlabArgs s) {
-    __shared__ cplx sG[kBW][kBW], sT[kBW][kBW], sM[kBW][kBW];        // 48 KB
-    const int e = threadIdx.x, r = e % kBW, c = e / kBW;
-    cplx g = mk(0.0, 0.0);
-    for (int k0 = 0; k0 < s.nslabs; k0 += 8) {          // eight independent loads per round trip, fixed summation order
-        cplx gp[8];
+    __shared__ cplx sG[kBW][kBW], sT[kBW][kBW], sM[kBW][kBW];        // 48 KB, [row][col]
+    // thread = (r, c) with c fastest: in the products below the left operand is a broadcast and the right one a
+    // conflict-free row; the (column-major) global reads are coalesced and transposed on their way into shared memory
+    const int e = threadIdx.x;
+    {
+        const int gr = e % kBW, gc = e / kBW;              // element e of a column-major b x b matrix
+        cplx g = mk(0.0, 0.0);
+        for (int k0 = 0; k0 < s.nslabs; k0 += 8) {          // eight independent loads per round trip, fixed summation order
+            cplx gp[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) gp[k] = (k0 + k < s.nslabs) ? s.Gp[(size_t)(k0 + k) * kBW * kBW + e] : mk(0.0, 0.0);
+            for (int k = 0; k < 8; ++k) gp[k] = (k0 + k < s.nslabs) ? s.Gp[(size_t)(k0 + k) * kBW * kBW + e] : mk(0.0, 0.0);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) g = g + gp[k];
+            for (int k = 0; k < 8; ++k) g = g + gp[k];
+        }
+        sG[gr][gc] = g;
+        sT[gr][gc] = s.Tk[e];
     }
-    sG[r][c] = g;
-    sT[r][c] = s.Tk[e];
     __syncthreads();
+    const int r = e / kBW, c = e % kBW;
     cplx acc = mk(0.0, 0.0);
     for (int k = 0; k <= c; ++k) cfma(acc, sG[r][k], sT[k][c]);             // M = G T, T upper triangular
     sM[r][c] = acc;
     __syncthreads();
     acc = mk(0.0, 0.0);
     for (int k = 0; k <= r; ++k) cfma_conj(acc, sT[k][r], sM[k][c]);        // T^H M
-    s.S[e] = mk(-0.5 * acc.x, -0.5 * acc.y);
+    s.S[r + c * kBW] = mk(-0.5 * acc.x, -0.5 * acc.y);
 }
 
 struct XArgs {
@@ -473,6 +479,58 @@ int twostage_available() {
     return g_ts_ok;
 }
 
+// Look-ahead: the panel QR (one cluster, ~115 us, latency-bound) of panel k+1 runs on a side stream next to the bulk of panel
+// k's HER2K (all SMs, DMMA-bound): the HER2K is split into the first block column of the trailing matrix (all the next
+// panel reads) and the rest.  Fork/join with events, so the whole thing stays capturable in a CUDA graph.
+struct LookAhead {
+    cudaStream_t st = nullptr;
+    cudaEvent_t col = nullptr, qr = nullptr;
+    int dev = -1;
+};
+static thread_local LookAhead g_la;
+int g_he2hb_lookahead = 1;
+
+static bool lookahead_ready() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (g_la.st && g_la.dev == dev) return true;
+    if (g_la.st) { cudaStreamDestroy(g_la.st); cudaEventDestroy(g_la.col); cudaEventDestroy(g_la.qr); g_la = LookAhead(); }
+    if (cudaStreamCreateWithFlags(&g_la.st, cudaStreamNonBlocking) != cudaSuccess) { g_la = LookAhead(); cudaGetLastError(); return false; }
+    if (cudaEventCreateWithFlags(&g_la.col, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g_la.qr, cudaEventDisableTiming) != cudaSuccess) {
+        cudaStreamDestroy(g_la.st); g_la = LookAhead(); cudaGetLastError(); return false;
+    }
+    g_la.dev = dev;
+    return true;
+}
+
+static int launch_panel_qr(const TwoStageWs &w, int j0, int kp, cudaStream_t st) {
+    QrArgs a{w.n, w.lda, w.ldv, w.ldab, j0, w.A, w.V1, w.tau1, w.Tk + (size_t)kp * kBW * kBW, w.AB};
+    cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
+    qr_launch_cfg(cfg, at, st);
+    prof_begin(ST_PANEL, st);
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, he2hb_panel_kernel, a);
+    prof_end(ST_PANEL, st);
+    g_launches++;
+    return e == cudaSuccess ? 0 : HPSD_ECUDA_;
+}
+
+// C (lower tiles, mirrored) -= X V^H + V X^H  for the M x N leading part of the trailing matrix at C
+static int launch_her2k_part(const TwoStageWs &w, const cplx *X, const cplx *V, cplx *C, int M, int N, cudaStream_t st) {
+    GemmProblem<cplx, cplx> gp;
+    gp.A = X; gp.lda = w.ldz2; gp.B = V; gp.ldb = w.ldv;
+    gp.A2 = V; gp.lda2 = w.ldv; gp.B2 = X; gp.ldb2 = w.ldz2;
+    gp.M = M; gp.N = N; gp.K = kBW; gp.K2 = kBW;
+    Her2kFullEpi epi{C, w.lda};
+    if (M <= 1536 || N <= 32) {
+        he2hb_her2k_small_kernel<<<dim3((M + 31) / 32, (N + 31) / 32), H2F_WM * H2F_WN * 32, kSmemH2Fs, st>>>(gp, epi);
+    } else {
+        he2hb_her2k_kernel<<<dim3((M + 63) / 64, (N + 63) / 64), H2F_WM * H2F_WN * 32, kSmemH2F, st>>>(gp, epi);
+    }
+    HPSD_LAUNCH_CHECK();
+    return 0;
+}
+
 int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
     const int n = w.n;
     int rc = twostage_init();
@@ -485,7 +543,8 @@ int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
     HPSD_CUDA_OK(cudaMemsetAsync(w.V1, 0, sizeof(cplx) * (size_t)w.ldv * n, st));
     HPSD_CUDA_OK(cudaMemsetAsync(w.AB, 0, sizeof(cplx) * (size_t)w.ldab * n, st));
     HPSD_CUDA_OK(cudaMemsetAsync(w.tau1, 0, sizeof(cplx) * (size_t)n, st));
-    HPSD_CUDA_OK(cudaMemsetAsync(w.counter, 0, sizeof(unsigned), st));
+    const bool la = g_he2hb_lookahead && lookahead_ready();
+    bool qr_on_side = false;          // the QR of the current panel was launched on the side stream by the previous iteration
     int kp = 0;
     for (int j0 = 0; j0 < n; j0 += kBW, ++kp) {
         const int m = n - j0 - kBW;
@@ -494,19 +553,16 @@ int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
             HPSD_LAUNCH_CHECK();
             break;
         }
-        cplx *Tk = w.Tk + (size_t)kp * kBW * kBW;
+        const cplx *Tk = w.Tk + (size_t)kp * kBW * kBW;
         const cplx *V = w.V1 + (size_t)j0 * w.ldv + j0 + kBW;
         cplx *A22 = w.A + (size_t)(j0 + kBW) * w.lda + j0 + kBW;
-        prof_begin(ST_PANEL, st);
-        {
-            QrArgs a{n, w.lda, w.ldv, w.ldab, j0, w.A, w.V1, w.tau1, Tk, w.AB};
-            cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
-            qr_launch_cfg(cfg, at, st);
-            const cudaError_t e = cudaLaunchKernelEx(&cfg, he2hb_panel_kernel, a);
-            g_launches++;
-            if (e != cudaSuccess) return HPSD_ECUDA_;
+        if (qr_on_side) {
+            if (cudaStreamWaitEvent(st, g_la.qr, 0) != cudaSuccess) return HPSD_ECUDA_;      // join: V, T of this panel are ready
+        } else {
+            rc = launch_panel_qr(w, j0, kp, st);
+            if (rc) return rc;
         }
-        prof_end(ST_PANEL, st);
+        qr_on_side = false;
         prof_begin(ST_HER2K, st);
         const int mt = (m + 63) / 64;
         int splits = (2 * sms + mt - 1) / mt;
@@ -529,19 +585,24 @@ int launch_he2hb(const TwoStageWs &w, cudaStream_t st) {
         XArgs x{m, w.ldv, w.ldz2, w.Z, V, Tk, w.S, w.X};
         he2hb_x_kernel<<<mt, HM_THREADS, kSmemHemm, st>>>(x);
         HPSD_LAUNCH_CHECK();
-        GemmProblem<cplx, cplx> gp;
-        gp.A = w.X; gp.lda = w.ldz2; gp.B = V; gp.ldb = w.ldv;
-        gp.A2 = V; gp.lda2 = w.ldv; gp.B2 = w.X; gp.ldb2 = w.ldz2;
-        gp.M = m; gp.N = m; gp.K = kBW; gp.K2 = kBW;
-        Her2kFullEpi epi{A22, w.lda};
-        if (m <= 1536) {
-            const int nt = (m + 31) / 32;
-            he2hb_her2k_small_kernel<<<dim3(nt, nt), H2F_WM * H2F_WN * 32, kSmemH2Fs, st>>>(gp, epi);
+        const int m_next = m - kBW;               // rows of the next panel
+        if (la && m_next > 0 && m > 512) {
+            // first block column (all the next panel's QR reads), then fork the QR, then the rest of the trailing matrix
+            rc = launch_her2k_part(w, w.X, V, A22, m, kBW, st);
+            if (rc) return rc;
+            if (cudaEventRecord(g_la.col, st) != cudaSuccess || cudaStreamWaitEvent(g_la.st, g_la.col, 0) != cudaSuccess) return HPSD_ECUDA_;
+            rc = launch_panel_qr(w, j0 + kBW, kp + 1, g_la.st);
+            const bool rec = cudaEventRecord(g_la.qr, g_la.st) == cudaSuccess;
+            qr_on_side = true;
+            int rc2 = launch_her2k_part(w, w.X + kBW, V + kBW, A22 + (size_t)kBW * w.lda + kBW, m_next, m_next, st);
+            if (rc || !rec || rc2) {              // never leave a capture forked
+                cudaStreamWaitEvent(st, g_la.qr, 0);
+                return rc ? rc : (rc2 ? rc2 : HPSD_ECUDA_);
+            }
         } else {
-            const int nt = (m + 63) / 64;
-            he2hb_her2k_kernel<<<dim3(nt, nt), H2F_WM * H2F_WN * 32, kSmemH2F, st>>>(gp, epi);
+            rc = launch_her2k_part(w, w.X, V, A22, m, m, st);
+            if (rc) return rc;
         }
-        HPSD_LAUNCH_CHECK();
         prof_end(ST_HER2K, st);
     }
     return 0;

@@ -63,10 +63,11 @@ struct Options {
     int overlap_factors = 1;          // compact-WY factors of S5 on a side stream next to S4
     int two_stage = 0;                // 0 one-stage reduction, 1 two-stage for every large block, 2 two-stage from two_stage_min_n on
     int two_stage_min_n = 1024;
+    int two_stage_lookahead = 1;      // S2: QR of the next panel on a side stream next to the HER2K of the current one
     bool same_routing(const Options &o) const {
         return jacobi_max_n == o.jacobi_max_n && medium_max_n == o.medium_max_n && medium_dc == o.medium_dc && medium_reroute == o.medium_reroute &&
                large_lanes == o.large_lanes && cluster_tridiag == o.cluster_tridiag && overlap_factors == o.overlap_factors &&
-               two_stage == o.two_stage && two_stage_min_n == o.two_stage_min_n;
+               two_stage == o.two_stage && two_stage_min_n == o.two_stage_min_n && two_stage_lookahead == o.two_stage_lookahead;
     }
 } g_opt;
 
@@ -76,6 +77,7 @@ void apply_runtime_options(const Options &o) {
     g_overlap_factors = o.overlap_factors;
     g_two_stage = o.two_stage;
     g_two_stage_min_n = o.two_stage_min_n;
+    g_he2hb_lookahead = o.two_stage_lookahead;
 }
 bool takes_two_stage(const Options &o, int n) {
     if (n < kTwoStageMinN || n > kTwoStageMaxN) return false;
@@ -422,6 +424,10 @@ int hpsd_set_option(const char *name, int value) {
     if (std::strcmp(name, "two_stage") == 0) {
         if (value < 0 || value > 2) return HPSD_EINVAL;
         g_opt.two_stage = value;
+        return HPSD_OK;
+    }
+    if (std::strcmp(name, "two_stage_lookahead") == 0) {
+        g_opt.two_stage_lookahead = (value != 0);
         return HPSD_OK;
     }
     if (std::strcmp(name, "two_stage_min_n") == 0) {

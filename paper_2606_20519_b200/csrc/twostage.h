@@ -38,6 +38,7 @@ struct TwoStageWs {
     int *q2flags;        // (n / 32 slabs) x (sweep groups): pipeline flags of the Q2 kernel
 };
 
+extern int g_he2hb_lookahead;                 // option "two_stage_lookahead" (default 1): panel QR of panel k+1 next to panel k's HER2K
 int twostage_init();
 int twostage_available();                     // 1 when 16-CTA clusters with the panel kernel's shared memory can be launched
 size_t twostage_hops(int n);                  // max hops of a sweep = ceil((n - 1) / kBW)

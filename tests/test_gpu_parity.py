@@ -398,6 +398,32 @@ def test_two_stage_whole_path(orc, hp, n):
         force_large(hp, False)
 
 
+def test_two_stage_in_a_mixed_cone_list(orc, hp):
+    """Option two_stage = 2 (by size): in one call the blocks of at least two_stage_min_n rows take S2 + S3 + Q2, the
+    others keep their routes (Jacobi, medium, cluster kernel); every block against the oracle, and the fused ADMM step."""
+    import torch
+    rng = np.random.default_rng(777)
+    sizes = [150, 36, 260, 1, 16, 200]
+    mats = [herm(rng, n, 1 / np.sqrt(max(n, 1))) for n in sizes]
+    sv = pack_all(orc, mats)
+    hp.set_option("two_stage", 2)
+    hp.set_option("two_stage_min_n", 200)
+    try:
+        got, _ = check_vs_oracle(orc, hp, sizes, sv, nthreads=orc.max_threads())
+        check_invariants(orc, hp, sizes, sv, got)
+        v = pack_all(orc, [herm(rng, n, 0.1) for n in sizes])
+        want_u, want_v = orc.admm_step(sizes, sv, v, nthreads=orc.max_threads())
+        t_ut, t_v = torch.from_numpy(sv).cuda(), torch.from_numpy(v.copy()).cuda()
+        t_u = torch.empty_like(t_ut)
+        hp.admm_step_(sizes, t_ut, t_v, t_u)
+        torch.cuda.synchronize()
+        assert rel_err(t_u.cpu().numpy(), want_u) <= TOL * max(sizes)
+        assert rel_err(t_v.cpu().numpy(), want_v) <= TOL * max(sizes)
+    finally:
+        hp.set_option("two_stage", 0)
+        hp.set_option("two_stage_min_n", 1024)
+
+
 @pytest.mark.parametrize("n", [150, 300])
 def test_two_stage_degenerate_inputs(orc, hp, n):
     """Edge cases of the method on the two-stage route: already banded / tridiagonal / diagonal input (every
