@@ -568,10 +568,12 @@ def main():
             t_enq = (time.perf_counter() - t0) / reps
             torch.cuda.synchronize()
             t_all = (time.perf_counter() - t0) / reps
+            c_us = pl1.host_overhead_us(v1, o1, 2000)
             pl1.destroy()
-            line["plan_host_overhead"] = {"workload": "cfg1 (1 x n=16) through hpsd_plan_project via the ctypes binding",
-                                          "enqueue_us_per_call": t_enq * 1e6, "us_per_call_back_to_back": t_all * 1e6,
-                                          "note": "enqueue time includes the Python/ctypes marshalling of the binding"}
+            line["plan_host_overhead"] = {"workload": "cfg1 (1 x n=16), hpsd_plan_project, CUDA graph warm, enqueue only",
+                                          "c_abi_enqueue_us_per_call": c_us,
+                                          "python_binding_enqueue_us_per_call": t_enq * 1e6, "python_us_per_call_back_to_back": t_all * 1e6,
+                                          "note": "c_abi figure: loop inside the library (hpsd_plan_host_overhead); the Python figure adds ctypes/torch marshalling"}
         line["other_configs"] = extra
         if "cfg5" in extra:
             line["ms_per_projection_n4096"] = extra["cfg5"]["ms_per_call"]

@@ -106,6 +106,9 @@ int hpsd_plan_admm_step(hpsd_plan *plan, const double *utilde, double *v, double
 int hpsd_plan_info(hpsd_plan *plan, const int **info_dev, size_t *workspace_bytes);
 /* Copies the n_blocks status words to HOST memory on `stream` and synchronises that stream. */
 int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream);
+/* Measurement aid: HOST microseconds per hpsd_plan_project call, averaged over `reps` back-to-back calls on `stream`
+ * (enqueue only, the stream is synchronised before and after the loop; the plan's CUDA graph is warm). */
+int hpsd_plan_host_overhead(hpsd_plan *plan, const double *in_svec, double *out_svec, int reps, void *stream, double *enqueue_us);
 
 /* The affine-projection step of the SCS iteration on the device:
  *     z_x = (a_x - A^T a_y) / 2,      z_y = a_y + A z_x,

@@ -18,7 +18,7 @@ EXPORTS = [
     "hpsd_set_option", "hpsd_last_launch_count", "hpsd_release", "hpsd_fp64_peak_probe",
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
     "hpsd_reduce_to_band", "hpsd_band_width",
-    "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info",
+    "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info", "hpsd_plan_host_overhead",
     "hpsd_project_approx",
     "hpsd_affine_create", "hpsd_affine_destroy", "hpsd_affine_dims", "hpsd_affine_apply_a", "hpsd_affine_apply_at", "hpsd_affine_project",
 ]
@@ -61,6 +61,7 @@ def load_library():
         lib.hpsd_plan_admm_step.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_plan_info.argtypes = [c_vp, ctypes.POINTER(c_vp), ctypes.POINTER(c_sz)]
         lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
+        lib.hpsd_plan_host_overhead.argtypes = [c_vp, c_vp, c_vp, c_int, c_vp, ctypes.POINTER(ctypes.c_double)]
         lib.hpsd_project_approx.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
         lib.hpsd_affine_create.argtypes = [c_int, ctypes.POINTER(c_vp)]
         lib.hpsd_affine_destroy.argtypes = [c_vp]
@@ -258,6 +259,15 @@ class Plan:
         with torch.cuda.device(self.device):
             _check(load_library().hpsd_plan_read_info(self._h, host, _stream(stream)), "hpsd_plan_read_info")
         return [int(host[i]) for i in range(nb)]
+
+    def host_overhead_us(self, in_svec: torch.Tensor, out_svec: torch.Tensor, reps: int = 1000,
+                         stream: Optional[torch.cuda.Stream] = None) -> float:
+        """hpsd_plan_host_overhead: host microseconds per hpsd_plan_project call, measured inside the library."""
+        us = ctypes.c_double()
+        with torch.cuda.device(self.device):
+            _check(load_library().hpsd_plan_host_overhead(self._h, in_svec.data_ptr(), out_svec.data_ptr(), int(reps), _stream(stream),
+                                                          ctypes.byref(us)), "hpsd_plan_host_overhead")
+        return float(us.value)
 
     def workspace_bytes(self) -> int:
         ptr, nbytes = ctypes.c_void_p(), ctypes.c_size_t()

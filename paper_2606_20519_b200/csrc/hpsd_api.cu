@@ -1,6 +1,7 @@
 // hpsd_api.cu -- C ABI (include/hpsd.h), S0 plan/dispatch of SURVEY.md §8(a):
 // size class per block, svec offsets sum n_k^2, workspace carve-up, launches on the caller's stream.
 #include <cstdlib>
+#include <ctime>
 #include <cstring>
 #include <algorithm>
 #include <map>
@@ -801,6 +802,23 @@ int hpsd_plan_admm_step(hpsd_plan *plan, const double *utilde, double *v, double
     if (total > 0 && (!utilde || !v || !u)) return HPSD_EINVAL;
     const SvecIo io{utilde, v, u, v};
     return plan_execute(plan, io, stream);
+}
+
+int hpsd_plan_host_overhead(hpsd_plan *plan, const double *in_svec, double *out_svec, int reps, void *stream, double *enqueue_us) {
+    if (!plan || !plan->pl || reps < 1 || !enqueue_us) return HPSD_EINVAL;
+    // measurement aid (like hpsd_fp64_peak_probe): host time of `reps` back-to-back hpsd_plan_project calls, no synchronisation inside
+    int rc = hpsd_plan_project(plan, in_svec, out_svec, stream);          // warm: plain launches
+    if (!rc) rc = hpsd_plan_project(plan, in_svec, out_svec, stream);     // capture
+    if (!rc) rc = hpsd_plan_project(plan, in_svec, out_svec, stream);     // first replay
+    if (rc) return rc;
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return HPSD_ECUDA;
+    timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    for (int i = 0; i < reps && !rc; ++i) rc = hpsd_plan_project(plan, in_svec, out_svec, stream);
+    clock_gettime(CLOCK_MONOTONIC, &t1);
+    if (rc) return rc;
+    *enqueue_us = ((t1.tv_sec - t0.tv_sec) * 1e9 + (t1.tv_nsec - t0.tv_nsec)) / 1e3 / reps;
+    return cudaStreamSynchronize((cudaStream_t)stream) == cudaSuccess ? HPSD_OK : HPSD_ECUDA;
 }
 
 int hpsd_plan_info(hpsd_plan *plan, const int **info_dev, size_t *workspace_bytes) {
