@@ -54,6 +54,7 @@ extern "C" {
 #define HPSD_EWORKSPACE -2   /* caller workspace too small or misaligned (256 B) */
 #define HPSD_ECUDA      -3   /* a CUDA runtime call or kernel launch failed */
 #define HPSD_EALLOC     -4   /* device or host allocation failed */
+#define HPSD_ETOOLARGE  -5   /* hpsd_project_static: n or count beyond the fixed capacity of the static scratch */
 
 /* Library version: major*10000 + minor*100 + patch. */
 int hpsd_version(void);
@@ -109,6 +110,25 @@ int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream);
 /* Measurement aid: HOST microseconds per hpsd_plan_project call, averaged over `reps` back-to-back calls on `stream`
  * (enqueue only, the stream is synchronised before and after the loop; the plan's CUDA graph is warm). */
 int hpsd_plan_host_overhead(hpsd_plan *plan, const double *in_svec, double *out_svec, int reps, void *stream, double *enqueue_us);
+
+/* Allocation-free exact projection (same operation and svec layout as hpsd_project) of `count` blocks of
+ * ONE size n, stored back to back: block i at in_svec + i n^2.  For callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it): the call makes no cudaMalloc / cudaFree and calls no
+ * allocating library routine, on the first call or any later one.  Its scratch is a fixed array of
+ * HPSD_STATIC_SCRATCH_BYTES in the library's device image, held by every GPU that loads the library until exit.
+ *   limits     2 <= n <= HPSD_STATIC_MAX_N and 0 <= count <= HPSD_STATIC_MAX_COUNT; beyond either: HPSD_ETOOLARGE,
+ *              nothing enqueued.  n < 2, count < 0, NULL svec with count > 0: HPSD_EINVAL.
+ *   in_svec    DEVICE, count n^2 doubles, read only.   out_svec  DEVICE, same size, may alias in_svec.
+ *   info_dev   DEVICE, count ints, or NULL: per-block status as in hpsd_project_ws (0 ok, 2 non-finite input -> NaN block).
+ *   stream     enqueue-only on this stream; no synchronisation.
+ * Every call shares the one array and finds the previous call's contents there; what must start at zero is cleared by
+ * each call on `stream`.  Two calls that overlap on the GPU (different streams without an event between them) RACE on
+ * the array: serialise them.  The result equals hpsd_project's to rounding (the route is the batched divide-and-conquer
+ * medium path for every n here, where hpsd_project takes the Jacobi kernel for n <= 32). */
+#define HPSD_STATIC_MAX_N          83
+#define HPSD_STATIC_MAX_COUNT      16
+#define HPSD_STATIC_SCRATCH_BYTES  (6u << 20)
+int hpsd_project_static(int n, int count, const double *in_svec, double *out_svec, int *info_dev, void *stream);
 
 /* The affine-projection step of the SCS iteration on the device:
  *     z_x = (a_x - A^T a_y) / 2,      z_y = a_y + A z_x,

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     Plan,
     Affine,
     project_approx,
+    project_static_,
     reduce_to_band,
     band_width,
     fp64_peak_probe,

@@ -19,7 +19,7 @@ EXPORTS = [
     "hpsd_profile_stage_count", "hpsd_profile_stage_name", "hpsd_profile_read", "hpsd_admm_step",
     "hpsd_reduce_to_band", "hpsd_band_width",
     "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info", "hpsd_plan_host_overhead",
-    "hpsd_project_approx",
+    "hpsd_project_approx", "hpsd_project_static",
     "hpsd_affine_create", "hpsd_affine_destroy", "hpsd_affine_dims", "hpsd_affine_apply_a", "hpsd_affine_apply_at", "hpsd_affine_project",
 ]
 
@@ -63,6 +63,7 @@ def load_library():
         lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
         lib.hpsd_plan_host_overhead.argtypes = [c_vp, c_vp, c_vp, c_int, c_vp, ctypes.POINTER(ctypes.c_double)]
         lib.hpsd_project_approx.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
+        lib.hpsd_project_static.argtypes = [c_int, c_int, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_affine_create.argtypes = [c_int, ctypes.POINTER(c_vp)]
         lib.hpsd_affine_destroy.argtypes = [c_vp]
         lib.hpsd_affine_dims.argtypes = [c_vp, ip, ip]
@@ -295,6 +296,25 @@ def project_approx(svec: torch.Tensor, n: int, iterations: int, stream: Optional
     with torch.cuda.device(svec.device):
         _check(load_library().hpsd_project_approx(n, svec.data_ptr(), out.data_ptr(), int(iterations), _stream(stream)), "hpsd_project_approx")
     return out
+
+
+def project_static_(n: int, count: int, in_svec: torch.Tensor, out_svec: torch.Tensor, info: Optional[torch.Tensor] = None,
+                    stream: Optional[torch.cuda.Stream] = None) -> None:
+    """hpsd_project_static: allocation-free exact projection of `count` blocks of one size n (n <= 83, count <= 16) on the
+    library's fixed device scratch.  The caller passes input and output (and optionally an int32 status tensor); nothing is
+    allocated here or in the library.  Calls that overlap on the GPU race on the scratch: keep them on one stream."""
+    _need_cuda_f64(in_svec, "in_svec")
+    _need_cuda_f64(out_svec, "out_svec")
+    if in_svec.numel() != count * n * n or out_svec.numel() != count * n * n:
+        raise HpsdError("svec length != count * n^2")
+    ip = 0
+    if info is not None:
+        if not (info.is_cuda and info.dtype == torch.int32 and info.is_contiguous() and info.numel() >= count):
+            raise HpsdError("info must be a contiguous CUDA int32 tensor of count entries")
+        ip = info.data_ptr()
+    with torch.cuda.device(in_svec.device):
+        _check(load_library().hpsd_project_static(int(n), int(count), in_svec.data_ptr(), out_svec.data_ptr(), ip, _stream(stream)),
+               "hpsd_project_static")
 
 
 class Affine:

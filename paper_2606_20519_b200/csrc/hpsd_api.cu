@@ -381,6 +381,7 @@ const char *hpsd_strerror(int code) {
         case HPSD_EWORKSPACE: return "workspace too small or misaligned";
         case HPSD_ECUDA: return "CUDA runtime or launch failure";
         case HPSD_EALLOC: return "allocation failed";
+        case HPSD_ETOOLARGE: return "size beyond the fixed capacity of the static scratch (hpsd_project_static: n <= 83, count <= 16)";
         default: return "unknown error";
     }
 }
