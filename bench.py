@@ -585,6 +585,19 @@ def main():
                                           "note": "enqueue figures: bursts of 16 calls with an untimed synchronisation in between (a full launch queue would "
                                                   "show the GPU's time per call); c_abi: loop inside the library (hpsd_plan_host_overhead); the Python "
                                                   "figure adds ctypes/torch marshalling; throughput: 2000 calls back to back including the final synchronise"}
+        # NEXT-1: the same projection on complex64 STORAGE (FP32 svecs in HBM, FP64 arithmetic): configs 3 and 2
+        if not args.no_secondary:
+            c64 = {}
+            for c in (3, 2):
+                sc, vc = device_inputs(c)
+                v32 = vc.float()
+                o32 = torch.empty_like(v32)
+                tot, _ = time_device(sc, v32, o32, 10, 3)
+                c64["cfg%d" % c] = {"ms_per_call": tot / 10, "svec_bytes_per_call": 2 * 4 * int(v32.numel())}
+                del v32, o32, vc
+            c64["note"] = ("hpsd_project_c64: FP32 svecs, every load widened and every store rounded, the FP64 kernels in between; "
+                           "FP32 arithmetic is not built (DESIGN.md section 10)")
+            line["c64_storage"] = c64
         line["other_configs"] = extra
         if "cfg5" in extra:
             line["ms_per_projection_n4096"] = extra["cfg5"]["ms_per_call"]

@@ -111,6 +111,23 @@ int hpsd_plan_read_info(hpsd_plan *plan, int *info_host, void *stream);
  * (enqueue only, the stream is synchronised before and after the loop; the plan's CUDA graph is warm). */
 int hpsd_plan_host_overhead(hpsd_plan *plan, const double *in_svec, double *out_svec, int reps, void *stream, double *enqueue_us);
 
+/* complex64 STORAGE ("a fixed number of initial iterations is performed in single
+ * precision", complex64 column of Table III).  The same operations as hpsd_project, hpsd_admm_step,
+ * hpsd_plan_project and hpsd_plan_admm_step on svecs stored as FP32: same layout (n^2 floats per block, sqrt(2)-scaled
+ * lower triangle), DEVICE pointers, same aliasing rules, same plans, routes and options, same NaN contract.  Every load
+ * widens to FP64, the path in between is the FP64 one, every store rounds to nearest FP32: the result is the FP32 rounding
+ * of the FP64 projection of the FP32 input, i.e. at least as accurate as a complex64 eigensolver (relative error 2^-24 per
+ * entry against n 2^-24 norm-wise), at the FP64 path's speed with half the svec traffic; FP32 ARITHMETIC is not built
+ * (DESIGN.md §10).  The single -> double switch of PAPER.md:1544 is the caller's: run the first iterations through the
+ * _c64 calls, widen the iterate once (hpsd_svec_convert), continue with the FP64 calls on the same plan. */
+int hpsd_project_c64(int n_blocks, const int *sizes, const float *in_svec, float *out_svec, void *stream);
+int hpsd_admm_step_c64(int n_blocks, const int *sizes, const float *utilde, float *v, float *u, void *stream);
+int hpsd_plan_project_c64(hpsd_plan *plan, const float *in_svec, float *out_svec, void *stream);
+int hpsd_plan_admm_step_c64(hpsd_plan *plan, const float *utilde, float *v, float *u, void *stream);
+/* dst[i] = src[i] for count svec entries between the two storage types (to_f32 != 0: double -> float, else float ->
+ * double); DEVICE pointers, no overlap, enqueue-only. */
+int hpsd_svec_convert(size_t count, const void *src, void *dst, int to_f32, void *stream);
+
 /* Allocation-free exact projection (same operation and svec layout as hpsd_project) of `count` blocks of
  * ONE size n, stored back to back: block i at in_svec + i n^2.  For callers that cannot call cudaMalloc (code under CUDA
  * graph capture, tight serving loops, harnesses that forbid it): the call makes no cudaMalloc / cudaFree and calls no

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     Affine,
     project_approx,
     project_static_,
+    svec_convert,
     reduce_to_band,
     band_width,
     fp64_peak_probe,

@@ -20,6 +20,7 @@ EXPORTS = [
     "hpsd_reduce_to_band", "hpsd_band_width",
     "hpsd_plan_create", "hpsd_plan_destroy", "hpsd_plan_project", "hpsd_plan_admm_step", "hpsd_plan_info", "hpsd_plan_read_info", "hpsd_plan_host_overhead",
     "hpsd_project_approx", "hpsd_project_static",
+    "hpsd_project_c64", "hpsd_admm_step_c64", "hpsd_plan_project_c64", "hpsd_plan_admm_step_c64", "hpsd_svec_convert",
     "hpsd_affine_create", "hpsd_affine_destroy", "hpsd_affine_dims", "hpsd_affine_apply_a", "hpsd_affine_apply_at", "hpsd_affine_project",
 ]
 
@@ -63,6 +64,11 @@ def load_library():
         lib.hpsd_plan_read_info.argtypes = [c_vp, ip, c_vp]
         lib.hpsd_plan_host_overhead.argtypes = [c_vp, c_vp, c_vp, c_int, c_vp, ctypes.POINTER(ctypes.c_double)]
         lib.hpsd_project_approx.argtypes = [c_int, c_vp, c_vp, c_int, c_vp]
+        lib.hpsd_project_c64.argtypes = [c_int, ip, c_vp, c_vp, c_vp]
+        lib.hpsd_admm_step_c64.argtypes = [c_int, ip, c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_plan_project_c64.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_plan_admm_step_c64.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        lib.hpsd_svec_convert.argtypes = [c_sz, c_vp, c_vp, c_int, c_vp]
         lib.hpsd_project_static.argtypes = [c_int, c_int, c_vp, c_vp, c_vp, c_vp]
         lib.hpsd_affine_create.argtypes = [c_int, ctypes.POINTER(c_vp)]
         lib.hpsd_affine_destroy.argtypes = [c_vp]
@@ -100,6 +106,17 @@ def _stream(stream: Optional[torch.cuda.Stream]) -> int:
     return int(s.cuda_stream)
 
 
+def _svec_suffix(*named) -> str:
+    """"" for float64 svecs, "_c64" for float32 ones (complex64 storage, NEXT-1); all tensors of a call share the dtype."""
+    dt = named[0][0].dtype
+    if dt not in (torch.float64, torch.float32):
+        raise HpsdError(f"{named[0][1]} must be a CUDA float64 (or float32: complex64 storage) tensor")
+    for t, name in named:
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise HpsdError(f"{name} must be a contiguous CUDA {dt} tensor")
+    return "" if dt == torch.float64 else "_c64"
+
+
 def _need_cuda_f64(t: torch.Tensor, name: str):
     if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
         raise HpsdError(f"{name} must be a contiguous CUDA float64 tensor")
@@ -129,14 +146,13 @@ def project_(sizes: Sequence[int], in_svec: torch.Tensor, out_svec: torch.Tensor
              stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     """hpsd_project: enqueue the projection of a cone list on `stream`; out may alias in."""
     lib = load_library()
-    _need_cuda_f64(in_svec, "in_svec")
-    _need_cuda_f64(out_svec, "out_svec")
+    sfx = _svec_suffix((in_svec, "in_svec"), (out_svec, "out_svec"))
     total = svec_len(sizes)
     if in_svec.numel() != total or out_svec.numel() != total:
         raise HpsdError(f"svec length {in_svec.numel()}/{out_svec.numel()} != sum n^2 = {total}")
     arr, nb = _sizes(sizes)
     with torch.cuda.device(in_svec.device):
-        _check(lib.hpsd_project(nb, arr, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)), "hpsd_project")
+        _check(getattr(lib, "hpsd_project" + sfx)(nb, arr, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)), "hpsd_project" + sfx)
     return out_svec
 
 
@@ -148,14 +164,13 @@ def admm_step_(sizes: Sequence[int], utilde: torch.Tensor, v: torch.Tensor, u: t
                stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     """hpsd_admm_step: u = Pi_C(utilde - v), v <- v - utilde + u (v updated in place); returns u."""
     lib = load_library()
-    for t, name in ((utilde, "utilde"), (v, "v"), (u, "u")):
-        _need_cuda_f64(t, name)
+    sfx = _svec_suffix((utilde, "utilde"), (v, "v"), (u, "u"))
     total = svec_len(sizes)
     if utilde.numel() != total or v.numel() != total or u.numel() != total:
         raise HpsdError(f"svec lengths != sum n^2 = {total}")
     arr, nb = _sizes(sizes)
     with torch.cuda.device(utilde.device):
-        _check(lib.hpsd_admm_step(nb, arr, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)), "hpsd_admm_step")
+        _check(getattr(lib, "hpsd_admm_step" + sfx)(nb, arr, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)), "hpsd_admm_step" + sfx)
     return u
 
 
@@ -241,16 +256,17 @@ class Plan:
             _check(load_library().hpsd_plan_create(nb, arr, ctypes.byref(self._h)), "hpsd_plan_create")
 
     def project_(self, in_svec: torch.Tensor, out_svec: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
-        _need_cuda_f64(in_svec, "in_svec"); _need_cuda_f64(out_svec, "out_svec")
+        sfx = _svec_suffix((in_svec, "in_svec"), (out_svec, "out_svec"))
         with torch.cuda.device(self.device):
-            _check(load_library().hpsd_plan_project(self._h, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)), "hpsd_plan_project")
+            _check(getattr(load_library(), "hpsd_plan_project" + sfx)(self._h, in_svec.data_ptr(), out_svec.data_ptr(), _stream(stream)),
+                   "hpsd_plan_project" + sfx)
         return out_svec
 
     def admm_step_(self, utilde: torch.Tensor, v: torch.Tensor, u: torch.Tensor, stream: Optional[torch.cuda.Stream] = None):
-        for t, nm in ((utilde, "utilde"), (v, "v"), (u, "u")):
-            _need_cuda_f64(t, nm)
+        sfx = _svec_suffix((utilde, "utilde"), (v, "v"), (u, "u"))
         with torch.cuda.device(self.device):
-            _check(load_library().hpsd_plan_admm_step(self._h, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)), "hpsd_plan_admm_step")
+            _check(getattr(load_library(), "hpsd_plan_admm_step" + sfx)(self._h, utilde.data_ptr(), v.data_ptr(), u.data_ptr(), _stream(stream)),
+                   "hpsd_plan_admm_step" + sfx)
         return u, v
 
     def info(self, stream: Optional[torch.cuda.Stream] = None):
@@ -296,6 +312,17 @@ def project_approx(svec: torch.Tensor, n: int, iterations: int, stream: Optional
     with torch.cuda.device(svec.device):
         _check(load_library().hpsd_project_approx(n, svec.data_ptr(), out.data_ptr(), int(iterations), _stream(stream)), "hpsd_project_approx")
     return out
+
+
+def svec_convert(src: torch.Tensor, dtype: torch.dtype, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hpsd_svec_convert: an svec between float64 and float32 storage (the single -> double switch of PAPER.md:1544)."""
+    if not (src.is_cuda and src.is_contiguous() and {src.dtype, dtype} == {torch.float32, torch.float64}):
+        raise HpsdError("svec_convert: contiguous CUDA tensor, float32 <-> float64")
+    dst = torch.empty(src.shape, dtype=dtype, device=src.device)
+    with torch.cuda.device(src.device):
+        _check(load_library().hpsd_svec_convert(src.numel(), src.data_ptr(), dst.data_ptr(), 1 if dtype == torch.float32 else 0,
+                                                _stream(stream)), "hpsd_svec_convert")
+    return dst
 
 
 def project_static_(n: int, count: int, in_svec: torch.Tensor, out_svec: torch.Tensor, info: Optional[torch.Tensor] = None,

@@ -50,29 +50,45 @@ __host__ __device__ __forceinline__ size_t svec_col_off(int n, int j) { return (
 // svec input/output of one call.  Plain projection: x = in, out = P(x).  ADMM step, Eqs. (D33)-(D34)
 // (PAPER.md:1466-1472): x = in - sub with in = u~ and sub = v;  out = u = P(x);  vout = sub - in + u.
 // vout may alias sub, out may alias in: every element is read before it is written, by the same thread.
+// Storage precision ("a fixed number of initial iterations is performed in single
+// precision"): with f32 = 1 every svec of the call is stored as FP32 (complex64 entries, 4 n^2 bytes per block); the pointers
+// below then address floats and must only be dereferenced through sv_ld / sv_st.  The arithmetic between load and store is
+// FP64 on every route.
 struct SvecIo {
     const double *in;
     const double *sub;     // nullptr for a plain projection
     double *out;
     double *vout;
+    int f32;
 };
+__device__ __forceinline__ double sv_ld(const double *p, size_t i, int f32) {
+    return f32 ? (double)reinterpret_cast<const float *>(p)[i] : p[i];
+}
+__device__ __forceinline__ void sv_st(double *p, size_t i, double v, int f32) {
+    if (f32) reinterpret_cast<float *>(p)[i] = (float)v;
+    else p[i] = v;
+}
 __device__ __forceinline__ double io_load(const SvecIo &io, size_t i) {
-    double x = io.in[i];
-    if (io.sub) x -= io.sub[i];
+    double x = sv_ld(io.in, i, io.f32);
+    if (io.sub) x -= sv_ld(io.sub, i, io.f32);
     return x;
 }
 __device__ __forceinline__ void io_store(const SvecIo &io, size_t i, double u) {
-    if (io.sub) io.vout[i] = (io.sub[i] - io.in[i]) + u;
-    io.out[i] = u;
+    if (io.sub) sv_st(io.vout, i, (sv_ld(io.sub, i, io.f32) - sv_ld(io.in, i, io.f32)) + u, io.f32);
+    sv_st(io.out, i, u, io.f32);
 }
 // all n^2 svec entries of one block <- NaN (and the ADMM v update with it), by nthreads threads
 __device__ __forceinline__ void io_fill_nan(const SvecIo &io, size_t base, int n, int tid, int nthreads) {
     for (size_t t = tid; t < (size_t)n * n; t += nthreads) io_store(io, base + t, nan_());
 }
+// element offset on a pointer that may address floats (never dereferenced as double in that case)
+template <class P> inline P sv_adv(P p, long long off, int f32) {
+    return f32 ? reinterpret_cast<P>(reinterpret_cast<uintptr_t>(p) + (uintptr_t)(off * 4)) : p + off;
+}
 inline SvecIo io_offset(const SvecIo &io, long long off) {
     SvecIo r = io;
-    r.in += off; r.out += off;
-    if (io.sub) { r.sub += off; r.vout += off; }
+    r.in = sv_adv(io.in, off, io.f32); r.out = sv_adv(io.out, off, io.f32);
+    if (io.sub) { r.sub = sv_adv(io.sub, off, io.f32); r.vout = sv_adv(io.vout, off, io.f32); }
     return r;
 }
 

@@ -103,6 +103,7 @@ struct LargeBlock { int n; long long off; int idx; int lane = -1; };   // lane >
 // n ~ 1000 the 20-170 dependent launches of a call are launch-latency-bound.  Keyed by every pointer of the call.
 struct GraphEntry {
     const void *in = nullptr, *sub = nullptr, *out = nullptr, *vout = nullptr, *ws = nullptr, *info = nullptr;
+    int f32 = 0;                        // storage precision of the svecs (part of the key)
     cudaGraphExec_t exec = nullptr;     // null until the second call with the same key
     int launches = 0;
     unsigned long long stamp = 0;
@@ -509,7 +510,7 @@ static int execute_plan(DeviceState &ds, Plan &plan, const SvecIo &io, void *ws,
     }
     GraphEntry *ge = nullptr;
     for (GraphEntry &g : pl->graphs)
-        if (g.in == io.in && g.sub == io.sub && g.out == io.out && g.vout == io.vout && g.ws == ws && g.info == info_dev) { ge = &g; break; }
+        if (g.in == io.in && g.sub == io.sub && g.out == io.out && g.vout == io.vout && g.ws == ws && g.info == info_dev && g.f32 == io.f32) { ge = &g; break; }
     if (ge && ge->exec) {
         ge->stamp = ++ds.stamp;
         g_launches = ge->launches;
@@ -524,7 +525,7 @@ static int execute_plan(DeviceState &ds, Plan &plan, const SvecIo &io, void *ws,
             pl->graphs.erase(pl->graphs.begin() + old);
         }
         GraphEntry g;
-        g.in = io.in; g.sub = io.sub; g.out = io.out; g.vout = io.vout; g.ws = ws; g.info = info_dev; g.stamp = ++ds.stamp;
+        g.in = io.in; g.sub = io.sub; g.out = io.out; g.vout = io.vout; g.ws = ws; g.info = info_dev; g.f32 = io.f32; g.stamp = ++ds.stamp;
         pl->graphs.push_back(g);
         return run_plan(ds, *pl, io, ws, info_dev, st);
     }
@@ -633,6 +634,26 @@ int hpsd_project(int n_blocks, const int *sizes, const double *in_svec, double *
     return project_io_lib(n_blocks, sizes, io, stream);
 }
 
+// ---- NEXT-1: complex64 STORAGE.  Same plans, same routes, same kernels: the svecs are FP32 in memory, every
+// load widens to FP64 and every store rounds to FP32 (SvecIo::f32), the arithmetic in between is the FP64 path.
+int hpsd_project_c64(int n_blocks, const int *sizes, const float *in_svec, float *out_svec, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, in_svec, out_svec, &total);
+    if (rc) return rc;
+    const SvecIo io{reinterpret_cast<const double *>(in_svec), nullptr, reinterpret_cast<double *>(out_svec), nullptr, 1};
+    return project_io_lib(n_blocks, sizes, io, stream);
+}
+
+int hpsd_admm_step_c64(int n_blocks, const int *sizes, const float *utilde, float *v, float *u, void *stream) {
+    size_t total;
+    int rc = check_args(n_blocks, sizes, utilde, u, &total);
+    if (rc) return rc;
+    if (total > 0 && v == nullptr) return HPSD_EINVAL;
+    const SvecIo io{reinterpret_cast<const double *>(utilde), reinterpret_cast<const double *>(v), reinterpret_cast<double *>(u),
+                    reinterpret_cast<double *>(v), 1};
+    return project_io_lib(n_blocks, sizes, io, stream);
+}
+
 int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, double *out_host, void *stream) {
     size_t total;
     int rc = check_args(n_blocks, sizes, in_host, out_host, &total);
@@ -663,6 +684,12 @@ int hpsd_project_host(int n_blocks, const int *sizes, const double *in_host, dou
     if (cudaMemcpyAsync(out_host, dout, total * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess) return HPSD_ECUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return HPSD_ECUDA;
     return HPSD_OK;
+}
+
+int hpsd_svec_convert(size_t count, const void *src, void *dst, int to_f32, void *stream) {
+    if (count > 0 && (!src || !dst)) return HPSD_EINVAL;
+    g_launches = 0;
+    return launch_svec_convert(count, src, dst, to_f32, (cudaStream_t)stream) ? HPSD_ECUDA : HPSD_OK;
 }
 
 int hpsd_pack(int n, const void *A, int lda, double *svec, void *stream) {
@@ -802,6 +829,25 @@ int hpsd_plan_admm_step(hpsd_plan *plan, const double *utilde, double *v, double
     for (int n : plan->pl->sizes) total += (size_t)n * n;
     if (total > 0 && (!utilde || !v || !u)) return HPSD_EINVAL;
     const SvecIo io{utilde, v, u, v};
+    return plan_execute(plan, io, stream);
+}
+
+int hpsd_plan_project_c64(hpsd_plan *plan, const float *in_svec, float *out_svec, void *stream) {
+    if (!plan || !plan->pl) return HPSD_EINVAL;
+    size_t total = 0;
+    for (int n : plan->pl->sizes) total += (size_t)n * n;
+    if (total > 0 && (!in_svec || !out_svec)) return HPSD_EINVAL;
+    const SvecIo io{reinterpret_cast<const double *>(in_svec), nullptr, reinterpret_cast<double *>(out_svec), nullptr, 1};
+    return plan_execute(plan, io, stream);
+}
+
+int hpsd_plan_admm_step_c64(hpsd_plan *plan, const float *utilde, float *v, float *u, void *stream) {
+    if (!plan || !plan->pl) return HPSD_EINVAL;
+    size_t total = 0;
+    for (int n : plan->pl->sizes) total += (size_t)n * n;
+    if (total > 0 && (!utilde || !v || !u)) return HPSD_EINVAL;
+    const SvecIo io{reinterpret_cast<const double *>(utilde), reinterpret_cast<const double *>(v), reinterpret_cast<double *>(u),
+                    reinterpret_cast<double *>(v), 1};
     return plan_execute(plan, io, stream);
 }
 

@@ -8,7 +8,8 @@ namespace hpsd {
 // svec -> column-major complex.  full=0: lower triangle incl. diagonal only.
 // sub != nullptr: unpack svec - sub (the ADMM argument u~ - v of Eq. D33)
 // nf != nullptr: non-finite entries are replaced by zero and *nf (device) is set to 1
-int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st, int *nf = nullptr);
+int launch_svec_convert(size_t count, const void *src, void *dst, int to_f32, cudaStream_t st);
+int launch_unpack(int n, const double *svec, const double *sub, cplx *A, int lda, int full, cudaStream_t st, int *nf = nullptr, int f32 = 0);
 int launch_pack(int n, const cplx *A, int lda, double *svec, cudaStream_t st);
 // n = 1 blocks: out = max(in, 0) for `count` scattered scalars
 int launch_clamp_scalars(int count, const long long *offs_dev, const SvecIo &io, cudaStream_t st);

@@ -33,7 +33,7 @@ extern int g_cluster_tridiag;            // option "cluster_tridiag" (default 1)
 int tridiag_cluster_init();
 int tridiag_cluster_size_ok(int n);      // device-independent part of the test below
 int tridiag_cluster_fits(int n);         // 1 when this device and this n are served by the cluster kernel
-int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf = nullptr);
+int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf = nullptr, int f32 = 0);
 
 
 // ---- stedc.cu (S4) ------------------------------------------------------------

@@ -137,24 +137,24 @@ bool side_ready(int slot) {
     return true;
 }
 
-int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, const double *sub, cudaStream_t st, bool two_stage) {
+int reduce_to_tridiagonal(LargeWs &w, int n, const double *in, const double *sub, cudaStream_t st, bool two_stage, int f32 = 0) {
     int *nf = w.b.cnt + 2;
     if (cudaMemsetAsync(w.b.cnt, 0, sizeof(int) * 8, st) != cudaSuccess) return HPSD_ECUDA_;
     if (two_stage) {
         if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
         prof_begin(ST_UNPACK, st);
-        int rc = launch_unpack(n, in, sub, w.t.A, w.t.lda, 1, st, nf);      // both triangles: the HEMM of S2 reads a plain full matrix
+        int rc = launch_unpack(n, in, sub, w.t.A, w.t.lda, 1, st, nf, f32);      // both triangles: the HEMM of S2 reads a plain full matrix
         prof_end(ST_UNPACK, st);
         if (rc) return rc;
         rc = launch_he2hb(w.q, st);
         if (rc) return rc;
         return launch_hb2st(w.q, st);
     }
-    if (g_cluster_tridiag && tridiag_cluster_fits(n)) return launch_tridiag_cluster(w.t, in, sub, st, nf);
+    if (g_cluster_tridiag && tridiag_cluster_fits(n)) return launch_tridiag_cluster(w.t, in, sub, st, nf, f32);
     if (cudaMemsetAsync(w.t.tau, 0, sizeof(cplx) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     if (cudaMemsetAsync(w.t.e, 0, sizeof(double) * (size_t)w.t.lda, st) != cudaSuccess) return HPSD_ECUDA_;
     prof_begin(ST_UNPACK, st);
-    int rc = launch_unpack(n, in, sub, w.t.A, w.t.lda, 0, st, nf);
+    int rc = launch_unpack(n, in, sub, w.t.A, w.t.lda, 0, st, nf, f32);
     prof_end(ST_UNPACK, st);
     if (rc) return rc;
     return launch_tridiag(w.t, st);
@@ -216,7 +216,7 @@ int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int
     w.b.info = info;
     const bool ts = use_two_stage(n);
     if (ts) { w.b.A = w.q.V1; w.b.tau = w.q.tau1; w.b.voff = kBW; }
-    int rc = reduce_to_tridiagonal(w, n, io.in, io.sub, st, ts);
+    int rc = reduce_to_tridiagonal(w, n, io.in, io.sub, st, ts, io.f32);
     if (rc) return rc;
     bool forked = false;
     if (g_overlap_factors && side_ready(slot) && cudaEventRecord(g_side.fork, st) == cudaSuccess &&

@@ -75,8 +75,7 @@ extern "C" int hpsd_project_static(int n, int count, const double *in_svec, doub
     g_launches++;
     if (cudaPeekAtLastError() != cudaSuccess) return HPSD_ECUDA;
     if (info_dev && cudaMemsetAsync(info_dev, 0, sizeof(int) * (size_t)count, st) != cudaSuccess) return HPSD_ECUDA;
-    SvecIo io;
-    io.in = in_svec; io.sub = nullptr; io.out = out_svec; io.vout = nullptr;
+    const SvecIo io{in_svec, nullptr, out_svec, nullptr, 0};
     rc = launch_meddc_project(n, count, offs, io, base + kStaticHead, info_dev, idx, st);
     return rc == 0 ? HPSD_OK : (rc == -1 ? HPSD_EINVAL : HPSD_ECUDA);
 }

@@ -92,6 +92,7 @@ struct ClusterArgs {
     double *d, *e;
     cplx *tau;
     int *nf;                       // device flag: non-finite input seen
+    int f32;                       // svec stored as FP32 (common.cuh)
 };
 
 __host__ __device__ inline int cl_ncols(int n, int r) { return r < n ? (n - r + kCl - 1) / kCl : 0; }
@@ -142,14 +143,14 @@ __device__ __forceinline__ void cl_householder(cplx alpha, double xnorm2, double
 
 // element (i, j), i >= j, of the input matrix from the svec (Eq. D10 inverted; same arithmetic as unpack_kernel)
 // non-finite entries are replaced by zero and *nf is set (common.cuh: the output block becomes NaN)
-__device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, const double *__restrict__ sub, int n, int i, int j, int *nf) {
+__device__ __forceinline__ cplx cl_load_svec(const double *__restrict__ sv, const double *__restrict__ sub, int n, int i, int j, int *nf, int f32) {
     const size_t o = svec_col_off(n, j);
     cplx v;
-    if (i == j) v = mk(sub ? sv[o] - sub[o] : sv[o], 0.0);
+    if (i == j) v = mk(sub ? sv_ld(sv, o, f32) - sv_ld(sub, o, f32) : sv_ld(sv, o, f32), 0.0);
     else {
         const size_t k = o + 1 + 2 * (size_t)(i - j - 1);
-        double re = sv[k], im = sv[k + 1];
-        if (sub) { re -= sub[k]; im -= sub[k + 1]; }
+        double re = sv_ld(sv, k, f32), im = sv_ld(sv, k + 1, f32);
+        if (sub) { re -= sv_ld(sub, k, f32); im -= sv_ld(sub, k + 1, f32); }
         v = mk(re / kSqrt2, im / kSqrt2);
     }
     if (nonfinite(v.x) || nonfinite(v.y)) { v = mk(0.0, 0.0); if (nf) *nf = 1; }
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
     for (int jl = wp; jl < nc; jl += kClWarps) {
         const int j = r + kCl * jl;
         cplx *col = stor + cl_col_off(n, r, jl);
-        for (int i = j + lane; i < n; i += 32) col[i - j] = cl_load_svec(p.in, p.sub, n, i, j, p.nf);
+        for (int i = j + lane; i < n; i += 32) col[i - j] = cl_load_svec(p.in, p.sub, n, i, j, p.nf, p.f32);
     }
     int row[kClR], dest[kClR], dslot[kClR];
     cplx v[kClR], w[kClR], u[kClR], z[kClR], raw[kClR];
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(kClThreads, 1) tridiag_cluster_kernel(ClusterA
         row[s] = 32 * cl_chunk(s, wp) + lane;
         dest[s] = row[s] / RS; dslot[s] = row[s] - dest[s] * RS;       // reducer CTA of the row and its slot there
         v[s] = w[s] = u[s] = z[s] = mk(0.0, 0.0);
-        raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0, p.nf) : mk(0.0, 0.0);
+        raw[s] = row[s] < n ? cl_load_svec(p.in, p.sub, n, row[s], 0, p.nf, p.f32) : mk(0.0, 0.0);
     }
     cplx wc = mk(0.0, 0.0);
     const unsigned mbar1 = (unsigned)__cvta_generic_to_shared(smem_raw + L.mbar), mbar2 = mbar1 + 8;
@@ -521,9 +522,9 @@ int tridiag_cluster_fits(int n) {
 }
 
 // S1 + S2 + S3 in one launch.  w.W (ldw x kNB) hosts the raw-column ring.
-int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf) {
+int launch_tridiag_cluster(const TridiagWs &w, const double *in, const double *sub, cudaStream_t st, int *nf, int f32) {
     ClusterArgs a;
-    a.n = w.n; a.lda = w.lda; a.in = in; a.sub = sub; a.A = w.A; a.raw = w.W; a.d = w.d; a.e = w.e; a.tau = w.tau; a.nf = nf;
+    a.n = w.n; a.lda = w.lda; a.in = in; a.sub = sub; a.A = w.A; a.raw = w.W; a.d = w.d; a.e = w.e; a.tau = w.tau; a.nf = nf; a.f32 = f32;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(kCl); cfg.blockDim = dim3(kClThreads); cfg.dynamicSmemBytes = cl_smem_max(w.n); cfg.stream = st;
     cudaLaunchAttribute at[1];
