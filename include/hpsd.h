@@ -245,6 +245,11 @@ int hpsd_eigvalsh(int n, const double *in_svec, double *lambda, void *stream);
  *   "large_lanes" (0/1, default 1): two or more blocks of one call whose reduction runs on a single 16-CTA cluster
  *       (sizes up to ~631) are processed next to each other on up to 8 internal lane streams, each with its own part of
  *       the workspace (hpsd_workspace_size accounts for it); fork and join are events on the caller's stream.
+ *   "panel_lanes" (0/1, default 1): two or more blocks of one call above the cluster limit (n <= 2600; they take the
+ *       grid-wide cooperative panel kernel, which is bound by per-column latency, not by throughput) are dealt to two
+ *       lanes: lane 1 runs on an internal stream with 64 CTAs, lane 0 on the caller's stream keeps every SM until its
+ *       remaining work equals lane 1's and then continues on the other SMs.  One more scratch area (accounted for by
+ *       hpsd_workspace_size); fork and join are events on the caller's stream.
  *   "medium_reroute" (0/1, default 1): a group of at most 32 blocks of one size in 84..116 (the in-CTA QL range), or of
  *       at most 4 blocks of one size in 64..83, goes through the large path (cluster-resident reduction, lanes) instead
  *       of the one-CTA medium kernels (5 and 1 blocks when "large_lanes" is off).

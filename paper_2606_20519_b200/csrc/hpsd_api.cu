@@ -3,6 +3,7 @@
 #include <cstdlib>
 #include <ctime>
 #include <cstring>
+#include <cmath>
 #include <algorithm>
 #include <map>
 #include <memory>
@@ -65,10 +66,12 @@ struct Options {
     int two_stage = 0;                // 0 one-stage reduction, 1 two-stage for every large block, 2 two-stage from two_stage_min_n on
     int two_stage_min_n = 1024;
     int two_stage_lookahead = 1;      // S2: QR of the next panel on a side stream next to the HER2K of the current one
+    int panel_lanes = 1;              // two or more blocks on the grid-wide panel kernel run on two disjoint sets of SMs
     bool same_routing(const Options &o) const {
         return jacobi_max_n == o.jacobi_max_n && medium_max_n == o.medium_max_n && medium_dc == o.medium_dc && medium_reroute == o.medium_reroute &&
                large_lanes == o.large_lanes && cluster_tridiag == o.cluster_tridiag && overlap_factors == o.overlap_factors &&
-               two_stage == o.two_stage && two_stage_min_n == o.two_stage_min_n && two_stage_lookahead == o.two_stage_lookahead;
+               two_stage == o.two_stage && two_stage_min_n == o.two_stage_min_n && two_stage_lookahead == o.two_stage_lookahead &&
+               panel_lanes == o.panel_lanes;
     }
 } g_opt;
 
@@ -97,7 +100,10 @@ struct JacobiGroup {
     size_t idx_index;   // index (in int units) of this group's info indices
 };
 
-struct LargeBlock { int n; long long off; int idx; int lane = -1; };   // lane >= 0: runs on that lane stream, next to other blocks
+constexpr int kPanelLaneMaxN = 2600;      // above this the panel kernel streams most of its tiles and wants every SM
+constexpr int kPanelLaneCtas = 64;        // CTAs of panel lane 1: the minimum of the panel kernel (its phase-A reducers)
+struct LargeBlock { int n; long long off; int idx; int lane = -1; int plane = -1; };   // lane >= 0: runs on that lane stream, next to other blocks
+                                                                                       // plane 0 / 1: panel lane (caller's stream / panel stream), capped CTA count
 
 // A projection replayed as a CUDA graph: ADMM calls the library with the same buffers every iteration, and below
 // n ~ 1000 the 20-170 dependent launches of a call are launch-latency-bound.  Keyed by every pointer of the call.
@@ -125,6 +131,8 @@ struct Plan {
     size_t ws_bytes = 0;               // scratch needed by the large path (max over large blocks) + info
     int n_lanes = 0;                   // blocks served by the cluster-resident reduction run on this many lane streams
     size_t base_ws = 0, lane_ws = 0;   // scratch of the sequential part | of ONE lane (lanes follow the sequential part)
+    bool panel_lanes = false;          // two panel lanes (LargeBlock::plane); the second lane's scratch follows the lanes
+    size_t panel_ws = 0;
     void drop_graphs() {
         for (GraphEntry &g : graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
         graphs.clear();
@@ -223,16 +231,49 @@ void route_plan(int n_blocks, const int *sizes, Plan &pl, int (*cluster_fits)(in
         int k = 0;
         for (auto &lb : pl.large) if (fits(lb.n)) lb.lane = (k++) % pl.n_lanes;
     }
-    size_t ws = 0, lane_ws = 0;
+    // Panel lanes.  The grid-wide panel kernel is bound by per-column latency (two grid barriers, L2 round trips), not by
+    // throughput: on 84 instead of 148 CTAs an n = 2401 projection takes 36.6 instead of 31.8 ms, on 64 CTAs n = 1296 takes 13.3
+    // instead of 12.3 (B200).  So when a call holds two or more such blocks they are dealt to two lanes (longest first, to
+    // the lane with less work), lane 0 on the caller's stream with (SMs - 64) CTAs, lane 1 on a library stream with 64 (the
+    // minimum of the panel kernel); both cooperative grids are co-resident, one CTA per SM.  Only when every sequential
+    // block is such a block (a full-width cooperative grid next to a capped one could not become resident until the other
+    // has finished), no cluster lanes are in use, the sizes are below the streaming-dominated regime and lane 1 gets at
+    // least a fifth of lane 0's work (cost model: columns x per-column time ~ n^2).
+    pl.panel_lanes = false;
+    if (g_opt.panel_lanes && pl.n_lanes == 0) {
+        std::vector<size_t> pb;
+        bool all = true;
+        for (size_t i = 0; i < pl.large.size(); ++i) {
+            const LargeBlock &lb = pl.large[i];
+            if (fits(lb.n)) continue;                           // one 16-CTA cluster on the caller's stream: fits beside lane 1
+            if (takes_two_stage(opt, lb.n) || lb.n > kPanelLaneMaxN) { all = false; break; }
+            pb.push_back(i);
+        }
+        if (all && pb.size() >= 2) {
+            std::sort(pb.begin(), pb.end(), [&](size_t a, size_t b) { return pl.large[a].n > pl.large[b].n; });
+            double c0 = 0.0, c1 = 0.0;
+            std::vector<int> pick(pb.size());
+            for (size_t k = 0; k < pb.size(); ++k) {
+                const double c = (double)pl.large[pb[k]].n * pl.large[pb[k]].n;
+                if (k == 0 || c0 <= c1) { pick[k] = 0; c0 += c; } else { pick[k] = 1; c1 += c; }
+            }
+            if (c1 >= 0.2 * c0) {
+                for (size_t k = 0; k < pb.size(); ++k) pl.large[pb[k]].plane = pick[k];
+                pl.panel_lanes = true;
+            }
+        }
+    }
+    size_t ws = 0, lane_ws = 0, panel_ws = 0;
     for (const JacobiGroup &g : pl.groups)
         if (g.dc) ws = std::max(ws, meddc_ws_bytes(g.n, g.count));
     for (auto &lb : pl.large) {
         const size_t w = align_up(largepath_ws_bytes(lb.n), 256);
         if (lb.lane >= 0) { if (w > lane_ws) lane_ws = w; }
+        else if (lb.plane == 1) { if (w > panel_ws) panel_ws = w; }
         else if (w > ws) ws = w;
     }
-    pl.base_ws = align_up(ws, 256); pl.lane_ws = lane_ws;
-    pl.ws_bytes = pl.base_ws + pl.n_lanes * pl.lane_ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
+    pl.base_ws = align_up(ws, 256); pl.lane_ws = lane_ws; pl.panel_ws = panel_ws;
+    pl.ws_bytes = pl.base_ws + pl.n_lanes * pl.lane_ws + pl.panel_ws + align_up((size_t)(n_blocks > 0 ? n_blocks : 1) * sizeof(int), 256);
 }
 
 size_t workspace_bound(int n_blocks, const int *sizes) {
@@ -353,13 +394,69 @@ int run_plan(DeviceState &ds, const Plan &pl, const SvecIo &io, void *ws, int *i
                                         info + lb.idx, ds.lane_stream[lb.lane], lb.lane);
         }
     }
+    // Panel lanes: lane 1 on the last library lane stream (cluster lanes are not in use then).  Lane 0 (the caller's stream)
+    // is enqueued first: while it has more work left than lane 1 holds in total it keeps every SM (full-width panels), and
+    // lane 1 starts behind an event recorded at the panel from which lane 0's estimated remaining time equals lane 1's
+    // (time model of one projection on the panel path, B200: T(n) = a n + b n^2 ms, and the same form for the work left at
+    // trailing size m); from there on lane 0 runs on (SMs - 64) CTAs.  The event is the fork of lane 1; joined below.
+    constexpr int kPL = kLargeLanes - 1;
+    int sms = 0;
+    if (pl.panel_lanes && !g_profile) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
+    }
+    const bool planes = pl.panel_lanes && !g_profile && sms >= 2 * kPanelLaneCtas && lanes_ready(ds, kLargeLanes);
+    unsigned char *panel_scratch = scratch + pl.base_ws + (size_t)pl.n_lanes * pl.lane_ws;
+    auto t_model = [](double m) { return 5.16e-3 * m + 3.35e-6 * m * m; };
+    double left0 = 0.0, total1 = 0.0;
+    if (planes)
+        for (const LargeBlock &lb : pl.large) { if (lb.plane == 0) left0 += t_model(lb.n); else if (lb.plane == 1) total1 += t_model(lb.n); }
+    const double target = 0.94 * total1;          // 1.08 / 1.15: the slow-downs of the two lanes on their share of the SMs
+    bool forked = false;
     for (const LargeBlock &lb : pl.large) {
         if (lanes && lb.lane >= 0) continue;
+        if (planes && lb.plane == 1) continue;
         // without lanes every block takes the sequential scratch (a lane block fits: base_ws or lane 0's area)
-        unsigned char *sc = (lb.lane >= 0 && pl.lane_ws > pl.base_ws) ? scratch + pl.base_ws : scratch;
-        rc = largepath_project(lb.n, io_offset(io, lb.off), sc, pl.tiles_dev.at(lb.n), info + lb.idx, st);
+        unsigned char *sc = (lb.lane >= 0 && pl.lane_ws > pl.base_ws) ? scratch + pl.base_ws : (lb.plane == 1 ? panel_scratch : scratch);
+        int ctas = 0, wide = 0;
+        cudaEvent_t ev = nullptr;
+        if (planes && lb.plane == 0) {
+            ctas = sms - kPanelLaneCtas;
+            if (!forked) {
+                const double after = left0 - t_model(lb.n);            // lane 0's work behind this block
+                if (after >= target) ctas = 0;                         // the whole block at full width, lane 1 starts later
+                else {
+                    // trailing size m at which  t_model(m) + after = target
+                    const double r = target - after, a = 5.16e-3, b = 3.35e-6;
+                    double m = (-a + std::sqrt(a * a + 4.0 * b * r)) / (2.0 * b);
+                    if (m > lb.n) m = lb.n;
+                    wide = (int)((lb.n - m) / kNB);
+                    ev = ds.lane_fork;
+                    forked = true;
+                }
+                left0 = after;
+            }
+        }
+        rc = largepath_project(lb.n, io_offset(io, lb.off), sc, pl.tiles_dev.at(lb.n), info + lb.idx, st, -1, ctas, wide, ev);
         if (rc) break;
     }
+    if (planes && !forked && !rc && cudaEventRecord(ds.lane_fork, st) == cudaSuccess) forked = true;     // lane 0 had no block to fork from
+    if (planes && forked && cudaStreamWaitEvent(ds.lane_stream[kPL], ds.lane_fork, 0) == cudaSuccess) {
+        for (const LargeBlock &lb : pl.large) {
+            if (lb.plane != 1 || rc_lane) continue;
+            rc_lane = largepath_project(lb.n, io_offset(io, lb.off), panel_scratch, pl.tiles_dev.at(lb.n), info + lb.idx, ds.lane_stream[kPL], kPL,
+                                        kPanelLaneCtas);
+        }
+        // always join: a capture must not be left forked
+        if (cudaEventRecord(ds.lane_join[kPL], ds.lane_stream[kPL]) != cudaSuccess || cudaStreamWaitEvent(st, ds.lane_join[kPL], 0) != cudaSuccess) rc_lane = HPSD_ECUDA;
+    } else if (planes) {
+        // no fork: lane 1's blocks on the caller's stream, after lane 0
+        for (const LargeBlock &lb : pl.large) {
+            if (lb.plane != 1 || rc || rc_lane) continue;
+            rc_lane = largepath_project(lb.n, io_offset(io, lb.off), panel_scratch, pl.tiles_dev.at(lb.n), info + lb.idx, st);
+        }
+    }
+
     if (lanes)                                           // always join: a capture must not be left forked
         for (int l = 0; l < pl.n_lanes; ++l)
             if (cudaEventRecord(ds.lane_join[l], ds.lane_stream[l]) != cudaSuccess || cudaStreamWaitEvent(st, ds.lane_join[l], 0) != cudaSuccess) rc_lane = HPSD_ECUDA;
@@ -391,6 +488,7 @@ int hpsd_set_option(const char *name, int value) {
     if (!name) return HPSD_EINVAL;
     std::lock_guard<std::recursive_mutex> lk(g_mu);
     // routing options are frozen into each plan (and its captured graphs): a change only selects a different plan
+    if (std::strcmp(name, "panel_lanes") == 0) { g_opt.panel_lanes = (value != 0); return HPSD_OK; }
     if (std::strcmp(name, "large_lanes") == 0) {
         g_opt.large_lanes = (value != 0);
         return HPSD_OK;

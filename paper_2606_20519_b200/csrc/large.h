@@ -20,6 +20,10 @@ struct TridiagWs {
     cplx *tot;      // 2 kNB
     double *qpart;  // G
     const int2 *tiles;
+    // panel lanes (hpsd_api.cu): from panel `wide_panels` on the cooperative kernel runs on max_ctas CTAs (0: never capped;
+    // the kernel needs >= 64); wide_done (may be null) is recorded on the stream after the last full-width panel
+    int max_ctas = 0, wide_panels = 0;
+    cudaEvent_t wide_done = nullptr;
 };
 int tridiag_init();
 int tridiag_tile_size(int n);

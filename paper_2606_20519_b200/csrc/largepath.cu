@@ -207,11 +207,13 @@ int largepath_eigvals(int n, const double *in, double *lambda, unsigned char *sc
     return 0;
 }
 
-int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st, int lane) {
+int largepath_project(int n, const SvecIo &io, unsigned char *scratch, const int2 *tiles, int *info, cudaStream_t st, int lane,
+                      int panel_ctas, int wide_panels, cudaEvent_t wide_done) {
     const int slot = (lane >= 0 && lane < kLargeLanes) ? lane + 1 : 0;
     Side &g_side = g_sides[slot];
     LargeWs w = carve(n, scratch);
     w.t.tiles = tiles;
+    w.t.max_ctas = panel_ctas; w.t.wide_panels = wide_panels; w.t.wide_done = wide_done;
     w.s.info = info;
     w.b.info = info;
     const bool ts = use_two_stage(n);

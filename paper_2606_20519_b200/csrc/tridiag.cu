@@ -712,7 +712,13 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
     if (n == 1) {
         // d[0] = Re A[0,0]; handled by a 1-column panel (sets d in the prologue)
     }
+    const int G_full = p.G;
+    const int G_cap = (w.max_ctas >= 2 * kNB && w.max_ctas < G_full) ? w.max_ctas : G_full;
+    if (w.wide_done && w.wide_panels <= 0 && cudaEventRecord(w.wide_done, st) != cudaSuccess) return HPSD_ECUDA_;
     for (int j0 = 0; j0 < n; j0 += kNB) {
+        // panel lanes: the first wide_panels panels on every SM, the rest next to the other lane's kernel
+        p.G = (j0 / kNB >= w.wide_panels) ? G_cap : G_full;
+        if (w.wide_done && w.wide_panels > 0 && j0 / kNB == w.wide_panels && cudaEventRecord(w.wide_done, st) != cudaSuccess) return HPSD_ECUDA_;
         p.j0 = j0;
         p.nbp = (n - j0 < kNB) ? (n - j0) : kNB;
         const int nbk = p.nblk - j0 / kTS;              // tile rows/columns of this panel's trailing matrix
@@ -749,6 +755,7 @@ int launch_tridiag(const TridiagWs &w, cudaStream_t st) {
             HPSD_LAUNCH_CHECK();
         }
     }
+    if (w.wide_done && w.wide_panels > 0 && (long long)w.wide_panels * kNB >= n && cudaEventRecord(w.wide_done, st) != cudaSuccess) return HPSD_ECUDA_;
     if (n > 1) {
         clean_v_kernel<<<dim3((n + 255) / 256, n), 256, 0, st>>>(n, w.A, w.lda);
         HPSD_LAUNCH_CHECK();

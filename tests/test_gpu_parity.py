@@ -821,6 +821,38 @@ def test_concurrent_lanes_of_cluster_sized_blocks(orc, hp):
     check_vs_oracle(orc, hp, sizes, sv, nthreads=orc.max_threads())
 
 
+def test_panel_lanes_of_blocks_above_the_cluster_limit(orc, hp):
+    """Option "panel_lanes" (default 1): two or more blocks that take the grid-wide cooperative panel kernel are dealt to two
+    lanes on disjoint sets of SMs (lane 1: 64 CTAs on a library stream, forked behind an event inside lane 0's reduction;
+    lane 0: the caller's stream, capped from that panel on).  The CTA count changes summation orders, so the result is
+    compared with the oracle (and with the sequential schedule to rounding), must be identical on every repetition
+    (plain launches, capture, graph replays) and must work through a caller-owned workspace."""
+    import torch
+    rng = np.random.default_rng(99)
+    for sizes in ([700, 640], [800, 36, 650, 1, 900, 625], [1000, 700, 700, 660]):
+        sv = pack_all(orc, [herm(rng, n, 1.0 / np.sqrt(max(n, 1))) for n in sizes])
+        hp.set_option("panel_lanes", 0)
+        try:
+            base = gpu_project(hp, sizes, sv)
+        finally:
+            hp.set_option("panel_lanes", 1)
+        got, want = check_vs_oracle(orc, hp, sizes, sv, nthreads=orc.max_threads())
+        assert rel_err(got, base) <= 1e-13
+        t_in = torch.from_numpy(sv).cuda()
+        t_out = torch.empty_like(t_in)
+        for it in range(5):
+            t_out.zero_()
+            hp.project_(sizes, t_in, t_out)
+            assert np.array_equal(t_out.cpu().numpy(), got), (sizes, it)
+        ws = torch.empty(hp.workspace_size(sizes), dtype=torch.uint8, device="cuda")
+        info = torch.full((len(sizes),), -1, dtype=torch.int32, device="cuda")
+        t_out.zero_()
+        hp.project_ws(sizes, t_in, t_out, ws, info)
+        torch.cuda.synchronize()
+        assert info.cpu().tolist() == [0] * len(sizes)
+        assert np.array_equal(t_out.cpu().numpy(), got)
+
+
 def test_random_cone_lists(orc, hp):
     """Seeded random cone lists across every route (scalars, Jacobi, one-CTA medium kernels, re-routed medium blocks,
     cluster-sized blocks on lanes, panel-kernel blocks) and several matrix structures (dense, low-rank + noise, exact

@@ -95,8 +95,9 @@ def test_product_never_imports_oracle():
 
 def test_workspace_size_bounds_every_routing(lib):
     """hpsd_workspace_size is host-only and must bound every plan a device can make (include/hpsd.h, options
-    "large_lanes", "medium_reroute"): lanes add one scratch area per concurrently processed cluster-sized block (up to 8),
-    re-routed medium blocks need the large path's scratch, and switching the options off never needs more."""
+    "large_lanes", "panel_lanes", "medium_reroute"): lanes add one scratch area per concurrently processed cluster-sized
+    block (up to 8), two or more blocks above the cluster limit run on two panel lanes (two areas), re-routed medium blocks
+    need the large path's scratch, and switching the options off never needs more."""
     def ws(sizes):
         arr = (ctypes.c_int * len(sizes))(*sizes)
         sz = ctypes.c_size_t(0)
@@ -107,13 +108,22 @@ def test_workspace_size_bounds_every_routing(lib):
     assert ws([625, 625]) >= 2 * one - 4096                   # two lanes, two scratch areas
     assert ws([625] * 8) >= 8 * one - 8 * 4096
     assert ws([625] * 20) <= ws([625] * 8) + 4096             # at most 8 lanes
-    assert ws([700, 700]) < 2 * ws([700])                     # above the cluster limit: one after the other, one area
+    assert ws([700, 700]) <= 2 * ws([700])                    # above the cluster limit: two panel lanes, two areas
+    assert ws([700] * 5) <= ws([700, 700]) + 4096             # at most two panel lanes
+    assert ws([4096, 4096]) < 1.5 * ws([4096])                # too large for panel lanes: one after the other, one area
+    assert lib.hpsd_set_option(b"panel_lanes", 0) == 0
+    try:
+        assert ws([700, 700]) <= ws([700]) + 4096
+    finally:
+        assert lib.hpsd_set_option(b"panel_lanes", 1) == 0
     assert ws([100]) > 16 * 100 * 100                         # a single n = 100 block is re-routed to the large path
     assert lib.hpsd_set_option(b"large_lanes", 0) == 0
+    assert lib.hpsd_set_option(b"panel_lanes", 0) == 0
     try:
         assert ws([625] * 8) <= ws([625]) + 4096
     finally:
         assert lib.hpsd_set_option(b"large_lanes", 1) == 0
+        assert lib.hpsd_set_option(b"panel_lanes", 1) == 0
     assert lib.hpsd_set_option(b"medium_reroute", 0) == 0
     try:
         assert ws([100]) < 4096                               # the one-CTA kernel needs no scratch
