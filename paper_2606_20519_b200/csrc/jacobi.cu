@@ -117,12 +117,25 @@ __global__ void __launch_bounds__(THREADS) jacobi_project_kernel(int n, const lo
                 double c = 1.0, s = 0.0;
                 cplx e = mk(1.0, 0.0);
                 if (b2 > tol2) {
-                    const double ab = sqrt(b2);
-                    const double tau = (ga - al) / (2.0 * ab);
-                    const double t = copysign(1.0, tau) / (fabs(tau) + sqrt(1.0 + tau * tau));
-                    c = 1.0 / sqrt(1.0 + t * t);
+                    // the parameters of a rotation are one dependent chain that every round waits for: reciprocal square
+                    // roots (each refined by one Newton step to working precision) and one reciprocal instead of three DSQRT
+                    // and four DDIV (~300 instead of ~750 cycles)
+                    double iab = rsqrt(b2);
+                    iab = fma(0.5 * iab, fma(-b2 * iab, iab, 1.0), iab);          // 1 / |beta|
+                    const double tau = (ga - al) * (0.5 * iab);
+                    double t;
+                    if (fabs(tau) < 1e150) {
+                        const double x = fma(tau, tau, 1.0);
+                        double rx = rsqrt(x);
+                        rx = fma(0.5 * rx, fma(-x * rx, rx, 1.0), rx);
+                        t = copysign(__drcp_rn(fabs(tau) + x * rx), tau);          // sgn(tau) / (|tau| + sqrt(1 + tau^2))
+                    } else t = 0.5 / tau;                                          // tau^2 would overflow
+                    const double y = fma(t, t, 1.0);
+                    double ry = rsqrt(y);
+                    ry = fma(0.5 * ry, fma(-y * ry, ry, 1.0), ry);
+                    c = ry;
                     s = t * c;
-                    e = mk(be.x / ab, -be.y / ab);           // e^{-i phi}
+                    e = mk(be.x * iab, -be.y * iab);         // e^{-i phi}
                     active = 1;
                 }
                 sm.p[tid] = p; sm.q[tid] = q; sm.c[tid] = c; sm.s[tid] = s; sm.eph[tid] = e;
