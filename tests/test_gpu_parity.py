@@ -851,6 +851,22 @@ def test_panel_lanes_of_blocks_above_the_cluster_limit(orc, hp):
         torch.cuda.synchronize()
         assert info.cpu().tolist() == [0] * len(sizes)
         assert np.array_equal(t_out.cpu().numpy(), got)
+    # caller-side capture: lane 1 joins the capture through the fork event inside lane 0's reduction and is joined at the end
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    t_in2, t_out2 = t_in.clone(), torch.zeros_like(t_in)
+    with torch.cuda.stream(side):
+        hp.project_(sizes, t_in2, t_out2)
+    side.synchronize()
+    g = torch.cuda.CUDAGraph()
+    t_out2.zero_()
+    with torch.cuda.graph(g, stream=side):
+        hp.project_(sizes, t_in2, t_out2)
+    for _ in range(2):
+        t_out2.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(t_out2.cpu().numpy(), got)
 
 
 def test_random_cone_lists(orc, hp):
