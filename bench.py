@@ -486,6 +486,9 @@ def main():
                                 "frac_of_fp64_peak": r2["whole_path"]["frac_of_fp64_peak"],
                                 "dominant_stage": {k: r2[k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac", "share_of_step", "regime") if k in r2},
                                 "stages_ms": {k: round(x["ms_per_step"], 4) for k, x in st2.items()}}
+            if c == 4:
+                extra["cfg4"]["note"] = ("ms_per_call: the two large blocks run side by side (panel lanes); stages_ms / share_of_step: the "
+                                         "library's stage timers, which run the blocks one after the other on one stream")
             del o2
         # one-stage (cluster / panel kernel) against the two-stage reduction (S2 dense -> band, S3 bulge chasing, Q2) on
         # the paper's large sizes: the measurement the default route rests on
