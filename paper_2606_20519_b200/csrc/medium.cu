@@ -25,6 +25,7 @@ struct MedSmem {
     cplx *tau;          // n
     cplx *x;            // n : Householder vector / work row
     cplx *y;            // n : A v, then w
+    cplx *x2, *y2;      // n each: second parity of (v, w) in the fused tridiagonalisation
     double *d, *e;      // n each
     double *rc, *rs;    // kRing each
     int *ri;            // kRing : column index i of the rotation (acts on columns i, i+1)
@@ -36,7 +37,7 @@ __host__ __device__ inline int med_ld(int n) { return n | 1; }
 
 __host__ __device__ inline size_t med_smem_bytes(int n) {
     const size_t ld = med_ld(n);
-    return sizeof(cplx) * ((size_t)n * ld + 3 * (size_t)n) + sizeof(double) * (2 * (size_t)n + 2 * kRing + 32) +
+    return sizeof(cplx) * ((size_t)n * ld + 5 * (size_t)n) + sizeof(double) * (2 * (size_t)n + 2 * kRing + 32) +
            sizeof(int) * (kRing + 16) + 64;
 }
 
@@ -47,7 +48,9 @@ __device__ __forceinline__ MedSmem med_carve(unsigned char *base, int n) {
     sm.tau = sm.A + (size_t)n * ld;
     sm.x = sm.tau + n;
     sm.y = sm.x + n;
-    sm.d = reinterpret_cast<double *>(sm.y + n);
+    sm.x2 = sm.y + n;
+    sm.y2 = sm.x2 + n;
+    sm.d = reinterpret_cast<double *>(sm.y2 + n);
     sm.e = sm.d + n;
     sm.rc = sm.e + n;
     sm.rs = sm.rc + kRing;
@@ -99,18 +102,32 @@ __device__ __forceinline__ void med_householder(cplx alpha, double xnorm2, doubl
 }
 
 // ---- phase 1: A (full Hermitian, shared memory) -> real tridiagonal (d, e), reflectors in the lower part
+// One pass over the trailing block per column: the rank-2 update of step c-1 is applied to an element right before the
+// element is used in the mat-vec of step c (as in tridiag_cluster.cu), so the block is read once and written once per
+// column instead of read twice and written once, with four block barriers per column instead of five.  (v, w) of two
+// consecutive steps live in two parities of shared-memory vectors; column c itself is brought up to date on the fly.
 __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
     cplx *A = sm.A;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int r = tid; r < n; r += kMedThreads) { sm.x[r] = sm.y[r] = sm.x2[r] = sm.y2[r] = mk(0.0, 0.0); }
+    __syncthreads();
     for (int c = 0; c < n - 1; ++c) {
-        const int m = n - c - 1;
-        // norm of the sub-column, alpha and the diagonal entry travel through ONE block barrier (red[0..7] partial
-        // norms, red[16..18] alpha and d_c; the next writes to these slots are several barriers away)
-        double S = 0.0;
-        for (int r = c + 2 + tid; r < n; r += kMedThreads) S += abs2(A[(size_t)c * ld + r]);
+        cplx *X = (c & 1) ? sm.x2 : sm.x, *W = (c & 1) ? sm.y2 : sm.y;                  // v_c, w_c
+        const cplx *Vp = (c & 1) ? sm.x : sm.x2, *Wp = (c & 1) ? sm.y : sm.y2;          // v_{c-1}, w_{c-1} (zero at c = 0)
+        // [1] column c of the current matrix (one row per thread: n <= 116), its norm, alpha and d_c through ONE barrier
+        cplx a = mk(0.0, 0.0);
+        const int rc = c + tid;
+        if (rc < n) {
+            a = A[(size_t)c * ld + rc];
+            const cplx vr = Vp[rc], wr = Wp[rc], vc = Vp[c], wc = Wp[c];
+            a.x -= vr.x * wc.x + vr.y * wc.y + wr.x * vc.x + wr.y * vc.y;
+            a.y -= vr.y * wc.x - vr.x * wc.y + wr.y * vc.x - wr.x * vc.y;
+        }
+        double S = (rc >= c + 2 && rc < n) ? abs2(a) : 0.0;
         S = warp_sum(S);
         if (lane == 0) sm.red[warp] = S;
-        if (tid == 32) { const cplx al = A[(size_t)c * ld + c + 1]; sm.red[16] = al.x; sm.red[17] = al.y; sm.red[18] = A[(size_t)c * ld + c].x; }
+        if (tid == 1) { sm.red[16] = a.x; sm.red[17] = a.y; }
+        if (tid == 0) sm.red[18] = a.x;
         __syncthreads();
         S = 0.0;
 #pragma unroll
@@ -119,25 +136,38 @@ __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
         double beta; cplx tau, scale;
         med_householder(alpha, S, beta, tau, scale);
         if (tid == 0) { sm.d[c] = sm.red[18]; sm.e[c] = beta; sm.tau[c] = tau; }
-        for (int r = c + 1 + tid; r < n; r += kMedThreads) {
-            const cplx v = (r == c + 1) ? mk(1.0, 0.0) : scale * A[(size_t)c * ld + r];
-            sm.x[r] = v;
-            A[(size_t)c * ld + r] = v;
+        // [2] v_c into its vector and over column c (the reflector the back-transformation reads)
+        if (rc >= c + 1 && rc < n) {
+            const cplx v = (rc == c + 1) ? mk(1.0, 0.0) : scale * a;
+            X[rc] = v;
+            A[(size_t)c * ld + rc] = v;
         }
         __syncthreads();
-        if (tau.x == 0.0 && tau.y == 0.0) continue;        // H = I (block-uniform)
-        // y = A22 v : 64 rows per pass, 4 column classes per row (lane >> 3), reduced by shuffles
+        // [3] fused pass over the trailing block: A22 -= v' w'^H + w' v'^H (step c-1), y = A22 v (step c).
+        // 64 rows per round (8 per warp), 4 column classes per row (lane >> 3), reduced by shuffles
         cplx q = mk(0.0, 0.0);
-        for (int base = 0; base < m; base += 64) {
-            const int r = c + 1 + base + (lane & 7) + 8 * warp;
+        for (int base = 0; base < n; base += 64) {
+            const int r = base + (lane & 7) + 8 * warp;
+            if (base + 63 < c + 1) continue;                                            // block-uniform
+            const bool rok = (r >= c + 1 && r < n);
             cplx acc = mk(0.0, 0.0);
-            if (r < n)
-                for (int j = c + 1 + (lane >> 3); j < n; j += 4) cfma(acc, A[(size_t)j * ld + r], sm.x[j]);
+            if (rok) {
+                const cplx vr = Vp[r], wr = Wp[r];
+                for (int j = c + 1 + (lane >> 3); j < n; j += 4) {
+                    const cplx vj = Vp[j], wj = Wp[j];
+                    cplx e = A[(size_t)j * ld + r];
+                    e.x -= vr.x * wj.x + vr.y * wj.y + wr.x * vj.x + wr.y * vj.y;
+                    e.y -= vr.y * wj.x - vr.x * wj.y + wr.y * vj.x - wr.x * vj.y;
+                    if (r == j) e.y = 0.0;
+                    A[(size_t)j * ld + r] = e;
+                    cfma(acc, e, X[j]);
+                }
+            }
             acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
             acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
-            if (r < n && lane < 8) {
-                sm.y[r] = acc;
-                cfma_conj(q, sm.x[r], acc);                 // conj(v_r) y_r
+            if (rok && lane < 8) {
+                W[r] = acc;                                     // y_r for now
+                cfma_conj(q, X[r], acc);                        // conj(v_r) y_r
             }
         }
         // v^H y (real): partials in red[8..15], one barrier, which also publishes y
@@ -146,33 +176,20 @@ __device__ void med_tridiagonalize(const MedSmem &sm, int n, int ld) {
             if (lane == 0) sm.red[8 + warp] = qs;
         }
         __syncthreads();
+        // [4] w = tau y - 1/2 |tau|^2 (v^H y) v
         double qsum = 0.0;
 #pragma unroll
         for (int k = 0; k < kMedThreads / 32; ++k) qsum += sm.red[8 + k];
         const double alphap = -0.5 * abs2(tau) * qsum;      // v^H A v is real
-        for (int r = c + 1 + tid; r < n; r += kMedThreads) sm.y[r] = tau * sm.y[r] + alphap * sm.x[r];
-        __syncthreads();
-        // A22 -= v w^H + w v^H on the full trailing block: lane = row (its v_r, w_r stay in registers), warp = column
-        // class; no integer divisions, the column's v_j, w_j are broadcast loads
-        for (int rb = 0; rb < m; rb += 32) {
-            const int r = c + 1 + rb + lane;
-            const bool rok = r < n;
-            const cplx vr = rok ? sm.x[r] : mk(0.0, 0.0), wr = rok ? sm.y[r] : mk(0.0, 0.0);
-            for (int j = c + 1 + warp; j < n; j += kMedThreads / 32) {
-                const cplx vj = sm.x[j], wj = sm.y[j];
-                if (rok) {
-                    cplx a = A[(size_t)j * ld + r];
-                    // v_r conj(w_j) + w_r conj(v_j)
-                    a.x -= vr.x * wj.x + vr.y * wj.y + wr.x * vj.x + wr.y * vj.y;
-                    a.y -= vr.y * wj.x - vr.x * wj.y + wr.y * vj.x - wr.x * vj.y;
-                    if (r == j) a.y = 0.0;
-                    A[(size_t)j * ld + r] = a;
-                }
-            }
-        }
+        if (rc >= c + 1 && rc < n) W[rc] = tau * W[rc] + alphap * X[rc];
         __syncthreads();
     }
-    if (tid == 0) { sm.d[n - 1] = A[(size_t)(n - 1) * ld + n - 1].x; sm.e[n - 1] = 0.0; sm.tau[n - 1] = mk(0.0, 0.0); }
+    // the update of the last step on the last diagonal entry: v_{n-1} = 1 there
+    if (tid == 0) {
+        double dl = A[(size_t)(n - 1) * ld + n - 1].x;
+        if (n >= 2) { const cplx *Wl = ((n - 2) & 1) ? sm.y2 : sm.y; dl -= 2.0 * Wl[n - 1].x; }
+        sm.d[n - 1] = dl; sm.e[n - 1] = 0.0; sm.tau[n - 1] = mk(0.0, 0.0);
+    }
     __syncthreads();
 }
 
@@ -474,19 +491,20 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
                                                                  int *__restrict__ info, const int *__restrict__ info_idx) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ld = med_ld(n);
-    cplx *A = reinterpret_cast<cplx *>(smem_raw);               // n x ld reflectors
-    cplx *Wm = A + (size_t)n * ld;                               // n x ld kept eigenvectors
-    cplx *tau = Wm + (size_t)n * ld;                             // n
-    cplx *sv = tau + n;                                          // n : v^H W
+    // Only the kept eigenvectors live in shared memory; the reflectors stream from L2 (52 KB per matrix, each column read
+    // once) through a two-entry ring, one reflector ahead.  Half the shared memory of the first version (which also held
+    // the n x n reflector block): two CTAs per SM, so the 256 matrices of config 2 are resident at once instead of in two waves.
+    cplx *Wm = reinterpret_cast<cplx *>(smem_raw);              // n x ld kept eigenvectors
+    cplx *vb = Wm + (size_t)n * ld;                              // 2 x n : reflector ring
+    cplx *tau = vb + 2 * n;                                      // n
+    cplx *sv = tau + n;                                          // n : tau v^H W
     double *lm = reinterpret_cast<double *>(sv + n);             // n
     __shared__ int s_p0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, t = blockIdx.x;
     const cplx *Ag = w.Ar + (size_t)t * n * w.ld;
-    for (int q = tid; q < n * n; q += kMedThreads) {
-        const int j = q / n, i = q % n;
-        if (i > j) A[(size_t)j * ld + i] = Ag[(size_t)j * w.ld + i];
-    }
     for (int i = tid; i < n; i += kMedThreads) { tau[i] = w.tau[(size_t)t * n + i]; lm[i] = lam[(size_t)t * n + i]; }
+    if (n >= 2)
+        for (int r = n - 1 + tid; r < n; r += kMedThreads) vb[((n - 2) & 1) * n + r] = Ag[(size_t)(n - 2) * w.ld + r];     // reflector n-2: one entry
     __syncthreads();
     if (tau[n - 1].x != tau[n - 1].x) {        // flag of meddc_tridiag_kernel: non-finite input (block-uniform)
         io_fill_nan(io, (size_t)offs[t], n, tid, kMedThreads);
@@ -503,35 +521,47 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
     const int p0 = s_p0, kpos = n - p0;
     // S6: W = Z_+ diag(sqrt(lambda_+)), real -> complex
     const double *Zt = Z + (size_t)t * n * ldz;
-    for (int q = tid; q < kpos * n; q += kMedThreads) {
-        const int j = q / n, r = q % n;
-        Wm[(size_t)j * ld + r] = mk(sqrt(lm[p0 + j]) * Zt[(size_t)(p0 + j) * ldz + r], 0.0);
+    for (int j = warp; j < kpos; j += kMedThreads / 32) {
+        const double sq = sqrt(lm[p0 + j]);
+        for (int r = lane; r < n; r += 32) Wm[(size_t)j * ld + r] = mk(sq * Zt[(size_t)(p0 + j) * ldz + r], 0.0);
     }
     __syncthreads();
     // S5: W <- H_0 H_1 ... H_{n-2} W, last reflector first
     for (int k = n - 2; k >= 0; --k) {
         const cplx tk = tau[k];
-        if (tk.x == 0.0 && tk.y == 0.0) continue;                // block-uniform
-        for (int base = 0; base < kpos; base += 64) {
-            const int j = base + (lane & 7) + 8 * warp;
-            cplx acc = mk(0.0, 0.0);
-            if (j < kpos)
-                for (int r = k + 1 + (lane >> 3); r < n; r += 4) cfma_conj(acc, A[(size_t)k * ld + r], Wm[(size_t)j * ld + r]);
-            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
-            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
-            if (j < kpos && lane < 8) sv[j] = tk * acc;
+        const cplx *vk = vb + (k & 1) * n;
+        // the next reflector (column k-1, rows k..n-1) is on its way while this one is applied; at most 83 entries
+        cplx pre = mk(0.0, 0.0);
+        const int rp = k + tid;
+        const bool has_pre = (k > 0 && rp < n);
+        if (has_pre) pre = Ag[(size_t)(k - 1) * w.ld + rp];
+        if (!(tk.x == 0.0 && tk.y == 0.0)) {                      // block-uniform
+            for (int base = 0; base < kpos; base += 64) {
+                const int j = base + (lane & 7) + 8 * warp;
+                cplx acc = mk(0.0, 0.0);
+                if (j < kpos)
+                    for (int r = k + 1 + (lane >> 3); r < n; r += 4) cfma_conj(acc, vk[r], Wm[(size_t)j * ld + r]);
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+                if (j < kpos && lane < 8) sv[j] = tk * acc;
+            }
+            __syncthreads();
+            // W[r, j] -= v_r s_j : lane = row, warp = column class (no integer divisions, v_r stays in a register)
+            for (int rb = k + 1; rb < n; rb += 32) {
+                const int r = rb + lane;
+                if (r < n) {
+                    const cplx v = vk[r];
+                    for (int j = warp; j < kpos; j += kMedThreads / 32) {
+                        const cplx sj = sv[j];
+                        cplx x = Wm[(size_t)j * ld + r];
+                        x.x -= v.x * sj.x - v.y * sj.y;
+                        x.y -= v.x * sj.y + v.y * sj.x;
+                        Wm[(size_t)j * ld + r] = x;
+                    }
+                }
+            }
         }
-        __syncthreads();
-        const int m = n - k - 1;
-        for (int q = tid; q < m * kpos; q += kMedThreads) {
-            const int rr = q % m, j = q / m;
-            const int r = k + 1 + rr;
-            const cplx v = A[(size_t)k * ld + r], s = sv[j];
-            cplx x = Wm[(size_t)j * ld + r];
-            x.x -= v.x * s.x - v.y * s.y;
-            x.y -= v.x * s.y + v.y * s.x;
-            Wm[(size_t)j * ld + r] = x;
-        }
+        if (has_pre) vb[((k - 1) & 1) * n + rp] = pre;
         __syncthreads();
     }
     // S7 + S8
@@ -556,7 +586,7 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
 }
 
 static size_t meddc_back_smem(int n) {
-    return sizeof(cplx) * (2 * (size_t)n * med_ld(n) + 2 * (size_t)n) + sizeof(double) * n + 64;
+    return sizeof(cplx) * ((size_t)n * med_ld(n) + 4 * (size_t)n) + sizeof(double) * n + 64;
 }
 
 static int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
