@@ -108,16 +108,29 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
     for (int l = 0; l < m; ++l) {
         int iter = 0;
         for (;;) {
-            if (lane == 0) {
-                int mm;
-                for (mm = l; mm < m - 1; ++mm) {
-                    const double s = fabs(dd[mm]) + fabs(dd[mm + 1]);
-                    if (fabs(ee[mm]) <= kEps * s || fabs(ee[mm]) <= kEps * an) break;
+            // first negligible off-diagonal entry at or after l: every lane tests its own entry, one ballot (the serial scan by
+            // lane 0 cost ~30 cycles per entry at the head of every QL iteration)
+            int mm;
+            {
+                bool small = false;
+                if (lane < m - 1) {
+                    const double ae = fabs(ee[lane]);
+                    small = ae <= kEps * (fabs(dd[lane]) + fabs(dd[lane + 1])) || ae <= kEps * an;
                 }
+                const unsigned hit = __ballot_sync(0xffffffffu, small) & (0xffffffffu << l);
+                mm = hit ? __ffs(hit) - 1 : m - 1;
+            }
+            if (lane == 0) {
                 int ilo = l;
                 if (mm != l) {
                     double g = (dd[l + 1] - dd[l]) / (2.0 * ee[l]);
-                    double r = hypot(g, 1.0);
+                    double r;
+                    if (fabs(g) < 1e150) {                      // sqrt(g^2 + 1) from a refined reciprocal square root
+                        const double x = fma(g, g, 1.0);
+                        double ix = rsqrt(x);
+                        ix = ix * fma(-0.5 * x * ix, ix, 1.5);
+                        r = x * ix;
+                    } else r = fabs(g);
                     g = dd[mm] - dd[l] + ee[l] / (g + copysign(r, g));
                     double s = 1.0, c = 1.0, p = 0.0;
                     int i;
@@ -153,10 +166,10 @@ __global__ void __launch_bounds__(32) stedc_leaf_kernel(int n, int depth, const 
                     if (under) ilo = i + 1;
                     else { dd[l] -= p; ee[l] = g; ee[mm] = 0.0; }
                 }
-                ctrl[0] = mm; ctrl[1] = ilo;
+                ctrl[1] = ilo;
             }
             __syncwarp();
-            const int mm = ctrl[0], ilo = ctrl[1];
+            const int ilo = ctrl[1];
             if (mm == l) break;
             if (++iter > 80) { fail = true; break; }
             if (lane < m && mm - 1 >= ilo) {
