@@ -447,10 +447,20 @@ __global__ void __launch_bounds__(256) stedc_gather_kernel(MergeArgs a) {
 // g(mu) = 1 + rho sum_j z_j^2 / (delta_j - mu),  delta_j = d_j - d_org,  lambda = d_org + mu.
 struct SecEval { double g, psi, dpsi, phi, dphi, asum; };
 
-__device__ __forceinline__ SecEval sec_eval(int K, int i, int org, double mu, double rho, const double *__restrict__ d, const double *__restrict__ z, int lane) {
+// sum over the GL lanes of a group (GL = 32: the warp; GL = 8: a quarter warp, mask = the group's lanes: groups of one warp
+// diverge freely, a shuffle only names its own group)
+template <int GL>
+__device__ __forceinline__ double group_sum(double v, unsigned mask) {
+#pragma unroll
+    for (int o = GL / 2; o > 0; o >>= 1) v += __shfl_xor_sync(mask, v, o);
+    return v;
+}
+
+template <int GL>
+__device__ __forceinline__ SecEval sec_eval(int K, int i, int org, double mu, double rho, const double *__restrict__ d, const double *__restrict__ z, int lane, unsigned mask) {
     double psi = 0.0, dpsi = 0.0, phi = 0.0, dphi = 0.0, asum = 0.0;
     const double dorg = d[org];
-    for (int j = lane; j < K; j += 32) {
+    for (int j = lane; j < K; j += GL) {
         const double del = (d[j] - dorg) - mu;
         const double t = z[j] / del;
         const double term = rho * z[j] * t, dterm = rho * t * t;
@@ -458,7 +468,8 @@ __device__ __forceinline__ SecEval sec_eval(int K, int i, int org, double mu, do
         asum += fabs(term);
     }
     SecEval r;
-    r.psi = warp_sum(psi); r.dpsi = warp_sum(dpsi); r.phi = warp_sum(phi); r.dphi = warp_sum(dphi); r.asum = warp_sum(asum);
+    r.psi = group_sum<GL>(psi, mask); r.dpsi = group_sum<GL>(dpsi, mask); r.phi = group_sum<GL>(phi, mask); r.dphi = group_sum<GL>(dphi, mask);
+    r.asum = group_sum<GL>(asum, mask);
     r.g = 1.0 + r.psi + r.phi;
     return r;
 }
@@ -484,12 +495,16 @@ __device__ __forceinline__ bool two_pole_step(double c, double s, double S, doub
     return (eta > D1 && eta < D2) && (eta == eta);
 }
 
+// GL lanes per root: a warp for large nodes; a quarter warp for nodes of at most 128 poles (the batched medium path: a root's
+// iteration is a latency chain, four roots per warp keep four times as many chains in flight)
+template <int GL>
 __global__ void __launch_bounds__(256) stedc_secular_kernel(MergeArgs a) {
     const int node = blockIdx.y;
     const int lo = node_bound(a.n, a.depth, node);
     const int K = a.nodeinfo[8 * node];
-    const int lane = threadIdx.x & 31;
-    const int i = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & (GL - 1);
+    const unsigned mask = (GL == 32) ? 0xffffffffu : (((1u << GL) - 1u) << ((threadIdx.x & 31) & ~(GL - 1)));
+    const int i = blockIdx.x * (256 / GL) + (threadIdx.x / GL);
     if (i >= K) return;
     const double *d = a.dt + lo, *z = a.zt + lo;
     const double rho = a.rho[node];
@@ -501,7 +516,7 @@ __global__ void __launch_bounds__(256) stedc_secular_kernel(MergeArgs a) {
     }
     if (!last) {
         const double gap = d[i + 1] - d[i];
-        const SecEval m = sec_eval(K, i, i, 0.5 * gap, rho, d, z, lane);
+        const SecEval m = sec_eval<GL>(K, i, i, 0.5 * gap, rho, d, z, lane, mask);
         const double ti = rho * z[i] * z[i], ti1 = rho * z[i + 1] * z[i + 1];
         const double c0 = m.g - (-2.0 * ti / gap) - (2.0 * ti1 / gap);
         double D1, D2;
@@ -512,8 +527,8 @@ __global__ void __launch_bounds__(256) stedc_secular_kernel(MergeArgs a) {
         else mu = 0.5 * (blo + bhi);
     } else {
         double zz = 0.0;
-        for (int j = lane; j < K; j += 32) zz += z[j] * z[j];
-        zz = warp_sum(zz);
+        for (int j = lane; j < K; j += GL) zz += z[j] * z[j];
+        zz = group_sum<GL>(zz, mask);
         org = K - 1; blo = 0.0; bhi = rho * zz;
         if (!(bhi > 0.0)) bhi = 1.0;
         // g at the upper bound is >= 0; start in the middle
@@ -521,7 +536,7 @@ __global__ void __launch_bounds__(256) stedc_secular_kernel(MergeArgs a) {
     }
     bool ok = false;
     for (int it = 0; it < 100; ++it) {
-        const SecEval ev = sec_eval(K, i, org, mu, rho, d, z, lane);
+        const SecEval ev = sec_eval<GL>(K, i, org, mu, rho, d, z, lane, mask);
         if (ev.g < 0.0) blo = mu; else bhi = mu;
         const double err = kEps * (8.0 * (1.0 + ev.asum) + fabs(mu) * (ev.dpsi + ev.dphi));
         if (fabs(ev.g) <= err || !(ev.g == ev.g)) { ok = (ev.g == ev.g); break; }
@@ -550,24 +565,26 @@ __global__ void __launch_bounds__(256) stedc_secular_kernel(MergeArgs a) {
 }
 
 // ---- M4: z^ (Loewner / Gu-Eisenstat) and final sorted positions ------------------------------
+template <int GL>
 __global__ void __launch_bounds__(256) stedc_zhat_kernel(MergeArgs a) {
     const int node = blockIdx.y;
     const int lo = node_bound(a.n, a.depth, node), hi = node_bound(a.n, a.depth, node + 1);
     const int N = hi - lo;
     const int *ni = a.nodeinfo + 8 * node;
     const int K = ni[0], ndefl = ni[5];
-    const int lane = threadIdx.x & 31;
-    const int j = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & (GL - 1);
+    const unsigned mask = (GL == 32) ? 0xffffffffu : (((1u << GL) - 1u) << ((threadIdx.x & 31) & ~(GL - 1)));
+    const int j = blockIdx.x * (256 / GL) + (threadIdx.x / GL);
     const double *d = a.dt + lo;
     if (j < K) {
         double p = 1.0;
         const double dj = d[j];
-        for (int i = lane; i < K; i += 32) {
+        for (int i = lane; i < K; i += GL) {
             const double del = (dj - d[a.org[lo + i]]) - a.mu[lo + i];      // d_j - lambda_i
             p *= (i == j) ? -del : del / (dj - d[i]);
         }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) p *= __shfl_xor_sync(0xffffffffu, p, o);
+        for (int o = GL / 2; o > 0; o >>= 1) p *= __shfl_xor_sync(mask, p, o);
         if (lane == 0) a.zhat[lo + j] = copysign(sqrt(fabs(p)), a.zt[lo + j]);
     }
     // positions: thread t of the first CTAs handles element t
@@ -585,29 +602,31 @@ __global__ void __launch_bounds__(256) stedc_zhat_kernel(MergeArgs a) {
 }
 
 // ---- M5: secular eigenvectors U (rows in grouped order) and copy of the deflated columns ------
+template <int GL>
 __global__ void __launch_bounds__(256) stedc_form_u_kernel(MergeArgs a) {
     const int node = blockIdx.y;
     const int lo = node_bound(a.n, a.depth, node), hi = node_bound(a.n, a.depth, node + 1);
     const int N = hi - lo;
     const int *ni = a.nodeinfo + 8 * node;
     const int K = ni[0], ndefl = ni[5];
-    const int lane = threadIdx.x & 31;
-    const int w = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & (GL - 1);
+    const unsigned mask = (GL == 32) ? 0xffffffffu : (((1u << GL) - 1u) << ((threadIdx.x & 31) & ~(GL - 1)));
+    const int w = blockIdx.x * (256 / GL) + (threadIdx.x / GL);
     const double *d = a.dt + lo;
     if (w < K) {
         const int i = w;
         const double dorg = d[a.org[lo + i]], mu = a.mu[lo + i];
         double ss = 0.0;
-        for (int j = lane; j < K; j += 32) { const double u = a.zhat[lo + j] / ((d[j] - dorg) - mu); ss += u * u; }
-        ss = warp_sum(ss);
+        for (int j = lane; j < K; j += GL) { const double u = a.zhat[lo + j] / ((d[j] - dorg) - mu); ss += u * u; }
+        ss = group_sum<GL>(ss, mask);
         const double inv = 1.0 / sqrt(ss);
         double *Ucol = a.U + (size_t)(lo + i) * a.ldz + row_off(lo, a.blk);
-        for (int j = lane; j < K; j += 32) Ucol[a.grow[lo + j]] = inv * (a.zhat[lo + j] / ((d[j] - dorg) - mu));
+        for (int j = lane; j < K; j += GL) Ucol[a.grow[lo + j]] = inv * (a.zhat[lo + j] / ((d[j] - dorg) - mu));
     } else if (w - K < ndefl && w < N) {
         const int m = w - K;
         const double *src = a.Zin + (size_t)(lo + a.dcol[lo + m]) * a.ldz + row_off(lo, a.blk);
         double *dst = a.Zout + (size_t)(lo + a.dest_defl[lo + m]) * a.ldz + row_off(lo, a.blk);
-        for (int r = lane; r < N; r += 32) dst[r] = src[r];
+        for (int r = lane; r < N; r += GL) dst[r] = src[r];
     }
 }
 
@@ -678,17 +697,23 @@ int launch_stedc(const StedcWs &w, const double *d, const double *e, double **la
         a.rc = w.rc; a.rs = w.rs; a.rho = w.rho;
         a.org = w.org; a.grow = w.grow; a.gsrc = w.gsrc; a.dcol = w.dcol; a.dest_root = w.dest_root; a.dest_defl = w.dest_defl;
         a.rp = w.rp; a.rq = w.rq; a.nodeinfo = w.nodeinfo; a.info = w.info;
+        // a quarter warp per root / column in the secular, z^ and U kernels: pays when a level holds many small nodes (the
+        // batched medium path: 20736 roots per level in config 2); with few roots a whole warp per root has the shorter chain
+        const bool quarter = maxN <= 128 && (long long)nodes * maxN >= 8192;
         stedc_merge_setup_kernel<<<nodes, 256, (size_t)24 * maxN, st>>>(a);
         HPSD_LAUNCH_CHECK();
         stedc_rotate_kernel<<<dim3((maxN + 255) / 256, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
         stedc_gather_kernel<<<dim3((maxN + 255) / 256, (maxN + kGatherCols - 1) / kGatherCols, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
-        stedc_secular_kernel<<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
+        if (quarter) stedc_secular_kernel<8><<<dim3((maxN + 31) / 32, nodes), 256, 0, st>>>(a);
+        else stedc_secular_kernel<32><<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
-        stedc_zhat_kernel<<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
+        if (quarter) stedc_zhat_kernel<8><<<dim3((maxN + 31) / 32, nodes), 256, 0, st>>>(a);
+        else stedc_zhat_kernel<32><<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
-        stedc_form_u_kernel<<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
+        if (quarter) stedc_form_u_kernel<8><<<dim3((maxN + 31) / 32, nodes), 256, 0, st>>>(a);
+        else stedc_form_u_kernel<32><<<dim3((maxN + 7) / 8, nodes), 256, 0, st>>>(a);
         HPSD_LAUNCH_CHECK();
         const int mt = (maxN / 2 + 1 + 63) / 64, nt = (maxN + 63) / 64;
         stedc_gemm_kernel<<<dim3(mt, nt, 2 * nodes), DG_WM * DG_WN * 32, kStedcGemmSmem, st>>>(a);
