@@ -492,19 +492,17 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ld = med_ld(n);
     // Only the kept eigenvectors live in shared memory; the reflectors stream from L2 (52 KB per matrix, each column read
-    // once) through a two-entry ring, one reflector ahead.  Half the shared memory of the first version (which also held
+    // once), two at a time, one pair ahead in registers.  Half the shared memory of the first version (which also held
     // the n x n reflector block): two CTAs per SM, so the 256 matrices of config 2 are resident at once instead of in two waves.
     cplx *Wm = reinterpret_cast<cplx *>(smem_raw);              // n x ld kept eigenvectors
-    cplx *vb = Wm + (size_t)n * ld;                              // 2 x n : reflector ring
+    cplx *vb = Wm + (size_t)n * ld;                              // 2 x n : the two reflectors in work
     cplx *tau = vb + 2 * n;                                      // n
-    cplx *sv = tau + n;                                          // n : tau v^H W
-    double *lm = reinterpret_cast<double *>(sv + n);             // n
+    cplx *sv = tau + n;                                          // 2 x n : x_k, x_{k-1}
+    double *lm = reinterpret_cast<double *>(sv + 2 * n) + 16;    // n (behind the 16 reduction slots)
     __shared__ int s_p0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, t = blockIdx.x;
     const cplx *Ag = w.Ar + (size_t)t * n * w.ld;
     for (int i = tid; i < n; i += kMedThreads) { tau[i] = w.tau[(size_t)t * n + i]; lm[i] = lam[(size_t)t * n + i]; }
-    if (n >= 2)
-        for (int r = n - 1 + tid; r < n; r += kMedThreads) vb[((n - 2) & 1) * n + r] = Ag[(size_t)(n - 2) * w.ld + r];     // reflector n-2: one entry
     __syncthreads();
     if (tau[n - 1].x != tau[n - 1].x) {        // flag of meddc_tridiag_kernel: non-finite input (block-uniform)
         io_fill_nan(io, (size_t)offs[t], n, tid, kMedThreads);
@@ -526,42 +524,71 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
         for (int r = lane; r < n; r += 32) Wm[(size_t)j * ld + r] = mk(sq * Zt[(size_t)(p0 + j) * ldz + r], 0.0);
     }
     __syncthreads();
-    // S5: W <- H_0 H_1 ... H_{n-2} W, last reflector first
-    for (int k = n - 2; k >= 0; --k) {
-        const cplx tk = tau[k];
-        const cplx *vk = vb + (k & 1) * n;
-        // the next reflector (column k-1, rows k..n-1) is on its way while this one is applied; at most 83 entries
-        cplx pre = mk(0.0, 0.0);
-        const int rp = k + tid;
-        const bool has_pre = (k > 0 && rp < n);
-        if (has_pre) pre = Ag[(size_t)(k - 1) * w.ld + rp];
-        if (!(tk.x == 0.0 && tk.y == 0.0)) {                      // block-uniform
-            for (int base = 0; base < kpos; base += 64) {
-                const int j = base + (lane & 7) + 8 * warp;
-                cplx acc = mk(0.0, 0.0);
-                if (j < kpos)
-                    for (int r = k + 1 + (lane >> 3); r < n; r += 4) cfma_conj(acc, vk[r], Wm[(size_t)j * ld + r]);
-                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);  acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
-                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
-                if (j < kpos && lane < 8) sv[j] = tk * acc;
+    // S5: W <- H_0 H_1 ... H_{n-2} W, last reflector first, TWO reflectors per pass over W:
+    //   H_{k-1} H_k W = W - v_k x_k - v_{k-1} x_{k-1},  x_k = tau_k v_k^H W,  x_{k-1} = tau_{k-1} (v_{k-1}^H W - (v_{k-1}^H v_k) x_k),
+    // so W is read twice and written once per PAIR (the kernel is bound by shared-memory bandwidth) with three block
+    // barriers per pair.  The next pair is on its way from L2 (one row per thread, in registers) while this one is applied.
+    cplx *v0 = vb, *v1 = vb + n;                                 // v_k, v_{k-1}: rows >= k, zero where the reflector has no entry
+    double *red = reinterpret_cast<double *>(sv + 2 * n);        // 16 : partials of v_{k-1}^H v_k
+    auto fetch = [&](int k, cplx &a, cplx &b) {                  // row tid of reflectors k and k-1
+        a = mk(0.0, 0.0); b = mk(0.0, 0.0);
+        if (tid < n && k >= 0) {
+            if (tid >= k + 1) a = Ag[(size_t)k * w.ld + tid];
+            if (k >= 1 && tid >= k) b = Ag[(size_t)(k - 1) * w.ld + tid];
+        }
+    };
+    cplx pa, pb;
+    fetch(n - 2, pa, pb);
+    for (int k = n - 2; k >= 0; k -= 2) {
+        const cplx tk = tau[k], tk1 = (k >= 1) ? tau[k - 1] : mk(0.0, 0.0);
+        // [a] the pair into shared memory, v_{k-1}^H v_k, and the next pair's loads issued
+        if (tid < n) { v0[tid] = pa; v1[tid] = pb; }
+        {
+            cplx gp = mk(0.0, 0.0);
+            cfma_conj(gp, pb, pa);
+            gp = warp_sum(gp);
+            if (lane == 0) { red[2 * warp] = gp.x; red[2 * warp + 1] = gp.y; }
+        }
+        fetch(k - 2, pa, pb);
+        __syncthreads();
+        cplx g = mk(0.0, 0.0);
+#pragma unroll
+        for (int q = 0; q < kMedThreads / 32; ++q) { g.x += red[2 * q]; g.y += red[2 * q + 1]; }
+        // [b] s_k = v_k^H W, s_{k-1} = v_{k-1}^H W per kept column: 8 columns per warp, 4 row classes per column
+        for (int base = 0; base < kpos; base += 64) {
+            const int j = base + (lane & 7) + 8 * warp;
+            cplx a0 = mk(0.0, 0.0), a1 = mk(0.0, 0.0);
+            if (j < kpos)
+                for (int r = k + (lane >> 3); r < n; r += 4) {
+                    const cplx x = Wm[(size_t)j * ld + r];
+                    cfma_conj(a0, v0[r], x);
+                    cfma_conj(a1, v1[r], x);
+                }
+            a0.x += __shfl_xor_sync(0xffffffffu, a0.x, 8);  a0.y += __shfl_xor_sync(0xffffffffu, a0.y, 8);
+            a1.x += __shfl_xor_sync(0xffffffffu, a1.x, 8);  a1.y += __shfl_xor_sync(0xffffffffu, a1.y, 8);
+            a0.x += __shfl_xor_sync(0xffffffffu, a0.x, 16); a0.y += __shfl_xor_sync(0xffffffffu, a0.y, 16);
+            a1.x += __shfl_xor_sync(0xffffffffu, a1.x, 16); a1.y += __shfl_xor_sync(0xffffffffu, a1.y, 16);
+            if (j < kpos && lane < 8) {
+                const cplx xk = tk * a0;
+                sv[j] = xk;
+                sv[n + j] = tk1 * (a1 - g * xk);
             }
-            __syncthreads();
-            // W[r, j] -= v_r s_j : lane = row, warp = column class (no integer divisions, v_r stays in a register)
-            for (int rb = k + 1; rb < n; rb += 32) {
-                const int r = rb + lane;
-                if (r < n) {
-                    const cplx v = vk[r];
-                    for (int j = warp; j < kpos; j += kMedThreads / 32) {
-                        const cplx sj = sv[j];
-                        cplx x = Wm[(size_t)j * ld + r];
-                        x.x -= v.x * sj.x - v.y * sj.y;
-                        x.y -= v.x * sj.y + v.y * sj.x;
-                        Wm[(size_t)j * ld + r] = x;
-                    }
+        }
+        __syncthreads();
+        // [c] W[r, j] -= v_k[r] x_k[j] + v_{k-1}[r] x_{k-1}[j] : lane = row, warp = column class
+        for (int rb = k; rb < n; rb += 32) {
+            const int r = rb + lane;
+            if (r < n) {
+                const cplx va = v0[r], vc = v1[r];
+                for (int j = warp; j < kpos; j += kMedThreads / 32) {
+                    const cplx xa = sv[j], xb = sv[n + j];
+                    cplx x = Wm[(size_t)j * ld + r];
+                    x.x -= va.x * xa.x - va.y * xa.y + vc.x * xb.x - vc.y * xb.y;
+                    x.y -= va.x * xa.y + va.y * xa.x + vc.x * xb.y + vc.y * xb.x;
+                    Wm[(size_t)j * ld + r] = x;
                 }
             }
         }
-        if (has_pre) vb[((k - 1) & 1) * n + rp] = pre;
         __syncthreads();
     }
     // S7 + S8
@@ -586,7 +613,7 @@ __global__ void __launch_bounds__(kMedThreads) meddc_back_kernel(int n, const lo
 }
 
 static size_t meddc_back_smem(int n) {
-    return sizeof(cplx) * ((size_t)n * med_ld(n) + 4 * (size_t)n) + sizeof(double) * n + 64;
+    return sizeof(cplx) * ((size_t)n * med_ld(n) + 5 * (size_t)n) + sizeof(double) * (n + 16) + 64;
 }
 
 static int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
